@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- plans/s of the gL-BFGS hot path (BASELINE.json metric) on N B200s of one node.
+
+A "step" is one pass of the whole hot path over one synthetic plan pool: gmco_create (a0),
+gmco_optimize (a1-a7), gmco_result (a8), gmco_destroy.  The workload at N = 1 is BASELINE.json
+configs[2] ("gMCO production": 252 dwell positions, 12000 points, K = 1000 plans, m = 10, 200
+iterations) -- the configuration the metric ("at K = 1000") is quoted on.  With N > 1 every rank
+optimises its own 1000-plan pool (plans are independent: K-sharding, no data-path collective,
+weak scaling).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C3]
+                  [--precision tf32x3|simt]
+
+Prints ONE JSON line on rank 0 (see DESIGN.md section 6 for every key).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import gmco_cases as gc  # noqa: E402
+
+METRIC, UNIT = "plans_per_s", "plans/s"
+
+
+def env_int(name, default):
+    return int(os.environ.get(name, default))
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm_gbs=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
+                    source="measured")
+    return dict(hbm_gbs=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_leg(case, sample_plans):
+    """The fp64 oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    import oracle
+    oracle.build()
+    w = case.weights[:sample_plans]
+    t0 = time.perf_counter()
+    oracle.optimize(case.D, case.structures, case.rx, case.T0, w, m=case.m, iters=case.iters)
+    dt = time.perf_counter() - t0
+    return sample_plans / dt, dt, oracle.num_threads()
+
+
+def run_reference(args, case):
+    rank = env_int("RANK", 0)
+    if rank != 0:
+        return
+    sample = args.ref_sample
+    vals = []
+    for i in range(args.warmup + args.steps):
+        v, dt, cores = oracle_leg(case, sample)
+        if i >= args.warmup:
+            vals.append((v, dt))
+    value = float(np.mean([v for v, _ in vals]))
+    ms = float(np.mean([dt for _, dt in vals]) * 1e3)
+    desc = f"{sample} of {case.n_plans} plans of {case.name}, full {case.iters} iterations, OpenMP over plans"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "plan_iterations_per_s": value * case.iters,
+        "config": workload_config(case, args, None),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def workload_config(case, args, stats):
+    cfg = {"workload": f"{case.name}: BASELINE.json configs[{['C1','C2','C3','C4'].index(case.name)}]",
+           "n_points": case.n_points, "n_dwell": case.n_dwell, "plans_per_gpu": case.n_plans, "m": case.m,
+           "iters": case.iters, "step": "gmco_create + gmco_optimize + gmco_result + gmco_destroy",
+           "l2": "flushed between timed steps (512 MiB write)", "parallelism": f"k-shard x{args.gpus}"}
+    if stats:
+        cfg["rounds"] = stats["rounds"]
+        cfg["device_bytes"] = stats["device_bytes"]
+    return cfg
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--precision", default="tf32x3", choices=["tf32x3", "simt"])
+    ap.add_argument("--ref-sample", type=int, default=32, help="plans per oracle step (bounded sample)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    case = gc.make_case(args.config, seed_weights=7 + rank)
+
+    if args.impl == "reference":
+        run_reference(args, case)
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_1904_01567_b200 import build
+    build.build()
+    import paper_1904_01567_b200 as g
+
+    prec = g.GMCO_PREC_TF32X3 if args.precision == "tf32x3" else g.GMCO_PREC_SIMT_FP32
+    K, A, S, N = case.n_plans, case.n_dwell, case.n_structs, case.n_points
+    stream = torch.cuda.current_stream()
+    D_dev = torch.from_numpy(case.D).cuda(); T0_dev = torch.from_numpy(case.T0).cuda()
+    w_dev = torch.from_numpy(case.weights).cuda()
+    D_pin = torch.from_numpy(case.D).pin_memory(); T0_pin = torch.from_numpy(case.T0).pin_memory()
+    w_pin = torch.from_numpy(case.weights).pin_memory()
+    out_pin = {k: torch.empty(s, dtype=dt).pin_memory() for k, s, dt in
+               (("T", (K, A), torch.float32), ("F", (K,), torch.float32), ("dvh", (K, S), torch.float32),
+                ("terms", (K, S, 2), torch.float32), ("it", (K,), torch.int32), ("st", (K,), torch.int32))}
+    out_dev = {k: torch.empty_like(v, device="cuda") for k, v in out_pin.items()}
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    L = g.lib()
+    last = {}
+
+    def step(host: bool, profile: bool = False):
+        Dm, Tm, wm, om = (D_pin, T0_pin, w_pin, out_pin) if host else (D_dev, T0_dev, w_dev, out_dev)
+        opt = g.binding.make_options(m=case.m, precision=prec)
+        opt.reserved[0] = 1 if profile else 0
+        h = g.gmco_create(Dm, case.structures, case.rx, opt, stream)
+        try:
+            g.gmco_optimize(h, Tm, wm, case.iters, stream)
+            g.binding._check(L.gmco_result(h.ptr, om["T"].data_ptr(), om["F"].data_ptr(), om["dvh"].data_ptr(),
+                                           om["terms"].data_ptr(), om["it"].data_ptr(), om["st"].data_ptr()), h)
+            last["stats"] = g.gmco_get_stats(h)
+        finally:
+            g.gmco_destroy(h)
+
+    def timed(host, steps, profile=False):
+        tot = 0.0
+        for _ in range(steps):
+            flush.fill_(1)                                   # evict L2 between timed steps
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); step(host, profile); e1.record(stream)
+            e1.synchronize()
+            tot += e0.elapsed_time(e1)
+        return tot
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    for _ in range(args.warmup):
+        step(False); step(True)
+    barrier()
+    with ClockSampler(local) as clk:
+        ms_dev = timed(False, args.steps)
+        barrier()
+    ms_dev = max_over_ranks(ms_dev)
+    stats = dict(last["stats"])
+    barrier()
+    ms_e2e = max_over_ranks(timed(True, args.steps))
+    barrier()
+    # roofline leg: same steps with per-launch CUDA events around the contraction kernel (in-library)
+    prof = None
+    if rank == 0:
+        timed(False, min(args.steps, 3), profile=True)
+        prof = dict(last["stats"])
+    barrier()
+
+    value = world * K * args.steps / (ms_dev * 1e-3)
+    e2e_value = world * K * args.steps / (ms_e2e * 1e-3)
+    h2d = case.D.nbytes + case.T0.nbytes + case.weights.nbytes
+    d2h = sum(v.numel() * v.element_size() for v in out_pin.values())
+
+    if rank == 0:
+        peaks = load_peaks()
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "tf32x3" if prec == g.GMCO_PREC_TF32X3 else "f32", "data": "synthetic",
+            "plan_iterations_per_s": value * case.iters,
+            "config": workload_config(case, args, stats),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(stats["kernel_launches"] * args.steps),
+            "clocks": clk.summary(),
+            "paper_context": "gL-BFGS 0.9 ms/plan = ~1111 plans/s on a Titan X (Pascal), real cases, eps=1e-3 (PAPER.md:180)",
+        }
+        line["roofline"] = roofline(case, prec, g, prof, peaks)
+        if not args.no_cpu_baseline:
+            v, dt, cores = oracle_leg(case, args.ref_sample)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{args.ref_sample} of {K} plans of {case.name}, full {case.iters} "
+                                              f"iterations, {dt:.1f} s, OpenMP over plans"}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def roofline(case, prec, g, prof, peaks):
+    """Dominant kernel = the contraction (fused dose+penalty+gradient) kernel.
+    Algorithmic flops per launch = 4 N A K (one D t and one D^T r per plan); the 3xTF32
+    split issues 3x that on the tensor pipe.  Peak: measured bf16 (sustained: the kernel runs inside a
+    long step) x the guide's nominal tf32/bf16 ratio 1.1/2.25; SIMT: 148 SM x 128 lanes x 2 x 1.965 GHz."""
+    if not prof or not prof.get("reserved_eval_launches"):
+        return None
+    flops = 4.0 * case.n_points * case.n_dwell * case.n_plans
+    ms = prof["reserved_eval_ms"] / prof["reserved_eval_launches"]
+    if prec == g.GMCO_PREC_TF32X3:
+        peak = peaks["bf16_sustained"] * (1.1 / 2.25)
+        issued = 3.0 * flops / (ms * 1e-3) / 1e12
+        return {"bound": "tensor", "kernel": "k_fused_tc (dose GEMM + penalty + gradient GEMM)",
+                "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
+                "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["reserved_eval_launches"],
+                "peak_source": f"{peaks['source']} bf16 sustained x 1.1/2.25 (nominal tf32:bf16)", "traffic": None}
+    peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    ach = flops / (ms * 1e-3) / 1e12
+    return {"bound": "alu", "kernel": "k_simt_dose + k_simt_grad", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+            "frac": ach / peak, "avg_launch_ms": ms, "launches": prof["reserved_eval_launches"],
+            "peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": None}
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,153 @@
+/* gmco.h -- C ABI of libgmco: the gL-BFGS hot path of gMCO (arXiv 1904.01567) on one B200.
+ *
+ * The library optimises K HDR-brachytherapy plans in parallel.  Every plan shares the
+ * dose-rate matrix D and the structure table and has its own hidden weights
+ * (Eq. 4).  One "round" on the device is
+ *     dose  d = D t, t = x o x            PAPER.md:55-59  (Eq. 1, dwell weights x = sqrt(t))
+ *     penalty f, derivative r = dF/dd     PAPER.md:61-66  (Eq. 2)
+ *     objective F = sum_j w_j mean_i f    PAPER.md:71-74  (Eq. 4)
+ *     gradient g = 2 x o (D^T r)          PAPER.md:66-69  (Eq. 3 summed over points)
+ *     L-BFGS two-loop + Armijo step       PAPER.md:115-119 (Liu & Nocedal; reading DESIGN.md 2.2)
+ * and nothing crosses the host/device boundary inside the loop.
+ *
+ * Conventions for EVERY entry point
+ *   - Pointers marked "host or device" may be either: copies use cudaMemcpyDefault (UVA).
+ *     All arrays are fp32 (int32 where stated), dense, C order, no aliasing between arguments.
+ *   - The caller owns every argument buffer; the handle owns only what it allocates itself
+ *     and gmco_destroy frees it.  Input buffers may be freed as soon as the call returns
+ *     (host inputs) or as soon as the stream has passed the call (device inputs).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *     gmco_create / gmco_optimize / gmco_evaluate only ENQUEUE work on it;
+ *     gmco_result synchronises it.
+ *   - Return value: GMCO_OK (0) or a negative gmco_status; never throws, aborts or prints.
+ *     gmco_last_error(h) gives a message for the last failure on that handle
+ *     (gmco_last_error(NULL) for a failed gmco_create).
+ *   - Requires an sm_100 device (B200).  There is no CPU fallback: without a usable GPU
+ *     every compute entry point returns GMCO_E_UNSUPPORTED or GMCO_E_CUDA.
+ */
+#ifndef GMCO_H_
+#define GMCO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GMCO_API __attribute__((visibility("default")))
+#else
+#define GMCO_API
+#endif
+
+#define GMCO_VERSION 100          /* 0.1.0 */
+#define GMCO_MAX_STRUCTS 8
+#define GMCO_MAX_HISTORY 16
+
+typedef enum gmco_status {
+  GMCO_OK = 0,
+  GMCO_E_INVALID = -1,      /* NULL pointer, bad size, NaN/negative input, sizes do not add up   */
+  GMCO_E_UNSUPPORTED = -2,  /* no sm_100 device, or a size outside the supported range            */
+  GMCO_E_CUDA = -3,         /* a CUDA call failed; message holds cudaGetErrorString               */
+  GMCO_E_NOMEM = -4,        /* device allocation failed                                           */
+  GMCO_E_STATE = -5         /* call out of order (e.g. gmco_result before gmco_optimize)          */
+} gmco_status;
+
+/* Precision / pipe of the two contractions D t and D^T r. */
+typedef enum gmco_precision {
+  GMCO_PREC_TF32X3 = 0,     /* tcgen05 kind::tf32, 3-product split (fp32-equivalent), fused kernel */
+  GMCO_PREC_SIMT_FP32 = 1   /* plain fp32 FMA kernels (reference datum and debug route)            */
+} gmco_precision;
+
+/* Per-plan exit status written by gmco_result. */
+typedef enum gmco_plan_status {
+  GMCO_PLAN_ITERS = 0,      /* ran the full iteration budget                                       */
+  GMCO_PLAN_CONVERGED = 1,  /* eps rule met or gradient exactly zero                */
+  GMCO_PLAN_STALLED = 2     /* max_trials step halvings without an Armijo decrease                 */
+} gmco_plan_status;
+
+/* One penalised point group ("structure": an organ, or one point class of it; Table 1,
+ * PAPER.md:80-88).  Rows of D belong to structures contiguously, in table order. */
+typedef struct gmco_structure {
+  int32_t n_points;   /* > 0                                                                      */
+  float d_lo, d_hi;   /* D_min, D_max of Eq. 2 in Gy; -INFINITY / +INFINITY disables a side       */
+  float w_lo, w_hi;   /* class-solution weights w_min, w_max (>= 0)                               */
+  int32_t dvh_kind;   /* 0 none | 1 V_level: % of points with d >= level% of Rx
+                                | 2 D_level: dose of the ceil(level% * n)-th hottest point, % of Rx */
+  float dvh_level;    /* percent, e.g. 100 (V100), 75 (V75), 10 (D10)         */
+} gmco_structure;
+
+typedef struct gmco_options {
+  int32_t m;          /* L-BFGS history length, 1..GMCO_MAX_HISTORY           default 10          */
+  float eps;          /* stop a plan when |F - F+| <= eps max(F, 1e-30); 0 = off      default 0   */
+  float c1;           /* Armijo constant                                      default 1e-4        */
+  int32_t max_trials; /* step halvings before a plan is declared stalled      default 20          */
+  int32_t precision;  /* gmco_precision                                       default TF32X3      */
+  int32_t reserved[3];/* must be 0                                                                */
+} gmco_options;
+
+/* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */
+typedef struct gmco_stats {
+  int64_t device_bytes;     /* bytes currently allocated by the handle                            */
+  int32_t rounds;           /* evaluation rounds executed (1 + iterations + backtracks of the slowest plan) */
+  int32_t kernel_launches;  /* kernels launched by the library since gmco_optimize was called     */
+  int32_t plans_iters, plans_converged, plans_stalled;
+  int32_t reserved[3];
+} gmco_stats;
+
+typedef struct gmco_handle gmco_handle;
+
+GMCO_API int gmco_version(void);                       /* GMCO_VERSION of the loaded library               */
+GMCO_API void gmco_default_options(gmco_options* opt); /* fills the defaults listed above                  */
+
+/* a0 -- case setup (PAPER.md:97 step (i) hands over the dose-rate matrix; PAPER.md:113 first
+ * transfer).  Copies D (host or device, [n_points][ldD] with ldD >= n_dwell, point-major as
+ * in Eq. 1) into the handle's padded, pre-split device layout; the caller may free D afterwards.
+ * structs: HOST array of n_structs (1..GMCO_MAX_STRUCTS) entries, sum n_points == n_points.
+ * rx_dose: prescription in Gy (> 0), used by the DVH indices only.  opt may be NULL.
+ * Limits: 1 <= n_dwell <= 480.  On failure *out is NULL. */
+GMCO_API int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_dwell, int64_t ldD,
+                const gmco_structure* structs, int32_t n_structs, float rx_dose,
+                const gmco_options* opt, void* cuda_stream);
+
+/* a1-a7 -- optimise K plans for `iters` L-BFGS iterations each.
+ * T0: start dwell times in seconds, >= 0, [K][n_dwell] or, if t0_broadcast != 0, [n_dwell]
+ * shared by all plans (host or device).  weights: hidden weights [K][n_structs][2] = (lo, hi)
+ * per structure, >= 0 (host or device); the effective weight of a term is
+ * weights[k][s][side] * structs[s].w_side / structs[s].n_points (Eq. 4 x Table 1; the
+ * library does NOT normalise hidden weights to sum 1).  K = 0 and iters = 0 are valid
+ * (iters = 0 evaluates the start point only).  Enqueues on cuda_stream and returns. */
+GMCO_API int gmco_optimize(gmco_handle* h, const float* T0, int32_t t0_broadcast, const float* weights,
+                  int32_t K, int32_t iters, void* cuda_stream);
+
+/* a8 -- results of the last gmco_optimize (PAPER.md:113 second transfer; DVH indices
+ * PAPER.md:132-140).  Finishes any plan that still has backtracking rounds outstanding,
+ * evaluates dose once more at the final dwell times, and writes (host or device, any may be NULL):
+ *   T [K][n_dwell] seconds; objective [K]; dvh [K][n_structs] (0 where dvh_kind = 0);
+ *   objective_terms [K][n_structs][2]; iters_done [K]; plan_status [K] (gmco_plan_status).
+ * Synchronises the stream given to gmco_optimize.  GMCO_E_STATE if no optimisation ran. */
+GMCO_API int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* objective_terms,
+                int32_t* iters_done, int32_t* plan_status);
+
+/* Test / debug hook -- one evaluation (Eqs. 1-4) of K plans at dwell times T ([K][n_dwell],
+ * or [n_dwell] if t_broadcast) through the SAME kernels the optimiser uses.  Outputs (host or
+ * device, any may be NULL): dose [n_points][K] (plan fastest) -- the fused path never stores
+ * dose otherwise; F [K]; grad_x [K][n_dwell] = dF/dx with x = sqrt(T).  Enqueues, then
+ * synchronises only if an output is a host pointer.  Discards any optimisation state. */
+GMCO_API int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const float* weights,
+                  int32_t K, float* dose, float* F, float* grad_x, void* cuda_stream);
+
+/* Counters of the last optimise/result pair.  GMCO_E_STATE before the first gmco_result. */
+GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);
+
+/* Frees everything the handle owns (synchronises its stream first).  NULL is a no-op. */
+GMCO_API void gmco_destroy(gmco_handle* h);
+
+/* Message of the last error on h (or of the last failed gmco_create if h is NULL).
+ * Valid until the next call on that handle from the same thread. */
+GMCO_API const char* gmco_last_error(const gmco_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GMCO_H_ */

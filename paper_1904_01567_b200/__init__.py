@@ -1,0 +1,10 @@
+"""paper_1904_01567_b200 -- B200-native gL-BFGS hot path of gMCO (arXiv 1904.01567).
+
+The product is ``libgmco.so`` (C ABI in ``include/gmco.h``, CUDA sources in ``csrc/``).
+This package is the thin Python binding: same entry-point names, argument marshalling only.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback:
+importing :mod:`paper_1904_01567_b200.binding` raises if the library has not been built.
+"""
+from .binding import (GmcoError, Handle, Options, gmco_create, gmco_destroy, gmco_evaluate, gmco_get_stats,  # noqa: F401
+                      gmco_optimize, gmco_result, gmco_version, lib, lib_path,
+                      GMCO_PREC_TF32X3, GMCO_PREC_SIMT_FP32)

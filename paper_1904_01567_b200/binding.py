@@ -1,0 +1,198 @@
+"""ctypes binding of libgmco.so: same names as include/gmco.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+GMCO_PREC_TF32X3, GMCO_PREC_SIMT_FP32 = 0, 1
+GMCO_MAX_STRUCTS = 8
+
+
+class GmcoError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libgmco error {code}: {msg}")
+        self.code = code
+
+
+class _Structure(C.Structure):
+    _fields_ = [("n_points", C.c_int32), ("d_lo", C.c_float), ("d_hi", C.c_float), ("w_lo", C.c_float),
+                ("w_hi", C.c_float), ("dvh_kind", C.c_int32), ("dvh_level", C.c_float)]
+
+
+class Options(C.Structure):
+    _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
+                ("precision", C.c_int32), ("reserved", C.c_int32 * 3)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("device_bytes", C.c_int64), ("rounds", C.c_int32), ("kernel_launches", C.c_int32),
+                ("plans_iters", C.c_int32), ("plans_converged", C.c_int32), ("plans_stalled", C.c_int32),
+                ("reserved", C.c_int32 * 3)]
+
+
+def lib_path() -> Path:
+    return _PKG / "libgmco.so"
+
+
+_lib = None
+
+
+def lib():
+    """Load libgmco.so.  Raises (never falls back) when it is missing: build it with
+    ``python -m paper_1904_01567_b200.build`` or ``__graft_entry__.build()``."""
+    global _lib
+    if _lib is None:
+        p = lib_path()
+        if not p.exists():
+            raise ImportError(f"{p} is missing: run `python paper_1904_01567_b200/build.py` (needs nvcc). "
+                              "There is no CPU fallback.")
+        L = C.CDLL(str(p))
+        vp, i32, i64, fp = C.c_void_p, C.c_int32, C.c_int64, C.c_void_p
+        L.gmco_version.restype = C.c_int
+        L.gmco_default_options.argtypes = [C.POINTER(Options)]
+        L.gmco_default_options.restype = None
+        L.gmco_create.argtypes = [C.POINTER(vp), fp, i64, i64, i64, C.POINTER(_Structure), i32, C.c_float,
+                                  C.POINTER(Options), vp]
+        L.gmco_optimize.argtypes = [vp, fp, i32, fp, i32, i32, vp]
+        L.gmco_result.argtypes = [vp, fp, fp, fp, fp, vp, vp]
+        L.gmco_evaluate.argtypes = [vp, fp, i32, fp, i32, fp, fp, fp, vp]
+        L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.gmco_destroy.argtypes = [vp]
+        L.gmco_destroy.restype = None
+        L.gmco_last_error.argtypes = [vp]
+        L.gmco_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def gmco_version() -> int:
+    return int(lib().gmco_version())
+
+
+class Handle:
+    def __init__(self, ptr, n_points, n_dwell, n_structs):
+        self.ptr, self.n_points, self.n_dwell, self.n_structs = ptr, n_points, n_dwell, n_structs
+        self.K = 0
+        self._keep = []          # inputs that must outlive the enqueued work
+
+
+def _check(rc, h=None):
+    if rc != 0:
+        msg = lib().gmco_last_error(h.ptr if h is not None else None)
+        raise GmcoError(rc, msg.decode() if msg else "")
+
+
+def _ptr(a):
+    """Raw address of a torch tensor (any device) or numpy array; None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert a.is_contiguous()
+    return a.data_ptr()
+
+
+def _f32(a):
+    if isinstance(a, np.ndarray):
+        return np.ascontiguousarray(a, dtype=np.float32)
+    import torch
+    return a.to(torch.float32).contiguous()
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return torch.cuda.current_stream().cuda_stream
+        return None
+    return getattr(stream, "cuda_stream", stream)
+
+
+def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3) -> Options:
+    o = Options()
+    lib().gmco_default_options(C.byref(o))
+    o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
+    return o
+
+
+def gmco_create(D, structures, rx, options: Options | None = None, stream=None) -> Handle:
+    """D: [n_points, n_dwell] fp32 tensor/array (host or device); structures: objects with the
+    fields of gmco_structure (e.g. gmco_cases.Structure)."""
+    D = _f32(D)
+    n_points, n_dwell = int(D.shape[0]), int(D.shape[1])
+    st = (_Structure * len(structures))()
+    for i, s in enumerate(structures):
+        st[i] = _Structure(int(s.n_points), float(s.d_lo), float(s.d_hi), float(s.w_lo), float(s.w_hi),
+                           int(s.dvh_kind), float(s.dvh_level))
+    out = C.c_void_p()
+    rc = lib().gmco_create(C.byref(out), _ptr(D), n_points, n_dwell, n_dwell, st, len(structures), float(rx),
+                           C.byref(options) if options is not None else None, _stream(stream))
+    _check(rc)
+    h = Handle(out, n_points, n_dwell, len(structures))
+    h._keep.append(D)
+    return h
+
+
+def gmco_optimize(h: Handle, T0, weights, iters: int, stream=None) -> None:
+    T0, weights = _f32(T0), _f32(weights)
+    K = int(weights.shape[0]) if weights.ndim == 3 else int(weights.numel() if hasattr(weights, "numel") else weights.size) // (2 * h.n_structs)
+    bc = 1 if T0.ndim == 1 else 0
+    h._keep = h._keep[:1] + [T0, weights]
+    h.K = K
+    _check(lib().gmco_optimize(h.ptr, _ptr(T0), bc, _ptr(weights), K, int(iters), _stream(stream)), h)
+
+
+def gmco_result(h: Handle, host: bool = False, want_terms: bool = True) -> dict:
+    """Returns dict(T, objective, dvh, objective_terms, iters_done, plan_status) as device tensors
+    (or numpy arrays when host=True)."""
+    K, A, S = h.K, h.n_dwell, h.n_structs
+    if host:
+        T = np.empty((K, A), np.float32); F = np.empty(K, np.float32); dvh = np.empty((K, S), np.float32)
+        terms = np.empty((K, S, 2), np.float32) if want_terms else None
+        it = np.empty(K, np.int32); stt = np.empty(K, np.int32)
+    else:
+        import torch
+        dev = torch.device("cuda")
+        T = torch.empty((K, A), dtype=torch.float32, device=dev); F = torch.empty(K, dtype=torch.float32, device=dev)
+        dvh = torch.empty((K, S), dtype=torch.float32, device=dev)
+        terms = torch.empty((K, S, 2), dtype=torch.float32, device=dev) if want_terms else None
+        it = torch.empty(K, dtype=torch.int32, device=dev); stt = torch.empty(K, dtype=torch.int32, device=dev)
+    _check(lib().gmco_result(h.ptr, _ptr(T), _ptr(F), _ptr(dvh), _ptr(terms), _ptr(it), _ptr(stt)), h)
+    return dict(T=T, objective=F, dvh=dvh, objective_terms=terms, iters_done=it, plan_status=stt)
+
+
+def gmco_evaluate(h: Handle, T, weights, want_dose=False, want_grad=True, host: bool = False, stream=None) -> dict:
+    T, weights = _f32(T), _f32(weights)
+    K = int(weights.shape[0])
+    bc = 1 if T.ndim == 1 else 0
+    N, A = h.n_points, h.n_dwell
+    if host:
+        dose = np.empty((N, K), np.float32) if want_dose else None
+        F = np.empty(K, np.float32); g = np.empty((K, A), np.float32) if want_grad else None
+    else:
+        import torch
+        dev = torch.device("cuda")
+        dose = torch.empty((N, K), dtype=torch.float32, device=dev) if want_dose else None
+        F = torch.empty(K, dtype=torch.float32, device=dev)
+        g = torch.empty((K, A), dtype=torch.float32, device=dev) if want_grad else None
+    h._keep = h._keep[:1] + [T, weights]
+    h.K = K
+    _check(lib().gmco_evaluate(h.ptr, _ptr(T), bc, _ptr(weights), K, _ptr(dose), _ptr(F), _ptr(g), _stream(stream)), h)
+    return dict(dose=dose, F=F, grad_x=g)
+
+
+def gmco_get_stats(h: Handle) -> dict:
+    s = Stats()
+    _check(lib().gmco_get_stats(h.ptr, C.byref(s)), h)
+    return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+
+
+def gmco_destroy(h: Handle) -> None:
+    if h is not None and h.ptr:
+        lib().gmco_destroy(h.ptr)
+        h.ptr = None
+        h._keep = []

@@ -1,0 +1,530 @@
+// gmco_api.cu -- the C ABI of include/gmco.h: argument checks, device layout, round driver.
+// Host logic only; every arithmetic step of the path runs in the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "gmco_internal.cuh"
+
+using namespace gmco;
+
+namespace {
+
+thread_local char g_create_error[512] = "";
+
+struct Arena {              // one stream-ordered allocation, carved into 256 B aligned pieces
+  char* base = nullptr; size_t size = 0, used = 0; cudaStream_t st = nullptr;
+  template <class T> T* take(size_t n) {
+    const size_t bytes = (n * sizeof(T) + 255) & ~size_t(255);
+    T* p = reinterpret_cast<T*>(base ? base + used : nullptr);
+    used += bytes;
+    return p;
+  }
+};
+
+enum HandleState { ST_CREATED = 0, ST_OPTIMIZED = 1, ST_RESULT = 2, ST_EVALUATED = 3 };
+
+}  // namespace
+
+struct gmco_handle {
+  gmco_options opt{};
+  CaseDev c{};
+  PlanDev p{};
+  std::vector<StructHost> sh;
+  std::vector<gmco_structure> structs;
+  Arena case_arena, plan_arena;
+  int plan_capacity_K = -1;
+  float* struct_scale = nullptr;     // [2S] device: base weight / n_points
+  float* dvh_thr = nullptr;          // [S] device
+  // staging
+  float* stage_D = nullptr;
+  float *in_T0 = nullptr, *in_w = nullptr;
+  float *out_T = nullptr, *out_F = nullptr, *out_dvh = nullptr, *out_terms = nullptr;
+  int *out_iters = nullptr, *out_status = nullptr;
+  int* host_flags = nullptr;         // pinned [4]
+  TcPlan* tc = nullptr;
+  cudaStream_t stream = nullptr;
+  int device = 0, num_sms = 0;
+  HandleState state = ST_CREATED;
+  int iters = 0, rounds_enqueued = 0, launches = 0;
+  gmco_stats stats{};
+  bool have_stats = false;
+  char err[512] = "";
+};
+
+namespace {
+
+int fail(gmco_handle* h, int code, const char* fmt, const char* a = "") {
+  char* dst = h ? h->err : g_create_error;
+  snprintf(dst, 512, fmt, a);
+  return code;
+}
+
+#define CK(h, call)                                                              \
+  do {                                                                           \
+    cudaError_t e_ = (call);                                                     \
+    if (e_ != cudaSuccess) {                                                     \
+      const int code_ = e_ == cudaErrorMemoryAllocation ? GMCO_E_NOMEM : GMCO_E_CUDA; \
+      return fail(h, code_, #call ": %s", cudaGetErrorString(e_));               \
+    }                                                                            \
+  } while (0)
+
+#define LN(h, expr)                                                              \
+  do {                                                                           \
+    int n_ = (expr);                                                             \
+    if (n_ < 0) return fail(h, GMCO_E_CUDA, #expr ": %s", cudaGetErrorString(cudaGetLastError())); \
+    (h)->launches += n_;                                                         \
+  } while (0)
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at{};
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int round_up(long long v, int a) { return (int)(((v + a - 1) / a) * a); }
+
+int arena_alloc(gmco_handle* h, Arena& a, cudaStream_t st) {
+  a.size = a.used ? a.used : 256;
+  a.used = 0;
+  a.st = st;
+  cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&a.base), a.size, st);
+  if (e != cudaSuccess) { a.base = nullptr; return fail(h, GMCO_E_NOMEM, "cudaMallocAsync: %s", cudaGetErrorString(e)); }
+  return GMCO_OK;
+}
+
+void arena_free(Arena& a, cudaStream_t st) {
+  if (a.base) cudaFreeAsync(a.base, st);
+  a = Arena{};
+}
+
+// carve (or, with base == nullptr, just measure) the case arena
+void carve_case(gmco_handle* h, bool want_split, bool need_stage) {
+  Arena& a = h->case_arena;
+  CaseDev& c = h->c;
+  const size_t nd = (size_t)c.N_alloc * c.A_pad;
+  c.D = a.take<float>(nd);
+  if (want_split) {
+    c.D_hi = a.take<float>(nd); c.D_lo = a.take<float>(nd);
+    c.DT_hi = a.take<float>(nd); c.DT_lo = a.take<float>(nd);
+  }
+  c.pt_lo = a.take<float>(c.N_alloc); c.pt_hi = a.take<float>(c.N_alloc);
+  c.tile_struct = a.take<int>(c.N_alloc / 64);
+  c.row_src = a.take<int>(c.N_alloc); c.sel_pos = a.take<int>(c.N_alloc);
+  h->struct_scale = a.take<float>(2 * GMCO_MAX_STRUCTS);
+  h->dvh_thr = a.take<float>(GMCO_MAX_STRUCTS);
+  h->stage_D = need_stage ? a.take<float>((size_t)c.N * c.A) : nullptr;
+}
+
+void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
+  Arena& a = h->plan_arena;
+  const CaseDev& c = h->c;
+  PlanDev& p = h->p;
+  p.K = K; p.K_pad = round_up(K, kPlanTile); p.m = h->opt.m;
+  const size_t ka = (size_t)p.K_pad * c.A_pad, kp = (size_t)p.K_pad;
+  p.x = a.take<float>(ka); p.g = a.take<float>(ka); p.p = a.take<float>(ka); p.xt = a.take<float>(ka);
+  p.T = a.take<float>(ka); p.T_hi = a.take<float>(ka); p.T_lo = a.take<float>(ka);
+  p.Sh = a.take<float>(ka * p.m); p.Yh = a.take<float>(ka * p.m);
+  p.rho = a.take<float>(kp * p.m); p.gam = a.take<float>(kp * p.m);
+  p.Weff = a.take<float>(kp * 2 * c.S);
+  p.F = a.take<float>(kp); p.gp = a.take<float>(kp); p.alpha = a.take<float>(kp);
+  p.it_done = a.take<int>(kp); p.trials = a.take<int>(kp); p.hcount = a.take<int>(kp); p.hhead = a.take<int>(kp);
+  p.status = a.take<int>(kp);
+  p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1);
+  // partials: the SIMT dose pass (also the final pass of gmco_result) needs [tiles][K_pad][2]
+  const size_t f_simt = (size_t)(c.N_alloc / 64) * kp * 2;
+  p.nFcomp = 2; p.nF = c.N_alloc / 64;
+  const bool simt = h->opt.precision == GMCO_PREC_SIMT_FP32;
+  size_t f_elems = f_simt, g_elems = 0;
+  if (simt) {
+    // split count depends on the point count only, so a plan's summation order does not depend on K
+    int ns = c.N_alloc / 256;
+    if (ns < 1) ns = 1;
+    if (ns > 32) ns = 32;
+    p.nG = ns;
+    g_elems = (size_t)ns * ka;
+    p.R = a.take<float>(kp * c.N_alloc);
+  } else {
+    // upper bound on stream-K segments: one per CTA plus one per plan tile
+    const size_t nseg = (size_t)h->num_sms + p.K_pad / kPlanTile + 1;
+    g_elems = nseg * kPlanTile * c.A_pad;
+    if (nseg * kPlanTile > f_elems) f_elems = nseg * kPlanTile;
+    p.R = nullptr; p.nG = 0;
+  }
+  p.Fpart = a.take<float>(f_elems); p.Gpart = a.take<float>(g_elems);
+  p.res_terms = a.take<float>(kp * 2 * c.S); p.res_cnt = a.take<int>(kp * c.S);
+  p.res_sel = a.take<float>(kp * (size_t)(c.n_sel > 0 ? c.n_sel : 1)); p.res_dvh = a.take<float>(kp * c.S);
+  h->in_T0 = a.take<float>((size_t)(K > 0 ? K : 1) * c.A); h->in_w = a.take<float>((size_t)(K > 0 ? K : 1) * 2 * c.S);
+  h->out_T = a.take<float>((size_t)(K > 0 ? K : 1) * c.A); h->out_F = a.take<float>(kp + 1);
+  h->out_dvh = a.take<float>(kp * c.S + 1); h->out_terms = a.take<float>(kp * 2 * c.S + 1);
+  h->out_iters = a.take<int>(kp + 1); h->out_status = a.take<int>(kp + 1);
+  (void)dose_stage_elems;
+}
+
+int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
+  if (h->plan_capacity_K == K && h->plan_arena.base && h->stream == st) {
+    return GMCO_OK;
+  }
+  if (h->tc) { tc_plan_destroy(h->tc); h->tc = nullptr; }
+  arena_free(h->plan_arena, h->stream);
+  carve_plans(h, K, 0);                       // measuring pass
+  int rc = arena_alloc(h, h->plan_arena, st);
+  if (rc) return rc;
+  carve_plans(h, K, 0);
+  h->plan_capacity_K = K;
+  if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
+    h->tc = tc_plan_create(h->c, h->p, h->num_sms, h->err, sizeof(h->err));
+    if (!h->tc) return GMCO_E_UNSUPPORTED;
+  }
+  return GMCO_OK;
+}
+
+StepParams make_step_params(const gmco_handle* h, int iters) {
+  StepParams sp{};
+  const PlanDev& p = h->p; const CaseDev& c = h->c;
+  sp.K = p.K; sp.A_pad = c.A_pad; sp.m = p.m; sp.iters = iters; sp.max_trials = h->opt.max_trials;
+  sp.c1 = h->opt.c1; sp.eps = h->opt.eps;
+  sp.Fpart = p.Fpart; sp.Gpart = p.Gpart;
+  if (h->opt.precision == GMCO_PREC_SIMT_FP32) {
+    sp.nF = p.nF; sp.nFcomp = 2; sp.f_slot_stride = (long long)p.K_pad * 2;
+    sp.nG = p.nG; sp.g_slot_stride = (long long)p.K_pad * c.A_pad;
+    sp.tile_local = 0; sp.tile_seg = nullptr;
+  } else {
+    sp.nF = 0; sp.nFcomp = 1; sp.f_slot_stride = kPlanTile;
+    sp.nG = 0; sp.g_slot_stride = (long long)kPlanTile * c.A_pad;
+    sp.tile_local = 1; sp.tile_seg = tc_tile_seg_dev(h->tc);
+  }
+  return sp;
+}
+
+// SIMT kernels emit r = 2 w (d - D_lim) / n, the tensor kernel emits r / 2 (one multiply less per element)
+float g_scale_of(const gmco_handle* h) { return h->opt.precision == GMCO_PREC_SIMT_FP32 ? 2.f : 4.f; }
+
+int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, cudaStream_t st) {
+  if (h->opt.precision == GMCO_PREC_SIMT_FP32) {
+    LN(h, launch_simt_eval(h->c, h->p, true, dose_dbg, false, nullptr, gate, st));
+    LN(h, launch_simt_grad(h->c, h->p, gate, st));
+  } else {
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, st));
+  }
+  return GMCO_OK;
+}
+
+int enqueue_rounds(gmco_handle* h, int n, cudaStream_t st) {
+  const StepParams sp = make_step_params(h, h->iters);
+  for (int i = 0; i < n; ++i) {
+    const int parity = h->rounds_enqueued & 1;
+    LN(h, launch_round_begin(h->p, parity, st));
+    int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, st);
+    if (rc) return rc;
+    LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
+    h->rounds_enqueued++;
+  }
+  return GMCO_OK;
+}
+
+int copy_inputs(gmco_handle* h, const float* T0, int bcast, const float* w, int K, cudaStream_t st,
+                const float** T0_dev, const float** w_dev) {
+  const CaseDev& c = h->c;
+  const size_t nT = (size_t)(bcast ? 1 : K) * c.A, nW = (size_t)K * 2 * c.S;
+  if (is_device_ptr(T0)) *T0_dev = T0;
+  else {
+    for (size_t i = 0; i < nT; ++i)
+      if (!(T0[i] >= 0.f) || isinf(T0[i])) return fail(h, GMCO_E_INVALID, "T0 holds a negative, NaN or infinite dwell time%s");
+    CK(h, cudaMemcpyAsync(h->in_T0, T0, nT * sizeof(float), cudaMemcpyHostToDevice, st));
+    *T0_dev = h->in_T0;
+  }
+  if (is_device_ptr(w)) *w_dev = w;
+  else {
+    for (size_t i = 0; i < nW; ++i)
+      if (!(w[i] >= 0.f) || isinf(w[i])) return fail(h, GMCO_E_INVALID, "weights hold a negative, NaN or infinite value%s");
+    CK(h, cudaMemcpyAsync(h->in_w, w, nW * sizeof(float), cudaMemcpyHostToDevice, st));
+    *w_dev = h->in_w;
+  }
+  return GMCO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gmco_version(void) { return GMCO_VERSION; }
+
+void gmco_default_options(gmco_options* o) {
+  if (!o) return;
+  memset(o, 0, sizeof(*o));
+  o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3;
+}
+
+const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
+
+int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_dwell, int64_t ldD,
+                const gmco_structure* structs, int32_t n_structs, float rx_dose, const gmco_options* opt,
+                void* cuda_stream) {
+  if (!out) return fail(nullptr, GMCO_E_INVALID, "out is NULL%s");
+  *out = nullptr;
+  if (!D || !structs) return fail(nullptr, GMCO_E_INVALID, "D or structs is NULL%s");
+  if (n_points <= 0 || n_dwell <= 0 || ldD < n_dwell || n_points > (1 << 28))
+    return fail(nullptr, GMCO_E_INVALID, "bad n_points / n_dwell / ldD%s");
+  if (n_structs < 1 || n_structs > GMCO_MAX_STRUCTS) return fail(nullptr, GMCO_E_INVALID, "n_structs outside 1..8%s");
+  if (!(rx_dose > 0.f) || isinf(rx_dose)) return fail(nullptr, GMCO_E_INVALID, "rx_dose must be positive and finite%s");
+  if (n_dwell > kMaxApad) return fail(nullptr, GMCO_E_UNSUPPORTED, "n_dwell above 480 is not supported%s");
+  gmco_options o;
+  gmco_default_options(&o);
+  if (opt) o = *opt;
+  if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
+      (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || o.reserved[0] || o.reserved[1] ||
+      o.reserved[2])
+    return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
+  long long tot = 0;
+  for (int s = 0; s < n_structs; ++s) {
+    const gmco_structure& g = structs[s];
+    if (g.n_points <= 0 || !(g.w_lo >= 0.f) || !(g.w_hi >= 0.f) || isinf(g.w_lo) || isinf(g.w_hi) || isnan(g.d_lo) ||
+        isnan(g.d_hi) || g.dvh_kind < 0 || g.dvh_kind > 2 || (g.dvh_kind && !(g.dvh_level > 0.f)))
+      return fail(nullptr, GMCO_E_INVALID, "bad gmco_structure entry%s");
+    tot += g.n_points;
+  }
+  if (tot != n_points) return fail(nullptr, GMCO_E_INVALID, "structure sizes do not add up to n_points%s");
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(nullptr, GMCO_E_UNSUPPORTED, "no CUDA device: %s", cudaGetErrorString(e));
+  cudaDeviceProp prop{};
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return fail(nullptr, GMCO_E_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+  if (prop.major != 10) return fail(nullptr, GMCO_E_UNSUPPORTED, "libgmco needs an sm_100 device (B200)%s");
+
+  gmco_handle* h = new (std::nothrow) gmco_handle();
+  if (!h) return fail(nullptr, GMCO_E_NOMEM, "host allocation failed%s");
+  h->opt = o; h->device = dev; h->num_sms = prop.multiProcessorCount;
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  h->structs.assign(structs, structs + n_structs);
+  cudaStream_t st = h->stream;
+
+  // keep freed blocks in the pool so that create/destroy cycles do not hit the OS allocator
+  cudaMemPool_t pool;
+  if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+    uint64_t thr = UINT64_MAX;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+  }
+
+  // ---- row layout: every structure padded to a multiple of 64 rows ----
+  CaseDev& c = h->c;
+  c.N = (int)n_points; c.A = (int)n_dwell; c.S = n_structs; c.rx = rx_dose;
+  c.A_pad = round_up(n_dwell, 32);
+  int row = 0, src = 0, sel = 0;
+  h->sh.resize(n_structs);
+  for (int s = 0; s < n_structs; ++s) {
+    StructHost& q = h->sh[s];
+    q.n_points = structs[s].n_points; q.row_begin = row; q.n_rows_pad = round_up(q.n_points, kStructAlign);
+    q.d_lo = structs[s].d_lo; q.d_hi = structs[s].d_hi; q.w_lo = structs[s].w_lo; q.w_hi = structs[s].w_hi;
+    q.dvh_kind = structs[s].dvh_kind; q.dvh_level = structs[s].dvh_level;
+    q.sel_begin = q.dvh_kind == 2 ? sel : -1;
+    if (q.dvh_kind == 2) sel += q.n_points;
+    row += q.n_rows_pad; src += q.n_points;
+  }
+  c.N_pad = row; c.N_alloc = round_up(row, kRowAlloc); c.n_sel = sel;
+
+  const bool want_split = o.precision == GMCO_PREC_TF32X3;
+  const bool dev_D = is_device_ptr(D);
+  carve_case(h, want_split, !dev_D);
+  int rc = arena_alloc(h, h->case_arena, st);
+  if (rc) { snprintf(g_create_error, 512, "%s", h->err); delete h; return rc; }
+  carve_case(h, want_split, !dev_D);
+
+#define CKC(call)                                                                                   \
+  do {                                                                                              \
+    cudaError_t e2_ = (call);                                                                       \
+    if (e2_ != cudaSuccess) {                                                                       \
+      fail(nullptr, GMCO_E_CUDA, #call ": %s", cudaGetErrorString(e2_));                            \
+      arena_free(h->case_arena, st); delete h; return GMCO_E_CUDA;                                  \
+    }                                                                                               \
+  } while (0)
+
+  std::vector<float> pt_lo(c.N_alloc, -INFINITY), pt_hi(c.N_alloc, INFINITY), scale(2 * GMCO_MAX_STRUCTS, 0.f),
+      thr(GMCO_MAX_STRUCTS, -1.f);
+  std::vector<int> tile_struct(c.N_alloc / 64, 0), row_src(c.N_alloc, -1), sel_pos(c.N_alloc, -1);
+  src = 0;
+  for (int s = 0; s < n_structs; ++s) {
+    const StructHost& q = h->sh[s];
+    for (int i = 0; i < q.n_points; ++i) {
+      pt_lo[q.row_begin + i] = q.d_lo; pt_hi[q.row_begin + i] = q.d_hi;
+      row_src[q.row_begin + i] = src + i;
+      if (q.dvh_kind == 2) sel_pos[q.row_begin + i] = q.sel_begin + i;
+    }
+    for (int t = q.row_begin / 64; t < (q.row_begin + q.n_rows_pad) / 64; ++t) tile_struct[t] = s;
+    scale[2 * s] = q.w_lo / (float)q.n_points; scale[2 * s + 1] = q.w_hi / (float)q.n_points;
+    if (q.dvh_kind == 1) thr[s] = q.dvh_level / 100.f * rx_dose;
+    src += q.n_points;
+  }
+  // tiles past N_pad keep structure 0 with infinite thresholds: zero contribution
+  CKC(cudaMemcpyAsync(c.pt_lo, pt_lo.data(), c.N_alloc * sizeof(float), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(c.pt_hi, pt_hi.data(), c.N_alloc * sizeof(float), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(c.tile_struct, tile_struct.data(), tile_struct.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(c.row_src, row_src.data(), c.N_alloc * sizeof(int), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(c.sel_pos, sel_pos.data(), c.N_alloc * sizeof(int), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(h->struct_scale, scale.data(), scale.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(h->dvh_thr, thr.data(), thr.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+  const float* D_dev = D;
+  long long ld = ldD;
+  if (!dev_D) {
+    CKC(cudaMemcpy2DAsync(h->stage_D, (size_t)c.A * sizeof(float), D, (size_t)ldD * sizeof(float),
+                          (size_t)c.A * sizeof(float), (size_t)c.N, cudaMemcpyHostToDevice, st));
+    D_dev = h->stage_D; ld = c.A;
+  }
+  // the host vectors above are pageable: the async copies have completed their staging on return
+  CKC(cudaStreamSynchronize(st));
+  if (launch_setup_case(c, D_dev, ld, c.row_src, want_split, st) < 0) {
+    fail(nullptr, GMCO_E_CUDA, "case setup kernels: %s", cudaGetErrorString(cudaGetLastError()));
+    arena_free(h->case_arena, st); delete h; return GMCO_E_CUDA;
+  }
+  CKC(cudaMallocHost(reinterpret_cast<void**>(&h->host_flags), 4 * sizeof(int)));
+#undef CKC
+  *out = h;
+  return GMCO_OK;
+}
+
+void gmco_destroy(gmco_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  if (h->tc) tc_plan_destroy(h->tc);
+  arena_free(h->plan_arena, h->stream);
+  arena_free(h->case_arena, h->stream);
+  if (h->host_flags) cudaFreeHost(h->host_flags);
+  delete h;
+}
+
+int gmco_optimize(gmco_handle* h, const float* T0, int32_t t0_broadcast, const float* weights, int32_t K,
+                  int32_t iters, void* cuda_stream) {
+  if (!h) return GMCO_E_INVALID;
+  if (K < 0 || iters < 0) return fail(h, GMCO_E_INVALID, "K and iters must be >= 0%s");
+  if (K > 0 && (!T0 || !weights)) return fail(h, GMCO_E_INVALID, "T0 or weights is NULL%s");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int rc = ensure_plans(h, K, st);
+  if (rc) return rc;
+  h->stream = st; h->iters = iters; h->rounds_enqueued = 0; h->launches = 0; h->have_stats = false;
+  h->state = ST_CREATED;
+  if (K == 0) { h->state = ST_OPTIMIZED; return GMCO_OK; }
+  const float *T0d = nullptr, *wd = nullptr;
+  rc = copy_inputs(h, T0, t0_broadcast, weights, K, st, &T0d, &wd);
+  if (rc) return rc;
+  LN(h, launch_init_plans(h->c, h->p, T0d, t0_broadcast ? 1 : 0, wd, h->struct_scale, st));
+  // round 0 evaluates the start point; every further round is one trial step of every running plan.
+  // Backtracking plans need extra rounds: enqueue some slack now (rounds with nothing running return
+  // at once), gmco_result adds more if a plan is still running.
+  const int slack = iters > 0 ? (iters / 6 > 4 ? iters / 6 : 4) : 0;
+  rc = enqueue_rounds(h, 1 + iters + slack, st);
+  if (rc) return rc;
+  h->state = ST_OPTIMIZED;
+  return GMCO_OK;
+}
+
+int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* objective_terms, int32_t* iters_done,
+                int32_t* plan_status) {
+  if (!h) return GMCO_E_INVALID;
+  if (h->state != ST_OPTIMIZED && h->state != ST_RESULT) return fail(h, GMCO_E_STATE, "gmco_result needs a prior gmco_optimize%s");
+  cudaStream_t st = h->stream;
+  const PlanDev& p = h->p; const CaseDev& c = h->c;
+  const int K = p.K;
+  if (K == 0) {
+    memset(&h->stats, 0, sizeof(h->stats));
+    h->stats.device_bytes = (int64_t)(h->case_arena.size + h->plan_arena.size);
+    h->have_stats = true; h->state = ST_RESULT;
+    return GMCO_OK;
+  }
+  if (h->state == ST_OPTIMIZED) {
+    const long long max_rounds = 1 + (long long)h->iters * ((long long)h->opt.max_trials + 1);
+    for (;;) {
+      const int parity = h->rounds_enqueued & 1;          // counter the NEXT round would read
+      CK(h, cudaMemcpyAsync(h->host_flags, p.n_running + parity, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(h, cudaStreamSynchronize(st));
+      if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
+      if (h->host_flags[0] == 0 || h->rounds_enqueued >= max_rounds) break;
+      int rc = enqueue_rounds(h, 8, st);
+      if (rc) return rc;
+    }
+    // final dose pass at the accepted dwell times: objective terms, V_level counts, D_level doses
+    LN(h, launch_prepare_final(c, p, st));
+    LN(h, launch_simt_eval(c, p, false, nullptr, true, h->dvh_thr, nullptr, st));
+    LN(h, launch_result(c, p, h->sh.data(), h->out_T, h->out_F, h->out_dvh, h->out_terms, h->out_iters,
+                        h->out_status, st));
+  }
+  if (T) CK(h, cudaMemcpyAsync(T, h->out_T, (size_t)K * c.A * sizeof(float), cudaMemcpyDefault, st));
+  if (objective) CK(h, cudaMemcpyAsync(objective, h->out_F, (size_t)K * sizeof(float), cudaMemcpyDefault, st));
+  if (dvh) CK(h, cudaMemcpyAsync(dvh, h->out_dvh, (size_t)K * c.S * sizeof(float), cudaMemcpyDefault, st));
+  if (objective_terms)
+    CK(h, cudaMemcpyAsync(objective_terms, h->out_terms, (size_t)K * 2 * c.S * sizeof(float), cudaMemcpyDefault, st));
+  if (iters_done) CK(h, cudaMemcpyAsync(iters_done, h->out_iters, (size_t)K * sizeof(int), cudaMemcpyDefault, st));
+  if (plan_status) CK(h, cudaMemcpyAsync(plan_status, h->out_status, (size_t)K * sizeof(int), cudaMemcpyDefault, st));
+  CK(h, cudaStreamSynchronize(st));
+  if (h->state == ST_OPTIMIZED) {
+    std::vector<int> stv(K);
+    CK(h, cudaMemcpy(stv.data(), h->out_status, (size_t)K * sizeof(int), cudaMemcpyDeviceToHost));
+    gmco_stats s{};
+    s.device_bytes = (int64_t)(h->case_arena.size + h->plan_arena.size);
+    s.rounds = h->rounds_enqueued; s.kernel_launches = h->launches;
+    for (int k = 0; k < K; ++k) {
+      if (stv[k] == GMCO_PLAN_ITERS) s.plans_iters++;
+      else if (stv[k] == GMCO_PLAN_CONVERGED) s.plans_converged++;
+      else s.plans_stalled++;
+    }
+    h->stats = s; h->have_stats = true;
+  }
+  h->state = ST_RESULT;
+  return GMCO_OK;
+}
+
+int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const float* weights, int32_t K, float* dose,
+                  float* F, float* grad_x, void* cuda_stream) {
+  if (!h) return GMCO_E_INVALID;
+  if (K < 0) return fail(h, GMCO_E_INVALID, "K must be >= 0%s");
+  if (K == 0) return GMCO_OK;
+  if (!T || !weights) return fail(h, GMCO_E_INVALID, "T or weights is NULL%s");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int rc = ensure_plans(h, K, st);
+  if (rc) return rc;
+  h->stream = st; h->state = ST_EVALUATED; h->launches = 0;
+  const CaseDev& c = h->c; const PlanDev& p = h->p;
+  const float *Td = nullptr, *wd = nullptr;
+  rc = copy_inputs(h, T, t_broadcast, weights, K, st, &Td, &wd);
+  if (rc) return rc;
+  LN(h, launch_init_plans(c, p, Td, t_broadcast ? 1 : 0, wd, h->struct_scale, st));
+  float* dose_dev = dose;
+  const bool dose_host = dose && !is_device_ptr(dose);
+  if (dose_host) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dose_dev), (size_t)c.N * K * sizeof(float), st));
+  rc = enqueue_eval(h, dose_dev, nullptr, st);
+  if (rc) return rc;
+  const StepParams sp = make_step_params(h, 0);
+  float* Fd = F ? h->out_F : nullptr;
+  float* gd = grad_x ? h->out_T : nullptr;
+  LN(h, launch_eval_finish_scaled(c, p, sp, g_scale_of(h), Fd, gd, st));
+  bool any_host = dose_host;
+  if (F) { CK(h, cudaMemcpyAsync(F, Fd, (size_t)K * sizeof(float), cudaMemcpyDefault, st)); any_host |= !is_device_ptr(F); }
+  if (grad_x) {
+    CK(h, cudaMemcpyAsync(grad_x, gd, (size_t)K * c.A * sizeof(float), cudaMemcpyDefault, st));
+    any_host |= !is_device_ptr(grad_x);
+  }
+  if (dose_host) {
+    CK(h, cudaMemcpyAsync(dose, dose_dev, (size_t)c.N * K * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CK(h, cudaFreeAsync(dose_dev, st));
+  }
+  CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
+  if (any_host) {
+    CK(h, cudaStreamSynchronize(st));
+    if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T or weights hold a negative, NaN or infinite value%s");
+  }
+  return GMCO_OK;
+}
+
+int gmco_get_stats(const gmco_handle* h, gmco_stats* out) {
+  if (!h || !out) return GMCO_E_INVALID;
+  if (!h->have_stats) return GMCO_E_STATE;
+  *out = h->stats;
+  return GMCO_OK;
+}
+
+}  // extern "C"

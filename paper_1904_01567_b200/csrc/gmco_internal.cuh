@@ -1,0 +1,108 @@
+// gmco_internal.cuh -- device layout, handle and kernel launch prototypes of libgmco.
+// Product code: shares nothing with oracle/.  See DESIGN.md section 4 for the HBM layout.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda.h>
+#include <stdint.h>
+
+#include "gmco.h"
+
+namespace gmco {
+
+constexpr int kChunk = 32;        // points per chunk: K-step granule of the gradient MMA, penalty granule
+constexpr int kStructAlign = 64;  // every structure is padded to a multiple of this many rows
+constexpr int kRowAlloc = 256;    // D rows are allocated up to a multiple of this (tile over-reads stay in bounds)
+constexpr int kPlanTile = 128;    // plans per tensor tile = TMEM lanes
+constexpr int kMaxApad = 480;     // 512 TMEM columns - at least one 32-point chunk of dose accumulator
+constexpr int kMaxNpl = kMaxApad / 32;  // dwell elements per lane in the warp-per-plan kernels
+
+// per-plan status codes on the device
+enum : int { PLAN_RUNNING = -1 };
+
+// Static description of the case (gmco_create), all device pointers.
+struct CaseDev {
+  int N = 0, A = 0, S = 0;          // user sizes
+  int N_pad = 0;                    // sum of structure sizes rounded up to kStructAlign
+  int N_alloc = 0;                  // N_pad rounded up to kRowAlloc (rows that exist in memory)
+  int A_pad = 0;                    // A rounded up to 32
+  float rx = 0.f;
+  float* D = nullptr;               // [N_alloc][A_pad] fp32, padded rows/cols are 0
+  float* D_hi = nullptr;            // [N_alloc][A_pad] tf32 hi part   (tensor path, dose MMA B operand)
+  float* D_lo = nullptr;            // [N_alloc][A_pad] tf32 lo part
+  float* DT_hi = nullptr;           // [A_pad][N_alloc] transposed hi  (tensor path, gradient MMA B operand)
+  float* DT_lo = nullptr;           // [A_pad][N_alloc] transposed lo
+  float* pt_lo = nullptr;           // [N_alloc] D_min of the point's structure (-inf on padding rows)
+  float* pt_hi = nullptr;           // [N_alloc] D_max (+inf on padding rows)
+  int* tile_struct = nullptr;       // [N_alloc / 64] structure id of each 64-row tile (uniform by construction)
+  int* row_src = nullptr;           // [N_alloc] original row index, -1 on padding rows
+  int* sel_pos = nullptr;           // [N_alloc] position inside the D_level selection buffer, -1 if unused
+  int n_sel = 0;                    // total points of dvh_kind == 2 structures
+};
+
+struct StructHost {
+  int n_points, row_begin /*padded*/, n_rows_pad, sel_begin;
+  float d_lo, d_hi, w_lo, w_hi;
+  int dvh_kind; float dvh_level;
+};
+
+// Per-K workspace (gmco_optimize / gmco_evaluate), all [K_pad] or [K_pad][A_pad].
+struct PlanDev {
+  int K = 0, K_pad = 0, m = 0;
+  float *x = nullptr, *g = nullptr, *p = nullptr, *xt = nullptr;   // [K_pad][A_pad]
+  float *T = nullptr, *T_hi = nullptr, *T_lo = nullptr;            // trial dwell times (GEMM operand)
+  float *Sh = nullptr, *Yh = nullptr;                              // [m][K_pad][A_pad] history
+  float *rho = nullptr, *gam = nullptr;                            // [m][K_pad] 1/(s.y) and (s.y)/(y.y)
+  float *Weff = nullptr;                                           // [K_pad][2*S] weights * base / n_s
+  float *F = nullptr, *gp = nullptr, *alpha = nullptr;             // [K_pad]
+  int *it_done = nullptr, *trials = nullptr, *hcount = nullptr, *hhead = nullptr, *status = nullptr;
+  int *n_running = nullptr;                                        // [2] ping-pong counter of RUNNING plans
+  int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
+  // partial results of one evaluation round
+  float *Fpart = nullptr; float *Gpart = nullptr; float *R = nullptr;
+  int nF = 0, nFcomp = 1, nG = 0;                                  // SIMT: slot counts (uniform over plans)
+  // result staging
+  float *res_terms = nullptr;                                      // [K_pad][2*S]
+  int *res_cnt = nullptr;                                          // [K_pad][S]
+  float *res_sel = nullptr;                                        // [K_pad][n_sel]
+  float *res_dvh = nullptr;                                        // [K_pad][S]
+};
+
+struct StepParams {
+  int K, A_pad, m, iters, max_trials;
+  float c1, eps;
+  // partial layout
+  const float* Fpart; int nF, nFcomp; long long f_slot_stride;
+  const float* Gpart; int nG; long long g_slot_stride;
+  int tile_local;                     // 1: partial rows are indexed by plan % 128 and slots come from tile_seg
+  const int* tile_seg;                // [n_tiles + 1] slot range of each plan tile (tensor path)
+};
+
+// ---- kernel launchers (each returns the number of kernels it launched, or < 0 on CUDA error) ----
+int launch_setup_case(const CaseDev& c, const float* D_user, long long ldD, const int* row_src_dev,
+                      bool want_split, cudaStream_t st);
+int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t0_bcast, const float* w_user,
+                      const float* struct_scale /*[2S] base/n*/, cudaStream_t st);
+// gate: device int; the kernel returns at once when *gate == 0 (no plan is running); nullptr = always run
+int launch_simt_eval(const CaseDev& c, const PlanDev& p, bool write_R, float* dose_out /*[N][K] or null*/,
+                     bool dvh_mode, const float* dvh_thr /*[S] device*/, const int* gate, cudaStream_t st);
+int launch_simt_grad(const CaseDev& c, const PlanDev& p, const int* gate, cudaStream_t st);
+int launch_round_begin(const PlanDev& p, int parity, cudaStream_t st);
+int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
+                       cudaStream_t st);
+int launch_eval_finish_scaled(const CaseDev& c, const PlanDev& p, const StepParams& sp, float g_scale, float* F_out,
+                              float* grad_out, cudaStream_t st);
+int launch_result(const CaseDev& c, const PlanDev& p, const StructHost* sh, float* T_out, float* F_out,
+                  float* dvh_out, float* terms_out, int* iters_out, int* status_out, cudaStream_t st);
+int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st);
+
+// tensor path (kernel_fused_tc.cu)
+struct TcPlan;                                   // host-side stream-K schedule + tensor maps
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, int num_sms, char* err, int errlen);
+void tc_plan_destroy(TcPlan*);
+int tc_num_segments(const TcPlan*);
+const int* tc_tile_seg_dev(const TcPlan*);
+int launch_tc_eval(const TcPlan* tp, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
+                   cudaStream_t st);
+
+}  // namespace gmco

@@ -1,0 +1,342 @@
+// kernels_lbfgs.cu -- per-plan state kernels: start point (a1), L-BFGS two-loop recursion (a6),
+// Armijo accept / backtrack, history update and stop test (a7).  One warp per plan; a dwell
+// vector of A_pad <= 480 floats lives in registers (A_pad / 32 per lane), dot products are
+// butterfly reductions in a fixed order, so a plan's trajectory does not depend on K.
+//
+// Algorithm = DESIGN.md section 2.2 (reading A5 of the paper's "description omitted" L-BFGS,
+// PAPER.md:115-119, after Liu & Nocedal 1989).  The batch advances in ROUNDS: in every round each
+// running plan has exactly one trial point x + alpha p evaluated by the contraction kernels; this
+// kernel then either accepts it (history push, new direction, alpha = 1) or halves alpha.
+#include "gmco_internal.cuh"
+
+namespace gmco {
+
+__device__ __forceinline__ float tf32_rn_(float v) {
+  uint32_t u;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
+  return __uint_as_float(u);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int off = 16; off; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  return v;
+}
+
+struct PlanPtrs {
+  float *x, *g, *p, *xt, *T, *T_hi, *T_lo, *Sh, *Yh, *rho, *gam, *F, *gp, *alpha;
+  int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input;
+  int K_pad;
+};
+
+static PlanPtrs make_ptrs(const PlanDev& p) {
+  PlanPtrs q;
+  q.x = p.x; q.g = p.g; q.p = p.p; q.xt = p.xt; q.T = p.T; q.T_hi = p.T_hi; q.T_lo = p.T_lo;
+  q.Sh = p.Sh; q.Yh = p.Yh; q.rho = p.rho; q.gam = p.gam; q.F = p.F; q.gp = p.gp; q.alpha = p.alpha;
+  q.it_done = p.it_done; q.trials = p.trials; q.hcount = p.hcount; q.hhead = p.hhead; q.status = p.status;
+  q.n_running = p.n_running; q.bad_input = p.bad_input; q.K_pad = p.K_pad;
+  return q;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1: x = sqrt(T0), trial point = start point, effective weights, per-plan scalars.
+__global__ void k_init_plans(PlanPtrs pp, int K, int A, int A_pad, int S, const float* __restrict__ T0, int bcast,
+                             const float* __restrict__ w_user, const float* __restrict__ scale, float* __restrict__ Weff) {
+  const int k = blockIdx.x;
+  int bad = 0;
+  for (int a = threadIdx.x; a < A_pad; a += blockDim.x) {
+    float t0 = 0.f;
+    if (k < K && a < A) {
+      t0 = bcast ? T0[a] : T0[(long long)k * A + a];
+      if (!(t0 >= 0.f) || isinf(t0)) { bad = 1; t0 = 0.f; }
+    }
+    const float x = sqrtf(t0), t = x * x, hi = tf32_rn_(t);
+    const long long i = (long long)k * A_pad + a;
+    pp.x[i] = x; pp.xt[i] = x; pp.g[i] = 0.f; pp.p[i] = 0.f;
+    pp.T[i] = t; pp.T_hi[i] = hi; pp.T_lo[i] = tf32_rn_(t - hi);
+  }
+  for (int j = threadIdx.x; j < 2 * S; j += blockDim.x) {
+    float w = 0.f;
+    if (k < K) { w = w_user[(long long)k * 2 * S + j]; if (!(w >= 0.f) || isinf(w)) { bad = 1; w = 0.f; } }
+    Weff[(long long)k * 2 * S + j] = w * scale[j];
+  }
+  if (bad) atomicExch(pp.bad_input, 1);
+  if (threadIdx.x == 0) {
+    pp.F[k] = 0.f; pp.gp[k] = 0.f; pp.alpha[k] = 1.f;
+    pp.it_done[k] = 0; pp.trials[k] = -1;                 // -1: the start point itself is being evaluated
+    pp.hcount[k] = 0; pp.hhead[k] = 0;
+    pp.status[k] = k < K ? PLAN_RUNNING : GMCO_PLAN_ITERS;
+    if (k == 0) { pp.n_running[0] = K; pp.n_running[1] = 0; }
+  }
+}
+
+int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t0_bcast, const float* w_user,
+                      const float* struct_scale, cudaStream_t st) {
+  if (p.K_pad == 0) return 0;
+  cudaMemsetAsync(p.bad_input, 0, sizeof(int), st);
+  k_init_plans<<<p.K_pad, 128, 0, st>>>(make_ptrs(p), p.K, c.A, c.A_pad, c.S, T0, t0_bcast, w_user, struct_scale,
+                                        p.Weff);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fixed-order reduction of the contraction kernels' partial results for plan k.
+template <int NPL>
+__device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, int lane, int npl, float (&G)[NPL]) {
+  int f0 = 0, f1 = sp.nF, g0 = 0, g1 = sp.nG;
+  long long prow = k;
+  if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
+  float f = 0.f;
+  const int nfe = (f1 - f0) * sp.nFcomp;                   // SIMT: (lo, hi) pairs per slot
+  for (int i = lane; i < nfe; i += 32) {
+    const int slot = f0 + i / sp.nFcomp, comp = i % sp.nFcomp;
+    f += sp.Fpart[(long long)slot * sp.f_slot_stride + prow * sp.nFcomp + comp];
+  }
+  f = warp_sum(f);
+#pragma unroll
+  for (int j = 0; j < NPL; ++j) G[j] = 0.f;
+  for (int s = g0; s < g1; ++s) {
+    const float* gp = sp.Gpart + (long long)s * sp.g_slot_stride + prow * sp.A_pad + lane;
+#pragma unroll
+    for (int j = 0; j < NPL; ++j)
+      if (j < npl) G[j] += gp[32 * j];
+  }
+  return f;
+}
+
+// ---------------------------------------------------------------------------------------------
+template <int NPL>
+__global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int parity, float g_scale) {
+  __shared__ float s_a[4][GMCO_MAX_HISTORY];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int k = blockIdx.x * 4 + warp;
+  if (pp.n_running[parity] == 0) return;
+  if (k >= sp.K || pp.status[k] != PLAN_RUNNING) return;
+  const int npl = sp.A_pad >> 5;
+  const long long row = (long long)k * sp.A_pad + lane;
+  const long long hstride = (long long)pp.K_pad * sp.A_pad;
+
+  float G[NPL], xt[NPL], gt[NPL], x[NPL], g[NPL];
+  const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G);
+#pragma unroll
+  for (int j = 0; j < NPL; ++j) {
+    xt[j] = j < npl ? pp.xt[row + 32 * j] : 0.f;
+    gt[j] = g_scale * xt[j] * G[j];                          // Eq. 3 summed: g = 2 x o (D^T r)
+  }
+
+  int tr = pp.trials[k];
+  float F = pp.F[k];
+  int it = pp.it_done[k];
+  int hc = pp.hcount[k], hh = pp.hhead[k];
+  int status = PLAN_RUNNING;
+  bool new_dir = false;
+
+  if (tr < 0) {                                              // start point: nothing to compare against
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) { x[j] = xt[j]; g[j] = gt[j]; }
+    F = Ft;
+    new_dir = true;
+    if (it >= sp.iters) status = GMCO_PLAN_ITERS;
+  } else {
+    const float alpha = pp.alpha[k], gp = pp.gp[k];
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) { x[j] = j < npl ? pp.x[row + 32 * j] : 0.f; g[j] = j < npl ? pp.g[row + 32 * j] : 0.f; }
+    if (Ft <= F + sp.c1 * alpha * gp) {                      // Armijo: accept x+ = x + alpha p
+      float sy = 0.f, ss = 0.f, yy = 0.f;
+      float sv[NPL], yv[NPL];
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) {
+        sv[j] = xt[j] - x[j]; yv[j] = gt[j] - g[j];
+        sy = fmaf(sv[j], yv[j], sy); ss = fmaf(sv[j], sv[j], ss); yy = fmaf(yv[j], yv[j], yy);
+      }
+      sy = warp_sum(sy); ss = warp_sum(ss); yy = warp_sum(yy);
+      if (sy > 1e-10f * sqrtf(ss) * sqrtf(yy)) {             // curvature guard
+        float* Sd = pp.Sh + hh * hstride + row;
+        float* Yd = pp.Yh + hh * hstride + row;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j)
+          if (j < npl) { Sd[32 * j] = sv[j]; Yd[32 * j] = yv[j]; }
+        if (lane == 0) { pp.rho[(long long)hh * pp.K_pad + k] = 1.f / sy; pp.gam[(long long)hh * pp.K_pad + k] = sy / yy; }
+        hh = hh + 1 == sp.m ? 0 : hh + 1;
+        hc = min(hc + 1, sp.m);
+      }
+      const float Fold = F;
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) { x[j] = xt[j]; g[j] = gt[j]; }
+      F = Ft;
+      it += 1;
+      new_dir = true;
+      if (sp.eps > 0.f && fabsf(Fold - F) <= sp.eps * fmaxf(Fold, 1e-30f)) status = GMCO_PLAN_CONVERGED;
+      else if (it >= sp.iters) status = GMCO_PLAN_ITERS;
+    } else {                                                 // reject: halve the step along the same p
+      tr += 1;
+      if (tr >= sp.max_trials) {
+        status = GMCO_PLAN_STALLED;
+      } else {
+        const float a2 = alpha * 0.5f;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j)
+          if (j < npl) {
+            const float pv = pp.p[row + 32 * j];
+            const float xn = fmaf(a2, pv, x[j]), t = xn * xn, hi = tf32_rn_(t);
+            pp.xt[row + 32 * j] = xn; pp.T[row + 32 * j] = t; pp.T_hi[row + 32 * j] = hi; pp.T_lo[row + 32 * j] = tf32_rn_(t - hi);
+          }
+        if (lane == 0) { pp.alpha[k] = a2; pp.trials[k] = tr; }
+      }
+    }
+  }
+
+  if (new_dir) {
+#pragma unroll
+    for (int j = 0; j < NPL; ++j)
+      if (j < npl) { pp.x[row + 32 * j] = x[j]; pp.g[row + 32 * j] = g[j]; }
+    float gg = 0.f;
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) gg = fmaf(g[j], g[j], gg);
+    const float gnorm = sqrtf(warp_sum(gg));
+    if (status == PLAN_RUNNING && gnorm == 0.f) status = GMCO_PLAN_CONVERGED;
+    if (status == PLAN_RUNNING) {
+      // two-loop recursion (Liu & Nocedal 1989): q = g; newest -> oldest; scale; oldest -> newest
+      float q[NPL];
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) q[j] = g[j];
+      for (int i = 0; i < hc; ++i) {
+        int slot = hh - 1 - i; if (slot < 0) slot += sp.m;
+        const float* Sd = pp.Sh + slot * hstride + row;
+        const float* Yd = pp.Yh + slot * hstride + row;
+        float sv[NPL], yv[NPL], d = 0.f;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) d = fmaf(sv[j], q[j], d);
+        const float a = pp.rho[(long long)slot * pp.K_pad + k] * warp_sum(d);
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) q[j] = fmaf(-a, yv[j], q[j]);
+        if (lane == 0) s_a[warp][i] = a;
+      }
+      __syncwarp();
+      int newest = hh - 1; if (newest < 0) newest += sp.m;
+      const float gamma = hc > 0 ? pp.gam[(long long)newest * pp.K_pad + k] : 1.f / gnorm;
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) q[j] *= gamma;
+      for (int i = hc - 1; i >= 0; --i) {
+        int slot = hh - 1 - i; if (slot < 0) slot += sp.m;
+        const float* Sd = pp.Sh + slot * hstride + row;
+        const float* Yd = pp.Yh + slot * hstride + row;
+        float sv[NPL], yv[NPL], d = 0.f;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) d = fmaf(yv[j], q[j], d);
+        const float b = pp.rho[(long long)slot * pp.K_pad + k] * warp_sum(d);
+        const float coef = s_a[warp][i] - b;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) q[j] = fmaf(sv[j], coef, q[j]);
+      }
+      float gpn = 0.f;
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) gpn = fmaf(g[j], -q[j], gpn);
+      gpn = warp_sum(gpn);
+      if (!(gpn < 0.f)) {                                    // not a descent direction: restart from -g/|g|
+        hc = 0;
+        const float inv = 1.f / gnorm;
+        gpn = 0.f;
+#pragma unroll
+        for (int j = 0; j < NPL; ++j) { q[j] = g[j] * inv; gpn = fmaf(g[j], -q[j], gpn); }
+        gpn = warp_sum(gpn);
+      }
+#pragma unroll
+      for (int j = 0; j < NPL; ++j)
+        if (j < npl) {
+          const float pv = -q[j];
+          const float xn = x[j] + pv, t = xn * xn, hi = tf32_rn_(t);
+          pp.p[row + 32 * j] = pv; pp.xt[row + 32 * j] = xn;
+          pp.T[row + 32 * j] = t; pp.T_hi[row + 32 * j] = hi; pp.T_lo[row + 32 * j] = tf32_rn_(t - hi);
+        }
+      if (lane == 0) { pp.gp[k] = gpn; pp.alpha[k] = 1.f; pp.trials[k] = 0; }
+    }
+    if (lane == 0) { pp.F[k] = F; pp.it_done[k] = it; pp.hcount[k] = hc; pp.hhead[k] = hh; }
+  }
+  if (lane == 0) {
+    if (status == PLAN_RUNNING) atomicAdd(&pp.n_running[parity ^ 1], 1);
+    else pp.status[k] = status;
+  }
+}
+
+template <int NPL>
+static void step_launch(const PlanDev& p, const StepParams& sp, int parity, float g_scale, cudaStream_t st) {
+  k_step<NPL><<<(p.K + 3) / 4, 128, 0, st>>>(sp, make_ptrs(p), parity, g_scale);
+}
+
+int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
+                       cudaStream_t st) {
+  if (p.K == 0) return 0;
+  const int npl = c.A_pad / 32;
+  if (npl <= 2) step_launch<2>(p, sp, parity, g_scale, st);
+  else if (npl <= 4) step_launch<4>(p, sp, parity, g_scale, st);
+  else if (npl <= 6) step_launch<6>(p, sp, parity, g_scale, st);
+  else if (npl <= 8) step_launch<8>(p, sp, parity, g_scale, st);
+  else if (npl <= 10) step_launch<10>(p, sp, parity, g_scale, st);
+  else if (npl <= 12) step_launch<12>(p, sp, parity, g_scale, st);
+  else step_launch<kMaxNpl>(p, sp, parity, g_scale, st);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// zero the "next round" counter; runs before the contraction kernels of a round
+__global__ void k_round_begin(int* n_running, int parity) { n_running[parity ^ 1] = 0; }
+
+int launch_round_begin(const PlanDev& p, int parity, cudaStream_t st) {
+  k_round_begin<<<1, 1, 0, st>>>(p.n_running, parity);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// gmco_evaluate: F and dF/dx of the trial point from the partials.
+template <int NPL>
+__global__ void __launch_bounds__(128) k_eval_finish(StepParams sp, const float* __restrict__ xt, int A, float g_scale,
+                                                     float* __restrict__ F_out, float* __restrict__ grad_out) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int k = blockIdx.x * 4 + warp;
+  if (k >= sp.K) return;
+  const int npl = sp.A_pad >> 5;
+  float G[NPL];
+  const float F = reduce_partials<NPL>(sp, k, lane, npl, G);
+  if (lane == 0 && F_out) F_out[k] = F;
+  if (grad_out) {
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) {
+      const int a = lane + 32 * j;
+      if (j < npl && a < A) grad_out[(long long)k * A + a] = g_scale * xt[(long long)k * sp.A_pad + a] * G[j];
+    }
+  }
+}
+
+int launch_eval_finish_scaled(const CaseDev& c, const PlanDev& p, const StepParams& sp, float g_scale, float* F_out,
+                              float* grad_out, cudaStream_t st) {
+  if (p.K == 0) return 0;
+  const int npl = c.A_pad / 32;
+  const int grid = (p.K + 3) / 4;
+  if (npl <= 4) k_eval_finish<4><<<grid, 128, 0, st>>>(sp, p.xt, c.A, g_scale, F_out, grad_out);
+  else if (npl <= 8) k_eval_finish<8><<<grid, 128, 0, st>>>(sp, p.xt, c.A, g_scale, F_out, grad_out);
+  else if (npl <= 12) k_eval_finish<12><<<grid, 128, 0, st>>>(sp, p.xt, c.A, g_scale, F_out, grad_out);
+  else k_eval_finish<kMaxNpl><<<grid, 128, 0, st>>>(sp, p.xt, c.A, g_scale, F_out, grad_out);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8 prologue: dwell times of the ACCEPTED point (not the last trial) for the final dose pass.
+__global__ void k_prepare_final(const float* __restrict__ x, float* __restrict__ T, long long n, int* __restrict__ cnt,
+                                long long ncnt) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { const float v = x[i]; T[i] = v * v; }
+  if (i < ncnt) cnt[i] = 0;
+}
+
+int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st) {
+  if (p.K_pad == 0) return 0;
+  const long long n = (long long)p.K_pad * c.A_pad, ncnt = (long long)p.K_pad * c.S;
+  k_prepare_final<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p.x, p.T, n, p.res_cnt, ncnt);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace gmco

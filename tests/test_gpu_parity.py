@@ -1,0 +1,259 @@
+"""-m gpu: element-by-element parity of the CUDA path (through the C ABI) with the fp64 oracle.
+
+Tolerances are the north_star's: per evaluation dose / objective / gradient within 1e-4 relative
+(gradient norm-wise per plan at non-converged points, reading A18); after a fixed iteration count
+final objective within 1e-3 relative and DVH indices within 0.5 percentage points.
+"""
+import numpy as np
+import pytest
+
+import gmco_cases as gc
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL_EVAL = 1e-4
+TOL_F_FINAL = 1e-3
+TOL_DVH_PP = 0.5
+
+
+@pytest.fixture(scope="module")
+def g():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a B200"
+    import paper_1904_01567_b200 as g
+    from paper_1904_01567_b200 import build
+    build.build()
+    return g
+
+
+PRECISIONS = [pytest.param(1, id="simt_fp32"), pytest.param(0, id="tf32x3")]
+
+
+def _opts(g, prec, **kw):
+    return g.binding.make_options(precision=prec, **kw)
+
+
+def _eval_points(case, n_random=3):
+    """Non-converged evaluation points: uniform start, random starts, the oracle's iterate 5."""
+    K = case.n_plans
+    pts = [np.repeat(case.T0[None], K, axis=0)]
+    for s in range(n_random):
+        pts.append(np.repeat(gc.random_starts(case, 1, seed=100 + s), K, axis=0) * np.linspace(0.5, 1.5, K)[:, None].astype(np.float32))
+    it5 = oracle.optimize(case.D, case.structures, case.rx, case.T0, case.weights, m=case.m, iters=5)["T"]
+    pts.append(it5.astype(np.float32))
+    return pts
+
+
+def _check_eval(g, case, prec, T):
+    ref = oracle.evaluate(case.D, case.structures, T, case.weights)
+    h = g.gmco_create(case.D, case.structures, case.rx, _opts(g, prec, m=case.m))
+    try:
+        out = g.gmco_evaluate(h, T, case.weights, want_dose=True, want_grad=True, host=True)
+    finally:
+        g.gmco_destroy(h)
+    dose_err = np.abs(out["dose"] - ref["dose"]) / np.abs(ref["dose"])
+    assert dose_err.max() < TOL_EVAL, f"dose {dose_err.max():.3e}"
+    f_err = np.abs(out["F"] - ref["F"]) / ref["F"]
+    assert f_err.max() < TOL_EVAL, f"F {f_err.max():.3e}"
+    gn = np.linalg.norm(out["grad_x"] - ref["grad_x"], axis=1) / np.linalg.norm(ref["grad_x"], axis=1)
+    assert gn.max() < TOL_EVAL, f"grad {gn.max():.3e}"
+    return dose_err.max(), f_err.max(), gn.max()
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_evaluation_parity_c1(g, prec, case_c1):
+    for T in _eval_points(case_c1):
+        _check_eval(g, case_c1, prec, T)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_evaluation_parity_ragged_shapes(g, prec):
+    """Several tiles and ragged tails in every dimension: N not a multiple of 64 per structure,
+    A = 5 x 9 = 45 (pads to 64), K = 130 (two plan tiles, the second almost empty)."""
+    c = gc.make_case("C1", n_cath=5, n_pos=9, counts=(333, 65, 127, 70), n_plans=130, seed_points=77, seed_weights=78)
+    for T in _eval_points(c, n_random=1):
+        _check_eval(g, c, prec, T)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_evaluation_parity_max_dwell_count(g, prec):
+    """The paper's largest N_act is 385: A = 385 pads to 416."""
+    c = gc.make_case("C1", n_cath=35, n_pos=11, counts=(300, 64, 100, 100), n_plans=5, seed_points=5)
+    assert c.n_dwell == 385
+    _check_eval(g, c, prec, np.repeat(c.T0[None], 5, axis=0))
+
+
+def _check_optimize(g, case, prec, iters=None, sample=None):
+    iters = case.iters if iters is None else iters
+    h = g.gmco_create(case.D, case.structures, case.rx, _opts(g, prec, m=case.m))
+    try:
+        g.gmco_optimize(h, case.T0, case.weights, iters)
+        out = g.gmco_result(h, host=True)
+        stats = g.gmco_get_stats(h)
+    finally:
+        g.gmco_destroy(h)
+    idx = np.arange(case.n_plans) if sample is None else np.asarray(sample)
+    ref = oracle.optimize(case.D, case.structures, case.rx, case.T0, case.weights[idx], m=case.m, iters=iters)
+    f_err = np.abs(out["objective"][idx] - ref["F"]) / ref["F"]
+    dvh_err = np.abs(out["dvh"][idx] - ref["dvh"])
+    assert (out["iters_done"][idx] == ref["iters_done"]).all()
+    assert f_err.max() < TOL_F_FINAL, f"final F {f_err.max():.3e}"
+    assert dvh_err.max() < TOL_DVH_PP, f"DVH {dvh_err.max():.3f} pp"
+    assert (out["T"] >= 0).all() and np.isfinite(out["T"]).all()
+    assert out["objective_terms"].sum(axis=(1, 2)) == pytest.approx(out["objective"], rel=1e-5)
+    assert stats["kernel_launches"] > 0 and stats["rounds"] >= 1 + iters
+    return out, ref, stats
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_optimize_parity_c1(g, prec, case_c1):
+    _check_optimize(g, case_c1, prec)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_optimize_parity_c2(g, prec):
+    _check_optimize(g, gc.make_case("C2"), prec)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_optimize_parity_c3_sampled(g, prec):
+    """BASELINE.json configs[2] at full size, in the configuration bench.py times; the oracle
+    checks a sample of plans one by one (plans are independent)."""
+    c = gc.make_case("C3")
+    _check_optimize(g, c, prec, sample=[0, 1, 127, 128, 500, 777, 998, 999])
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_iters_zero_is_an_evaluation(g, prec, case_c1):
+    c = case_c1
+    h = g.gmco_create(c.D, c.structures, c.rx, _opts(g, prec))
+    try:
+        g.gmco_optimize(h, c.T0, c.weights, 0)
+        out = g.gmco_result(h, host=True)
+    finally:
+        g.gmco_destroy(h)
+    ref = oracle.evaluate(c.D, c.structures, c.T0, c.weights)
+    assert out["objective"] == pytest.approx(ref["F"], rel=TOL_EVAL)
+    assert out["T"] == pytest.approx(np.repeat(c.T0[None], c.n_plans, 0), rel=1e-6)
+    assert (out["iters_done"] == 0).all()
+    d = oracle.evaluate(c.D, c.structures, c.T0, c.weights)["dose"]
+    ref_dvh = np.stack([oracle.dvh(d[:, k], c.structures, c.rx) for k in range(c.n_plans)])
+    assert np.abs(out["dvh"] - ref_dvh).max() < TOL_DVH_PP
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_empty_batch_and_single_plan(g, prec, case_c1):
+    c = case_c1
+    h = g.gmco_create(c.D, c.structures, c.rx, _opts(g, prec, m=c.m))
+    try:
+        g.gmco_optimize(h, c.T0, c.weights[:0], 10)
+        out = g.gmco_result(h, host=True)
+        assert out["T"].shape == (0, c.n_dwell)
+        g.gmco_optimize(h, c.T0, c.weights[3:4], 20)
+        one = g.gmco_result(h, host=True)
+    finally:
+        g.gmco_destroy(h)
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights[3:4], m=c.m, iters=20)
+    assert one["objective"] == pytest.approx(ref["F"], rel=TOL_F_FINAL)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_zero_penalty_plan_returns_the_start(g, prec, case_small):
+    c = case_small
+    d = c.D.astype(np.float64) @ c.T0.astype(np.float64)
+    st, o = [], 0
+    for s in c.structures:
+        dd = d[o:o + s.n_points]; o += s.n_points
+        st.append(gc.Structure(s.name, s.n_points, float(dd.min()) - 1e-2, float(dd.max()) + 1e-2, 2.0, 3.0, s.dvh_kind, s.dvh_level))
+    h = g.gmco_create(c.D, st, c.rx, _opts(g, prec))
+    try:
+        g.gmco_optimize(h, c.T0, np.ones((3, 4, 2), np.float32), 25)
+        out = g.gmco_result(h, host=True)
+    finally:
+        g.gmco_destroy(h)
+    assert (out["objective"] == 0).all() and (out["iters_done"] == 0).all() and (out["plan_status"] == 1).all()
+    assert out["T"] == pytest.approx(np.repeat(c.T0[None], 3, 0), rel=1e-6)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_dwell_at_zero_stays_at_zero_and_times_stay_nonnegative(g, prec, case_small):
+    c = case_small
+    T0 = np.repeat(c.T0[None], c.n_plans, axis=0).copy(); T0[:, [3, 17]] = 0.0
+    h = g.gmco_create(c.D, c.structures, c.rx, _opts(g, prec, m=5))
+    try:
+        g.gmco_optimize(h, T0, c.weights, 30)
+        out = g.gmco_result(h, host=True)
+    finally:
+        g.gmco_destroy(h)
+    assert (out["T"][:, [3, 17]] == 0).all() and (out["T"] >= 0).all()
+    ref = oracle.optimize(c.D, c.structures, c.rx, T0, c.weights, m=5, iters=30)
+    assert out["objective"] == pytest.approx(ref["F"], rel=TOL_F_FINAL)
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_plan_independence_and_determinism(g, prec, case_c1):
+    c = case_c1
+    def run(w):
+        h = g.gmco_create(c.D, c.structures, c.rx, _opts(g, prec, m=c.m))
+        try:
+            g.gmco_optimize(h, c.T0, w, 15)
+            return g.gmco_result(h, host=True)
+        finally:
+            g.gmco_destroy(h)
+    a, b = run(c.weights), run(c.weights)
+    assert (a["T"] == b["T"]).all() and (a["objective"] == b["objective"]).all()     # reruns are bit-identical
+    one = run(c.weights[5:6])
+    assert one["objective"][0] == pytest.approx(a["objective"][5], rel=1e-5)
+    if prec == 1:   # the SIMT route sums in an order that does not depend on K
+        assert (one["T"][0] == a["T"][5]).all()
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_eps_stopping_rule(g, prec, case_c1):
+    c = case_c1
+    res = {}
+    for eps in (1e-2, 1e-4):
+        h = g.gmco_create(c.D, c.structures, c.rx, _opts(g, prec, m=c.m, eps=eps))
+        try:
+            g.gmco_optimize(h, c.T0, c.weights, 200)
+            res[eps] = g.gmco_result(h, host=True)
+        finally:
+            g.gmco_destroy(h)
+    assert (res[1e-2]["iters_done"] <= res[1e-4]["iters_done"]).all()
+    assert (res[1e-2]["iters_done"] < 200).all() and (res[1e-2]["plan_status"] == 1).all()
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=200, eps=1e-2)
+    assert np.abs(res[1e-2]["iters_done"] - ref["iters_done"]).max() <= 2
+
+
+def test_invalid_inputs_are_rejected(g, case_small):
+    c = case_small
+    h = g.gmco_create(c.D, c.structures, c.rx)
+    try:
+        bad = np.repeat(c.T0[None], c.n_plans, 0).copy(); bad[1, 2] = np.nan
+        with pytest.raises(g.GmcoError) as e:
+            g.gmco_optimize(h, bad, c.weights, 3)
+        assert e.value.code == -1
+        with pytest.raises(g.GmcoError) as e:
+            g.gmco_optimize(h, c.T0, -c.weights, 3)
+        assert e.value.code == -1
+        with pytest.raises(g.GmcoError) as e:
+            g.gmco_result(h)
+        assert e.value.code == -5
+    finally:
+        g.gmco_destroy(h)
+
+
+def test_device_resident_inputs_and_outputs(g, case_c1):
+    import torch
+    c = case_c1
+    D = torch.from_numpy(c.D).cuda(); T0 = torch.from_numpy(c.T0).cuda(); w = torch.from_numpy(c.weights).cuda()
+    h = g.gmco_create(D, c.structures, c.rx, _opts(g, 1, m=c.m))
+    try:
+        g.gmco_optimize(h, T0, w, c.iters)
+        dev = g.gmco_result(h)
+    finally:
+        g.gmco_destroy(h)
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=c.iters)
+    assert dev["objective"].is_cuda
+    assert dev["objective"].cpu().numpy() == pytest.approx(ref["F"], rel=TOL_F_FINAL)
