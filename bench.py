@@ -188,9 +188,10 @@ def main():
     def step(host: bool, profile: bool = False):
         Dm, Tm, wm, om = (D_pin, T0_pin, w_pin, out_pin) if host else (D_dev, T0_dev, w_dev, out_dev)
         opt = g.binding.make_options(m=case.m, precision=prec)
-        opt.reserved[0] = 1 if profile else 0
         h = g.gmco_create(Dm, case.structures, case.rx, opt, stream)
         try:
+            if profile:
+                g.gmco_set_profiling(h, True)
             g.gmco_optimize(h, Tm, wm, case.iters, stream)
             g.binding._check(L.gmco_result(h.ptr, om["T"].data_ptr(), om["F"].data_ptr(), om["dvh"].data_ptr(),
                                            om["terms"].data_ptr(), om["it"].data_ptr(), om["st"].data_ptr()), h)
@@ -274,21 +275,21 @@ def roofline(case, prec, g, prof, peaks):
     Algorithmic flops per launch = 4 N A K (one D t and one D^T r per plan); the 3xTF32
     split issues 3x that on the tensor pipe.  Peak: measured bf16 (sustained: the kernel runs inside a
     long step) x the guide's nominal tf32/bf16 ratio 1.1/2.25; SIMT: 148 SM x 128 lanes x 2 x 1.965 GHz."""
-    if not prof or not prof.get("reserved_eval_launches"):
+    if not prof or not prof.get("eval_launches"):
         return None
     flops = 4.0 * case.n_points * case.n_dwell * case.n_plans
-    ms = prof["reserved_eval_ms"] / prof["reserved_eval_launches"]
+    ms = prof["eval_ms"] / prof["eval_launches"]
     if prec == g.GMCO_PREC_TF32X3:
         peak = peaks["bf16_sustained"] * (1.1 / 2.25)
         issued = 3.0 * flops / (ms * 1e-3) / 1e12
         return {"bound": "tensor", "kernel": "k_fused_tc (dose GEMM + penalty + gradient GEMM)",
                 "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
-                "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["reserved_eval_launches"],
+                "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["eval_launches"],
                 "peak_source": f"{peaks['source']} bf16 sustained x 1.1/2.25 (nominal tf32:bf16)", "traffic": None}
     peak = 148 * 128 * 2 * 1.965e9 / 1e12
     ach = flops / (ms * 1e-3) / 1e12
     return {"bound": "alu", "kernel": "k_simt_dose + k_simt_grad", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-            "frac": ach / peak, "avg_launch_ms": ms, "launches": prof["reserved_eval_launches"],
+            "frac": ach / peak, "avg_launch_ms": ms, "launches": prof["eval_launches"],
             "peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": None}
 
 

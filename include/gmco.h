@@ -83,7 +83,11 @@ typedef struct gmco_options {
   float c1;           /* Armijo constant                                      default 1e-4        */
   int32_t max_trials; /* step halvings before a plan is declared stalled      default 20          */
   int32_t precision;  /* gmco_precision                                       default TF32X3      */
-  int32_t reserved[3];/* must be 0                                                                */
+  float eps_f;        /* objective-noise allowance of the approximate line-search test: a trial
+                         step that fails Armijo is still accepted when F+ <= F + eps_f |F| and
+                         g+.p <= (2 c1 - 1) g.p (Hager & Zhang 2005; reading A5b).
+                         0 = Armijo only                                      default 1e-6        */
+  int32_t reserved[2];/* must be 0                                                                */
 } gmco_options;
 
 /* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */
@@ -92,7 +96,9 @@ typedef struct gmco_stats {
   int32_t rounds;           /* evaluation rounds executed (1 + iterations + backtracks of the slowest plan) */
   int32_t kernel_launches;  /* kernels launched by the library since gmco_optimize was called     */
   int32_t plans_iters, plans_converged, plans_stalled;
-  int32_t reserved[3];
+  int32_t eval_launches;    /* profiling only: contraction launches that had work (see gmco_set_profiling) */
+  float eval_ms;            /* profiling only: summed device time of those launches, CUDA events  */
+  int32_t reserved[1];
 } gmco_stats;
 
 typedef struct gmco_handle gmco_handle;
@@ -139,6 +145,13 @@ GMCO_API int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, 
 
 /* Counters of the last optimise/result pair.  GMCO_E_STATE before the first gmco_result. */
 GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);
+
+/* Measurement aid (bench.py's roofline leg).  With enable != 0 every contraction launch of the
+ * following gmco_optimize / gmco_result (the kernels that compute D t, the penalty and D^T r) is
+ * bracketed by a pair of CUDA events on the caller's stream; gmco_result sums their elapsed
+ * times over the rounds in which at least one plan was running and reports them in gmco_stats
+ * (eval_ms, eval_launches).  Off by default; results are identical either way. */
+GMCO_API int gmco_set_profiling(gmco_handle* h, int32_t enable);
 
 /* Frees everything the handle owns (synchronises its stream first).  NULL is a no-op. */
 GMCO_API void gmco_destroy(gmco_handle* h);

@@ -40,13 +40,15 @@ class OrcStruct(C.Structure):
 
 class LbfgsOpt(C.Structure):
     _fields_ = [("m", C.c_int32), ("iters", C.c_int32), ("eps", C.c_double), ("c1", C.c_double),
-                ("max_trials", C.c_int32)]
+                ("max_trials", C.c_int32), ("eps_f", C.c_double)]
 
 
 class LbfgsStat(C.Structure):
     _fields_ = [("iters_done", C.c_int32), ("status", C.c_int32), ("n_evals", C.c_int32),
-                ("n_backtracks", C.c_int32), ("n_skipped", C.c_int32)]
+                ("n_backtracks", C.c_int32), ("n_skipped", C.c_int32), ("n_approx", C.c_int32)]
 
+
+EPS_F = 1e-6   # default objective-noise allowance of the approximate line-search test (reading A5b)
 
 FG_FN = C.CFUNCTYPE(C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p)
 
@@ -107,7 +109,7 @@ def evaluate(D, structures, T, weights, want_dose=True):
     return dict(F=F, dose=dose, Fterm=Ft, grad_x=gx, G=G)
 
 
-def lbfgs(fg, x0, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20):
+def lbfgs(fg, x0, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20, eps_f=EPS_F):
     """Generic driver on a Python objective fg(x) -> (F, g); used to PIN the driver."""
     x = np.array(x0, dtype=np.float64); n = x.size
 
@@ -118,20 +120,20 @@ def lbfgs(fg, x0, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20):
         return float(F)
 
     cb = FG_FN(_cb)
-    opt = LbfgsOpt(m, iters, eps, c1, max_trials); st = LbfgsStat()
+    opt = LbfgsOpt(m, iters, eps, c1, max_trials, eps_f); st = LbfgsStat()
     Ff = C.c_double(); hist = np.empty(iters + 1)
     lib().orc_lbfgs(cb, None, C.c_int64(n), _p(x), C.byref(opt), C.byref(Ff), _p(hist), C.byref(st))
     return dict(x=x, F=Ff.value, F_hist=hist, iters_done=st.iters_done, status=st.status,
-                n_evals=st.n_evals, n_backtracks=st.n_backtracks, n_skipped=st.n_skipped)
+                n_evals=st.n_evals, n_backtracks=st.n_backtracks, n_skipped=st.n_skipped, n_approx=st.n_approx)
 
 
 def optimize(D, structures, rx, T0, weights, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20,
-             want_hist=False):
+             want_hist=False, eps_f=EPS_F):
     """K plans of gL-BFGS from dwell times T0 ([K, A] or [A]).  Returns dict of fp64 arrays."""
     D = _f32(D); N, A = D.shape; S = len(structures)
     weights = _f32(weights).reshape(-1, S, 2); K = weights.shape[0]
     T0 = _f32(T0); bc = 1 if T0.ndim == 1 else 0
-    opt = LbfgsOpt(m, iters, eps, c1, max_trials)
+    opt = LbfgsOpt(m, iters, eps, c1, max_trials, eps_f)
     T = np.empty((K, A)); F = np.empty(K); dvh = np.empty((K, S)); Ft = np.empty((K, S, 2))
     stats = (LbfgsStat * K)(); hist = np.empty((K, iters + 1)) if want_hist else None
     rc = lib().orc_optimize(_p(D, C.c_float), C.c_int64(N), C.c_int64(A), _structs(structures),
@@ -145,7 +147,8 @@ def optimize(D, structures, rx, T0, weights, m=10, iters=100, eps=0.0, c1=1e-4, 
                 status=np.array([s.status for s in stats]),
                 n_evals=np.array([s.n_evals for s in stats]),
                 n_backtracks=np.array([s.n_backtracks for s in stats]),
-                n_skipped=np.array([s.n_skipped for s in stats]))
+                n_skipped=np.array([s.n_skipped for s in stats]),
+                n_approx=np.array([s.n_approx for s in stats]))
 
 
 def dvh(dose, structures, rx):

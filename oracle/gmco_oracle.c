@@ -45,6 +45,7 @@ typedef struct {
   double eps;            /* 0 = run exactly iters (PAPER.md:119 stopping rule, A6)     */
   double c1;             /* Armijo constant, 1e-4                                      */
   int32_t max_trials;    /* 20                                                         */
+  double eps_f;          /* relative objective-noise allowance of the approximate test (A5b); 0 = Armijo only */
 } orc_lbfgs_opt;
 
 typedef struct {
@@ -53,6 +54,7 @@ typedef struct {
   int32_t n_evals;       /* objective/gradient evaluations, start point included       */
   int32_t n_backtracks;  /* rejected trial steps                                       */
   int32_t n_skipped;     /* (s, y) pairs rejected by the curvature guard               */
+  int32_t n_approx;      /* steps accepted by the approximate test only (A5b)          */
 } orc_lbfgs_stat;
 
 int orc_num_threads(void) {
@@ -169,7 +171,7 @@ int orc_lbfgs(orc_fg_fn fg, void* ctx, int64_t n, double* x, const orc_lbfgs_opt
   double* rho = (double*)malloc(sizeof(double) * (m > 0 ? m : 1));
   double* a = (double*)malloc(sizeof(double) * (m > 0 ? m : 1));
   int h = 0;                                    /* pairs held, index 0 = oldest, h-1 = newest */
-  orc_lbfgs_stat s = {0, 0, 0, 0, 0};
+  orc_lbfgs_stat s = {0, 0, 0, 0, 0, 0};
 
   double F = fg(x, g, ctx); s.n_evals = 1;
   if (F_hist) F_hist[0] = F;
@@ -204,13 +206,19 @@ int orc_lbfgs(orc_fg_fn fg, void* ctx, int64_t n, double* x, const orc_lbfgs_opt
       gp = dot(g, p, n);
     }
 
-    /* backtracking Armijo line search: alpha = 1, 1/2, 1/4, ...; phi(alpha) = F(x + alpha p) */
+    /* backtracking line search: alpha = 1, 1/2, 1/4, ...; phi(alpha) = F(x + alpha p).
+     * A trial step is accepted by the Armijo test, or -- reading A5b, the "approximate Wolfe"
+     * test of Hager & Zhang (2005), needed once the decrease per step falls below what the
+     * objective can resolve -- when F has not risen by more than eps_f |F| and the slope at the
+     * trial point satisfies phi'(alpha) <= (2 c1 - 1) phi'(0) (identical to Armijo for a quadratic phi). */
     double alpha = 1.0, Fn = 0.0;
     int accepted = 0;
     for (int trial = 0; trial < opt->max_trials; ++trial) {
       for (int64_t l = 0; l < n; ++l) xn[l] = x[l] + alpha * p[l];
       Fn = fg(xn, gn, ctx); s.n_evals++;
       if (Fn <= F + opt->c1 * alpha * gp) { accepted = 1; break; }
+      if (opt->eps_f > 0.0 && Fn <= F + opt->eps_f * fabs(F) &&
+          dot(gn, p, n) <= (2.0 * opt->c1 - 1.0) * gp) { accepted = 1; s.n_approx++; break; }
       s.n_backtracks++;
       alpha *= 0.5;
     }

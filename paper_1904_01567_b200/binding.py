@@ -24,13 +24,13 @@ class _Structure(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
-                ("precision", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("precision", C.c_int32), ("eps_f", C.c_float), ("reserved", C.c_int32 * 2)]
 
 
 class Stats(C.Structure):
     _fields_ = [("device_bytes", C.c_int64), ("rounds", C.c_int32), ("kernel_launches", C.c_int32),
                 ("plans_iters", C.c_int32), ("plans_converged", C.c_int32), ("plans_stalled", C.c_int32),
-                ("reserved", C.c_int32 * 3)]
+                ("eval_launches", C.c_int32), ("eval_ms", C.c_float), ("reserved", C.c_int32 * 1)]
 
 
 def lib_path() -> Path:
@@ -60,6 +60,7 @@ def lib():
         L.gmco_result.argtypes = [vp, fp, fp, fp, fp, vp, vp]
         L.gmco_evaluate.argtypes = [vp, fp, i32, fp, i32, fp, fp, fp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.gmco_set_profiling.argtypes = [vp, i32]
         L.gmco_destroy.argtypes = [vp]
         L.gmco_destroy.restype = None
         L.gmco_last_error.argtypes = [vp]
@@ -112,10 +113,12 @@ def _stream(stream):
     return getattr(stream, "cuda_stream", stream)
 
 
-def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3) -> Options:
+def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None) -> Options:
     o = Options()
     lib().gmco_default_options(C.byref(o))
     o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
+    if eps_f is not None:
+        o.eps_f = eps_f
     return o
 
 
@@ -189,6 +192,10 @@ def gmco_get_stats(h: Handle) -> dict:
     s = Stats()
     _check(lib().gmco_get_stats(h.ptr, C.byref(s)), h)
     return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+
+
+def gmco_set_profiling(h: Handle, enable: bool) -> None:
+    _check(lib().gmco_set_profiling(h.ptr, 1 if enable else 0), h)
 
 
 def gmco_destroy(h: Handle) -> None:

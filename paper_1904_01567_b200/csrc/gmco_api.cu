@@ -52,6 +52,9 @@ struct gmco_handle {
   int iters = 0, rounds_enqueued = 0, launches = 0;
   gmco_stats stats{};
   bool have_stats = false;
+  bool profile = false;              // gmco_set_profiling
+  std::vector<cudaEvent_t> ev;       // 2 per profiled round
+  int ev_used = 0;
   char err[512] = "";
 };
 
@@ -134,6 +137,7 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   p.it_done = a.take<int>(kp); p.trials = a.take<int>(kp); p.hcount = a.take<int>(kp); p.hhead = a.take<int>(kp);
   p.status = a.take<int>(kp);
   p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1);
+  p.round_log = a.take<int>(kRoundLogCap);
   // partials: the SIMT dose pass (also the final pass of gmco_result) needs [tiles][K_pad][2]
   const size_t f_simt = (size_t)(c.N_alloc / 64) * kp * 2;
   p.nFcomp = 2; p.nF = c.N_alloc / 64;
@@ -186,7 +190,7 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
   StepParams sp{};
   const PlanDev& p = h->p; const CaseDev& c = h->c;
   sp.K = p.K; sp.A_pad = c.A_pad; sp.m = p.m; sp.iters = iters; sp.max_trials = h->opt.max_trials;
-  sp.c1 = h->opt.c1; sp.eps = h->opt.eps;
+  sp.c1 = h->opt.c1; sp.eps = h->opt.eps; sp.eps_f = h->opt.eps_f;
   sp.Fpart = p.Fpart; sp.Gpart = p.Gpart;
   if (h->opt.precision == GMCO_PREC_SIMT_FP32) {
     sp.nF = p.nF; sp.nFcomp = 2; sp.f_slot_stride = (long long)p.K_pad * 2;
@@ -217,9 +221,19 @@ int enqueue_rounds(gmco_handle* h, int n, cudaStream_t st) {
   const StepParams sp = make_step_params(h, h->iters);
   for (int i = 0; i < n; ++i) {
     const int parity = h->rounds_enqueued & 1;
-    LN(h, launch_round_begin(h->p, parity, st));
+    LN(h, launch_round_begin(h->p, parity, h->rounds_enqueued, st));
+    const bool prof = h->profile && h->rounds_enqueued < kRoundLogCap;
+    if (prof) {
+      while ((int)h->ev.size() < h->ev_used + 2) {
+        cudaEvent_t e;
+        CK(h, cudaEventCreate(&e));
+        h->ev.push_back(e);
+      }
+      CK(h, cudaEventRecord(h->ev[h->ev_used], st));
+    }
     int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, st);
     if (rc) return rc;
+    if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
     LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
     h->rounds_enqueued++;
   }
@@ -256,7 +270,7 @@ int gmco_version(void) { return GMCO_VERSION; }
 void gmco_default_options(gmco_options* o) {
   if (!o) return;
   memset(o, 0, sizeof(*o));
-  o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3;
+  o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f;
 }
 
 const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
@@ -276,8 +290,8 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   gmco_default_options(&o);
   if (opt) o = *opt;
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
-      (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || o.reserved[0] || o.reserved[1] ||
-      o.reserved[2])
+      !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
+      (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || o.reserved[0] || o.reserved[1])
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   long long tot = 0;
   for (int s = 0; s < n_structs; ++s) {
@@ -387,9 +401,16 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   return GMCO_OK;
 }
 
+int gmco_set_profiling(gmco_handle* h, int32_t enable) {
+  if (!h) return GMCO_E_INVALID;
+  h->profile = enable != 0;
+  return GMCO_OK;
+}
+
 void gmco_destroy(gmco_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   if (h->tc) tc_plan_destroy(h->tc);
   arena_free(h->plan_arena, h->stream);
   arena_free(h->case_arena, h->stream);
@@ -406,7 +427,7 @@ int gmco_optimize(gmco_handle* h, const float* T0, int32_t t0_broadcast, const f
   int rc = ensure_plans(h, K, st);
   if (rc) return rc;
   h->stream = st; h->iters = iters; h->rounds_enqueued = 0; h->launches = 0; h->have_stats = false;
-  h->state = ST_CREATED;
+  h->state = ST_CREATED; h->ev_used = 0;
   if (K == 0) { h->state = ST_OPTIMIZED; return GMCO_OK; }
   const float *T0d = nullptr, *wd = nullptr;
   rc = copy_inputs(h, T0, t0_broadcast, weights, K, st, &T0d, &wd);
@@ -471,6 +492,19 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
       if (stv[k] == GMCO_PLAN_ITERS) s.plans_iters++;
       else if (stv[k] == GMCO_PLAN_CONVERGED) s.plans_converged++;
       else s.plans_stalled++;
+    }
+    if (h->profile && h->ev_used > 0) {
+      const int nr = h->ev_used / 2;
+      std::vector<int> log(nr);
+      CK(h, cudaMemcpy(log.data(), p.round_log, (size_t)nr * sizeof(int), cudaMemcpyDeviceToHost));
+      double ms = 0.0;
+      for (int r = 0; r < nr; ++r) {
+        if (log[r] <= 0) continue;                         // nothing was running: the launch returned at once
+        float t = 0.f;
+        CK(h, cudaEventElapsedTime(&t, h->ev[2 * r], h->ev[2 * r + 1]));
+        ms += t; s.eval_launches++;
+      }
+      s.eval_ms = (float)ms;
     }
     h->stats = s; h->have_stats = true;
   }

@@ -16,6 +16,7 @@ constexpr int kRowAlloc = 256;    // D rows are allocated up to a multiple of th
 constexpr int kPlanTile = 128;    // plans per tensor tile = TMEM lanes
 constexpr int kMaxApad = 480;     // 512 TMEM columns - at least one 32-point chunk of dose accumulator
 constexpr int kMaxNpl = kMaxApad / 32;  // dwell elements per lane in the warp-per-plan kernels
+constexpr int kRoundLogCap = 8192;      // rounds whose running-plan count is logged (profiling aid)
 
 // per-plan status codes on the device
 enum : int { PLAN_RUNNING = -1 };
@@ -57,6 +58,7 @@ struct PlanDev {
   float *F = nullptr, *gp = nullptr, *alpha = nullptr;             // [K_pad]
   int *it_done = nullptr, *trials = nullptr, *hcount = nullptr, *hhead = nullptr, *status = nullptr;
   int *n_running = nullptr;                                        // [2] ping-pong counter of RUNNING plans
+  int *round_log = nullptr;                                        // [kRoundLogCap] running plans at the start of round r
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
   // partial results of one evaluation round
   float *Fpart = nullptr; float *Gpart = nullptr; float *R = nullptr;
@@ -70,7 +72,7 @@ struct PlanDev {
 
 struct StepParams {
   int K, A_pad, m, iters, max_trials;
-  float c1, eps;
+  float c1, eps, eps_f;
   // partial layout
   const float* Fpart; int nF, nFcomp; long long f_slot_stride;
   const float* Gpart; int nG; long long g_slot_stride;
@@ -87,7 +89,7 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
 int launch_simt_eval(const CaseDev& c, const PlanDev& p, bool write_R, float* dose_out /*[N][K] or null*/,
                      bool dvh_mode, const float* dvh_thr /*[S] device*/, const int* gate, cudaStream_t st);
 int launch_simt_grad(const CaseDev& c, const PlanDev& p, const int* gate, cudaStream_t st);
-int launch_round_begin(const PlanDev& p, int parity, cudaStream_t st);
+int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st);
 int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
                        cudaStream_t st);
 int launch_eval_finish_scaled(const CaseDev& c, const PlanDev& p, const StepParams& sp, float g_scale, float* F_out,

@@ -141,7 +141,17 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     const float alpha = pp.alpha[k], gp = pp.gp[k];
 #pragma unroll
     for (int j = 0; j < NPL; ++j) { x[j] = j < npl ? pp.x[row + 32 * j] : 0.f; g[j] = j < npl ? pp.g[row + 32 * j] : 0.f; }
-    if (Ft <= F + sp.c1 * alpha * gp) {                      // Armijo: accept x+ = x + alpha p
+    bool accept = Ft <= F + sp.c1 * alpha * gp;              // Armijo
+    if (!accept && sp.eps_f > 0.f && Ft <= F + sp.eps_f * fabsf(F)) {
+      // approximate test (reading A5b): F within its noise allowance and slope condition
+      // phi'(alpha) <= (2 c1 - 1) phi'(0), with alpha phi'(alpha) = g+ . (x+ - x)
+      float gts = 0.f;
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) gts = fmaf(gt[j], xt[j] - x[j], gts);
+      gts = warp_sum(gts);
+      accept = gts <= (2.f * sp.c1 - 1.f) * alpha * gp;
+    }
+    if (accept) {                                            // accept x+ = x + alpha p
       float sy = 0.f, ss = 0.f, yy = 0.f;
       float sv[NPL], yv[NPL];
 #pragma unroll
@@ -283,10 +293,13 @@ int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp,
 }
 
 // zero the "next round" counter; runs before the contraction kernels of a round
-__global__ void k_round_begin(int* n_running, int parity) { n_running[parity ^ 1] = 0; }
+__global__ void k_round_begin(int* n_running, int parity, int* log_slot) {
+  n_running[parity ^ 1] = 0;
+  if (log_slot) *log_slot = n_running[parity];
+}
 
-int launch_round_begin(const PlanDev& p, int parity, cudaStream_t st) {
-  k_round_begin<<<1, 1, 0, st>>>(p.n_running, parity);
+int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st) {
+  k_round_begin<<<1, 1, 0, st>>>(p.n_running, parity, round < kRoundLogCap ? p.round_log + round : nullptr);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

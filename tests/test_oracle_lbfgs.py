@@ -18,13 +18,46 @@ def test_convex_quadratic_reaches_closed_form_minimiser():
     """1/2 x'Ax - b'x, SPD: minimiser A^-1 b (numpy.linalg.solve), F monotone."""
     A, b = _spd(10, 0)
     fg = lambda x: (0.5 * x @ A @ x - b @ x, A @ x - b)
-    r = oracle.lbfgs(fg, np.zeros(10), m=10, iters=150)
     xs = np.linalg.solve(A, b)
-    # a function-value line search stalls at |x - x*| ~ sqrt(machine eps): status 2 is expected
+    # Armijo only (eps_f = 0): F is monotone; a function-value line search stalls at
+    # |x - x*| ~ sqrt(machine eps), so status 2 is expected
+    r = oracle.lbfgs(fg, np.zeros(10), m=10, iters=150, eps_f=0.0)
     assert r["x"] == pytest.approx(xs, rel=1e-6, abs=1e-7)
     assert r["F"] == pytest.approx(-0.5 * b @ xs, rel=1e-12)
     assert (np.diff(r["F_hist"]) <= 0).all()
-    assert r["n_skipped"] == 0 and r["status"] in (0, 2)
+    assert r["n_skipped"] == 0 and r["status"] in (0, 2) and r["n_approx"] == 0
+    # default (reading A5b): the approximate test may pass steps that Armijo cannot resolve;
+    # F never rises by more than eps_f |F| per step and the minimiser is reached all the same
+    r = oracle.lbfgs(fg, np.zeros(10), m=10, iters=150)
+    assert r["x"] == pytest.approx(xs, rel=1e-6, abs=1e-7)
+    assert r["F"] == pytest.approx(-0.5 * b @ xs, rel=1e-12)
+    h = r["F_hist"]
+    assert (np.diff(h) <= oracle.EPS_F * np.abs(h[:-1])).all()
+
+
+def test_approximate_test_equals_armijo_on_a_quadratic_line():
+    """For quadratic phi, phi'(a) <= (2 c1 - 1) phi'(0)  <=>  phi(a) <= phi(0) + c1 a phi'(0):
+    with a noise-free objective the two tests take the same decisions, so the iterates agree."""
+    A, b = _spd(8, 3, cond=30.0)
+    fg = lambda x: (0.5 * x @ A @ x - b @ x, A @ x - b)
+    r0 = oracle.lbfgs(fg, np.ones(8), m=5, iters=12, eps_f=0.0)
+    r1 = oracle.lbfgs(fg, np.ones(8), m=5, iters=12, eps_f=1e-6)
+    assert r1["n_approx"] == 0 and (r0["x"] == r1["x"]).all() and r0["n_evals"] == r1["n_evals"]
+
+
+def test_approximate_test_accepts_a_step_hidden_by_objective_noise():
+    """F quantised to 7 significant digits (an fp32-like objective), exact gradient: near the
+    minimum Armijo cannot see the decrease and burns step halvings on every iteration; the
+    approximate test accepts those steps at once and ends closer to the minimiser."""
+    A, b = _spd(6, 5, cond=20.0)
+    xs = np.linalg.solve(A, b)
+    def fg(x):
+        F = 10.0 + 0.5 * (x - xs) @ A @ (x - xs)
+        return float(np.float32(F)), A @ (x - xs)
+    r0 = oracle.lbfgs(fg, xs + 1.0, m=6, iters=60, eps_f=0.0)
+    r1 = oracle.lbfgs(fg, xs + 1.0, m=6, iters=60, eps_f=1e-6)
+    assert r1["n_approx"] > 0 and r1["n_backtracks"] < 5 and r0["n_backtracks"] > 100
+    assert np.linalg.norm(r1["x"] - xs) < 0.1 * np.linalg.norm(r0["x"] - xs)
 
 
 def test_first_step_is_normalised_steepest_descent():
