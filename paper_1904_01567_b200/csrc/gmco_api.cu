@@ -112,10 +112,9 @@ void carve_case(gmco_handle* h, bool want_split, bool need_stage) {
   c.D = a.take<float>(nd);
   if (want_split) {
     c.D_hi = a.take<float>(nd); c.D_lo = a.take<float>(nd);
-    c.DT_hi = a.take<float>(nd); c.DT_lo = a.take<float>(nd);
   }
   c.pt_lo = a.take<float>(c.N_alloc); c.pt_hi = a.take<float>(c.N_alloc);
-  c.tile_struct = a.take<int>(c.N_alloc / 64);
+  c.tile_struct = a.take<int>(c.N_alloc / 64); c.tile_valid = a.take<int>(c.N_alloc / 64);
   c.row_src = a.take<int>(c.N_alloc); c.sel_pos = a.take<int>(c.N_alloc);
   h->struct_scale = a.take<float>(2 * GMCO_MAX_STRUCTS);
   h->dvh_thr = a.take<float>(GMCO_MAX_STRUCTS);
@@ -157,6 +156,7 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
     g_elems = nseg * kPlanTile * c.A_pad;
     if (nseg * kPlanTile > f_elems) f_elems = nseg * kPlanTile;
     p.R = nullptr; p.nG = 0;
+    p.R_hi = a.take<float>(kp * c.N_alloc); p.R_lo = a.take<float>(kp * c.N_alloc);
   }
   p.Fpart = a.take<float>(f_elems); p.Gpart = a.take<float>(g_elems);
   p.res_terms = a.take<float>(kp * 2 * c.S); p.res_cnt = a.take<int>(kp * c.S);
@@ -180,7 +180,7 @@ int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   carve_plans(h, K, 0);
   h->plan_capacity_K = K;
   if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
-    h->tc = tc_plan_create(h->c, h->p, h->num_sms, h->err, sizeof(h->err));
+    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->err, sizeof(h->err));
     if (!h->tc) return GMCO_E_UNSUPPORTED;
   }
   return GMCO_OK;
@@ -360,7 +360,8 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
 
   std::vector<float> pt_lo(c.N_alloc, -INFINITY), pt_hi(c.N_alloc, INFINITY), scale(2 * GMCO_MAX_STRUCTS, 0.f),
       thr(GMCO_MAX_STRUCTS, -1.f);
-  std::vector<int> tile_struct(c.N_alloc / 64, 0), row_src(c.N_alloc, -1), sel_pos(c.N_alloc, -1);
+  std::vector<int> tile_struct(c.N_alloc / 64, 0), tile_valid(c.N_alloc / 64, 0), row_src(c.N_alloc, -1),
+      sel_pos(c.N_alloc, -1);
   src = 0;
   for (int s = 0; s < n_structs; ++s) {
     const StructHost& q = h->sh[s];
@@ -369,7 +370,11 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
       row_src[q.row_begin + i] = src + i;
       if (q.dvh_kind == 2) sel_pos[q.row_begin + i] = q.sel_begin + i;
     }
-    for (int t = q.row_begin / 64; t < (q.row_begin + q.n_rows_pad) / 64; ++t) tile_struct[t] = s;
+    for (int t = q.row_begin / 64; t < (q.row_begin + q.n_rows_pad) / 64; ++t) {
+      tile_struct[t] = s;
+      const int left = q.n_points - (t * 64 - q.row_begin);
+      tile_valid[t] = left >= 64 ? 64 : left;
+    }
     scale[2 * s] = q.w_lo / (float)q.n_points; scale[2 * s + 1] = q.w_hi / (float)q.n_points;
     if (q.dvh_kind == 1) thr[s] = q.dvh_level / 100.f * rx_dose;
     src += q.n_points;
@@ -378,6 +383,7 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   CKC(cudaMemcpyAsync(c.pt_lo, pt_lo.data(), c.N_alloc * sizeof(float), cudaMemcpyHostToDevice, st));
   CKC(cudaMemcpyAsync(c.pt_hi, pt_hi.data(), c.N_alloc * sizeof(float), cudaMemcpyHostToDevice, st));
   CKC(cudaMemcpyAsync(c.tile_struct, tile_struct.data(), tile_struct.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+  CKC(cudaMemcpyAsync(c.tile_valid, tile_valid.data(), tile_valid.size() * sizeof(int), cudaMemcpyHostToDevice, st));
   CKC(cudaMemcpyAsync(c.row_src, row_src.data(), c.N_alloc * sizeof(int), cudaMemcpyHostToDevice, st));
   CKC(cudaMemcpyAsync(c.sel_pos, sel_pos.data(), c.N_alloc * sizeof(int), cudaMemcpyHostToDevice, st));
   CKC(cudaMemcpyAsync(h->struct_scale, scale.data(), scale.size() * sizeof(float), cudaMemcpyHostToDevice, st));

@@ -29,13 +29,12 @@ struct CaseDev {
   int A_pad = 0;                    // A rounded up to 32
   float rx = 0.f;
   float* D = nullptr;               // [N_alloc][A_pad] fp32, padded rows/cols are 0
-  float* D_hi = nullptr;            // [N_alloc][A_pad] tf32 hi part   (tensor path, dose MMA B operand)
+  float* D_hi = nullptr;            // [N_alloc][A_pad] tf32 hi part   (tensor path: B operand of both contractions)
   float* D_lo = nullptr;            // [N_alloc][A_pad] tf32 lo part
-  float* DT_hi = nullptr;           // [A_pad][N_alloc] transposed hi  (tensor path, gradient MMA B operand)
-  float* DT_lo = nullptr;           // [A_pad][N_alloc] transposed lo
   float* pt_lo = nullptr;           // [N_alloc] D_min of the point's structure (-inf on padding rows)
   float* pt_hi = nullptr;           // [N_alloc] D_max (+inf on padding rows)
   int* tile_struct = nullptr;       // [N_alloc / 64] structure id of each 64-row tile (uniform by construction)
+  int* tile_valid = nullptr;        // [N_alloc / 64] leading rows of the tile that are real points (rest is padding)
   int* row_src = nullptr;           // [N_alloc] original row index, -1 on padding rows
   int* sel_pos = nullptr;           // [N_alloc] position inside the D_level selection buffer, -1 if unused
   int n_sel = 0;                    // total points of dvh_kind == 2 structures
@@ -61,7 +60,8 @@ struct PlanDev {
   int *round_log = nullptr;                                        // [kRoundLogCap] running plans at the start of round r
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
   // partial results of one evaluation round
-  float *Fpart = nullptr; float *Gpart = nullptr; float *R = nullptr;
+  float *Fpart = nullptr; float *Gpart = nullptr; float *R = nullptr;   // R [K_pad][N_alloc]: SIMT route
+  float *R_hi = nullptr, *R_lo = nullptr;                            // [N_alloc][K_pad] tf32 parts of dF/dd / 2: tensor route
   int nF = 0, nFcomp = 1, nG = 0;                                  // SIMT: slot counts (uniform over plans)
   // result staging
   float *res_terms = nullptr;                                      // [K_pad][2*S]
@@ -99,8 +99,8 @@ int launch_result(const CaseDev& c, const PlanDev& p, const StructHost* sh, floa
 int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st);
 
 // tensor path (kernel_fused_tc.cu)
-struct TcPlan;                                   // host-side stream-K schedule + tensor maps
-TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, int num_sms, char* err, int errlen);
+struct TcPlan;                                   // host-side schedule + tensor maps
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 const int* tc_tile_seg_dev(const TcPlan*);

@@ -32,34 +32,12 @@ __global__ void k_pad_D(const float* __restrict__ Du, long long ldD, int A, cons
   }
 }
 
-// [R][C] -> [C][R] for the hi/lo parts (gradient MMA wants points contiguous).
-__global__ void k_transpose2(const float* __restrict__ in0, const float* __restrict__ in1, float* __restrict__ out0,
-                             float* __restrict__ out1, int R, int C) {
-  __shared__ float t0[32][33], t1[32][33];
-  const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
-  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-    const int r = r0 + j, c = c0 + threadIdx.x;
-    if (r < R && c < C) { t0[j][threadIdx.x] = in0[(long long)r * C + c]; t1[j][threadIdx.x] = in1[(long long)r * C + c]; }
-  }
-  __syncthreads();
-  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-    const int c = c0 + j, r = r0 + threadIdx.x;
-    if (r < R && c < C) { out0[(long long)c * R + r] = t0[threadIdx.x][j]; out1[(long long)c * R + r] = t1[threadIdx.x][j]; }
-  }
-}
-
 int launch_setup_case(const CaseDev& c, const float* D_user, long long ldD, const int* row_src_dev,
                       bool want_split, cudaStream_t st) {
   const long long tot = (long long)c.N_alloc * c.A_pad;
   k_pad_D<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(D_user, ldD, c.A, row_src_dev, c.N_alloc, c.A_pad, c.D,
                                                           want_split ? c.D_hi : nullptr, want_split ? c.D_lo : nullptr);
-  int n = 1;
-  if (want_split) {
-    dim3 grid((c.A_pad + 31) / 32, (c.N_alloc + 31) / 32), block(32, 8);
-    k_transpose2<<<grid, block, 0, st>>>(c.D_hi, c.D_lo, c.DT_hi, c.DT_lo, c.N_alloc, c.A_pad);
-    n++;
-  }
-  return cudaGetLastError() == cudaSuccess ? n : -1;
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -1,0 +1,561 @@
+// kernels_tc.cu -- the tensor-core contractions of one evaluation round, sm_100a only.
+//
+//   k_dose_tc : d = D t (Eq. 1) on tcgen05 with a 3xTF32 split, penalty and
+//               derivative (Eq. 2) and the per-plan objective partial sums
+//               (Eq. 4) fused into the epilogue.  Dose never reaches HBM; the
+//               epilogue emits r = dF/dd / 2 as two tf32 parts for the second contraction.
+//   k_grad_tc : G = D^T r (Eq. 3 summed over points) on tcgen05, 3xTF32,
+//               split over points with per-segment partial sums (fixed order, no float atomics).
+//
+// Tile orientation (both kernels): the 128 TMEM lanes hold 128 PLANS (MMA M = 128).
+//   dose : acc[128 plans x 64 points]  = T[128 x A] (A operand) . D_chunk[64 x A]^T (B, K-major)
+//          T_hi lives in TMEM for the whole kernel (A-from-TMEM MMAs), T_lo in shared memory;
+//          D streams through a TMA ring in slabs of 32 dwell positions (hi and lo part).
+//   grad : acc[128 plans x A]  +=  R[32 points x 128 plans]^T (A, MN-major) . D[32 points x A] (B, MN-major)
+//          R and D stream through a TMA ring in slabs of 32 (or 16) points.
+// 3xTF32: x = hi + lo with hi, lo representable in tf32; x.y ~ hi.hi + hi.lo + lo.hi accumulated
+// in fp32 by the tensor core (the dropped lo.lo term is ~2^-22 relative).
+//
+// Roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM allocator + MMA issuer (one lane),
+// warps 2-5 = epilogue (TMEM lane quadrant = warp_id % 4).  Pipelines are mbarrier rings.
+#include <cudaTypedefs.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "gmco_internal.cuh"
+
+namespace gmco {
+
+namespace {
+
+constexpr int kPC = 64;                 // points per dose chunk (= MMA N of the dose contraction)
+constexpr int kSlabBytes = kPC * 128;   // one 32-dwell slab of a dose chunk, one part: 8 KB
+constexpr int kTloBox = 128 * 128;      // T_lo: 128 plans x 32 dwell: 16 KB
+constexpr int kThreads = 192;
+constexpr uint32_t kWatchdog = 1u << 26;
+
+// ---------------------------------------------------------------------------------------------
+// PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+// Bounded wait: a protocol bug traps (launch failure reported by the API) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++spins > kWatchdog) __trap();
+  }
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_3d(const CUtensorMap* map, void* dst, uint64_t* bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
+}
+
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t* dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// all previously issued MMAs of this thread arrive on `bar` when they complete
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// D[tmem] (+)= A[smem] . B[smem]
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// D[tmem] (+)= A[tmem] . B[smem]
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc)
+      : "memory");
+}
+
+#define GMCO_R32(v, o)                                                                                           \
+  "=r"(v[o + 0]), "=r"(v[o + 1]), "=r"(v[o + 2]), "=r"(v[o + 3]), "=r"(v[o + 4]), "=r"(v[o + 5]), "=r"(v[o + 6]), \
+      "=r"(v[o + 7]), "=r"(v[o + 8]), "=r"(v[o + 9]), "=r"(v[o + 10]), "=r"(v[o + 11]), "=r"(v[o + 12]),          \
+      "=r"(v[o + 13]), "=r"(v[o + 14]), "=r"(v[o + 15])
+#define GMCO_W32(v, o)                                                                                   \
+  "r"(v[o + 0]), "r"(v[o + 1]), "r"(v[o + 2]), "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), \
+      "r"(v[o + 7]), "r"(v[o + 8]), "r"(v[o + 9]), "r"(v[o + 10]), "r"(v[o + 11]), "r"(v[o + 12]),          \
+      "r"(v[o + 13]), "r"(v[o + 14]), "r"(v[o + 15])
+
+// 32 lanes x 32 consecutive columns: thread i of the warp gets lane (base lane + i), register j = column j
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : GMCO_R32(v, 0), GMCO_R32(v, 16)
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x32.b32 [%32], "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31};"
+      ::GMCO_W32(v, 0), GMCO_W32(v, 16), "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor, version 1 (sm_100).  Addresses and offsets in 16 B units.
+//   kSwz128 : K-major operand, rows of 128 B = 32 fp32 along K, 16 B chunks XOR-swizzled over 8 rows
+//             (TMA SWIZZLE_128B).  SBO = bytes between 8-row groups (1024), LBO unused (1).
+//   kSwz128Base32 : MN-major tf32 operand (the only MN-major layout tf32 has): rows of 128 B = 32 fp32
+//             along M/N, one row per K index, 32 B chunks XOR-swizzled over 4 rows (TMA
+//             SWIZZLE_128B_ATOM_32B).  LBO = bytes between 32-element groups along M/N,
+//             SBO = bytes between 4-row groups along K (512).
+constexpr uint32_t kSwz128 = 2, kSwz128Base32 = 1;
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3fff);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32;
+  d |= (uint64_t)1 << 46;   // descriptor version
+  d |= (uint64_t)layout << 61;
+  return d;
+}
+// Instruction descriptor, kind::tf32, fp32 accumulator, M = 128.
+__host__ __device__ constexpr uint32_t instr_desc(int n, int a_mn_major, int b_mn_major) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)a_mn_major << 15) | ((uint32_t)b_mn_major << 16) |
+         ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+
+struct Thresholds { float d_lo[GMCO_MAX_STRUCTS], d_hi[GMCO_MAX_STRUCTS]; };
+
+struct DoseArgs {
+  const float* T_hi;          // [K_pad][A_pad]
+  float *R_hi, *R_lo;         // [N_alloc][K_pad]
+  float* Fpart;               // [n_tiles * segs][128]
+  const float* Weff;          // [K_pad][2S]
+  const int* tile_struct;     // [N_alloc / 64]
+  const int* tile_valid;      // [N_alloc / 64]
+  const int* row_src;         // [N_alloc]
+  float* dose_dbg;            // [N][K] or null
+  const int* gate;
+  int A_pad, K_pad, K, S, n_chunks, segs, n_stage;
+  Thresholds thr;
+};
+
+struct GradArgs {
+  float* Gpart;               // [n_tiles * segs][128][A_pad]
+  const int* gate;
+  int A_pad, n_slabs, segs, n_stage;
+};
+
+// ---------------------------------------------------------------------------------------------
+// a2-a4 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
+// point chunks [seg n_chunks / segs, (seg + 1) n_chunks / segs).
+__global__ void __launch_bounds__(kThreads, 1)
+k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
+          const __grid_constant__ CUtensorMap tmT_lo, const DoseArgs a) {
+  if (a.gate && *a.gate == 0) return;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int G = a.A_pad >> 5;                       // 32-dwell slabs
+  uint8_t* tlo = smem;                              // [G][128 plans][128 B]
+  uint8_t* ring = smem + (size_t)G * kTloBox;       // [n_stage][hi 8 KB | lo 8 KB]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + (size_t)a.n_stage * 2 * kSlabBytes);
+  uint64_t* full = bars;                            // [n_stage]
+  uint64_t* empty = bars + a.n_stage;               // [n_stage]
+  uint64_t* tlo_full = bars + 2 * a.n_stage;
+  uint64_t* thi_ready = tlo_full + 1;
+  uint64_t* acc_full = thi_ready + 1;               // [2]
+  uint64_t* acc_empty = acc_full + 2;               // [2]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int seg = blockIdx.x, tile = blockIdx.y;
+  const int c0 = (int)((long long)seg * a.n_chunks / a.segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / a.segs);
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    mbar_init(tlo_full, 1);
+    mbar_init(thi_ready, 128);
+    for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 128); }
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT_lo); }
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t t_thi = tmem;                      // columns [0, A_pad): T_hi
+  const uint32_t t_acc = tmem + a.A_pad;            // columns [A_pad, A_pad + 128): two dose accumulators
+
+  if (warp == 0) {
+    if (lane == 0 && c1 > c0) {
+      mbar_expect_tx(tlo_full, (uint32_t)G * kTloBox);
+      for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g);
+      int st = 0; uint32_t ph = 0;
+      for (int c = c0; c < c1; ++c) {
+        for (int g = 0; g < G; ++g) {
+          mbar_wait(empty + st, ph ^ 1);
+          uint8_t* dst = ring + (size_t)st * 2 * kSlabBytes;
+          mbar_expect_tx(full + st, 2 * kSlabBytes);
+          tma_load_3d(&tmD_hi, dst, full + st, 0, c * kPC, g);
+          tma_load_3d(&tmD_lo, dst + kSlabBytes, full + st, 0, c * kPC, g);
+          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && c1 > c0) {
+      constexpr uint32_t idesc = instr_desc(kPC, 0, 0);
+      mbar_wait(tlo_full, 0);
+      mbar_wait(thi_ready, 0);
+      tc_fence_after();
+      int st = 0; uint32_t ph = 0;
+      for (int c = c0; c < c1; ++c) {
+        const int b = (c - c0) & 1, use = (c - c0) >> 1;
+        mbar_wait(acc_empty + b, (use & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t acc = t_acc + b * kPC;
+        for (int g = 0; g < G; ++g) {
+          mbar_wait(full + st, ph);
+          tc_fence_after();
+          const uint32_t s_hi = smem_u32(ring + (size_t)st * 2 * kSlabBytes);
+          const uint64_t d_hi = smem_desc(s_hi, 16, 1024, kSwz128), d_lo = smem_desc(s_hi + kSlabBytes, 16, 1024, kSwz128);
+          const uint64_t a_lo = smem_desc(smem_u32(tlo + (size_t)g * kTloBox), 16, 1024, kSwz128);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {             // 4 K-steps of 8 dwell positions: +32 B inside the swizzled row
+            const uint32_t a_hi = t_thi + g * 32 + j * 8;
+            mma_ts(acc, a_hi, d_hi + 2 * j, idesc, (g | j) != 0);
+            mma_ts(acc, a_hi, d_lo + 2 * j, idesc, 1);
+            mma_ss(acc, a_lo + 2 * j, d_hi + 2 * j, idesc, 1);
+          }
+          tc_commit(empty + st);
+          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        }
+        tc_commit(acc_full + b);
+      }
+    }
+  } else {
+    const int q = warp & 3;                         // TMEM lane quadrant this warp may access
+    const int L = q * 32 + lane;                    // lane = plan inside the tile
+    const int plan = tile * 128 + L;
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    float f = 0.f;
+    if (c1 > c0) {
+      // T_hi row of this plan -> TMEM columns [0, A_pad)
+      const float4* src = reinterpret_cast<const float4*>(a.T_hi + (size_t)plan * a.A_pad);
+      for (int g = 0; g < G; ++g) {
+        uint32_t v[32];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float4 t = src[g * 8 + i];
+          v[4 * i + 0] = __float_as_uint(t.x); v[4 * i + 1] = __float_as_uint(t.y);
+          v[4 * i + 2] = __float_as_uint(t.z); v[4 * i + 3] = __float_as_uint(t.w);
+        }
+        tmem_st32(t_thi + lane_base + g * 32, v);
+      }
+      tmem_st_wait();
+      tc_fence_before();
+      mbar_arrive(thi_ready);
+
+      for (int c = c0; c < c1; ++c) {
+        const int b = (c - c0) & 1, use = (c - c0) >> 1;
+        const int s = a.tile_struct[c], nv = a.tile_valid[c];
+        const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
+        const float wlo = a.Weff[(size_t)plan * 2 * a.S + 2 * s], whi = a.Weff[(size_t)plan * 2 * a.S + 2 * s + 1];
+        mbar_wait(acc_full + b, use & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int h = 0; h < kPC / 32; ++h) {
+          uint32_t v[32];
+          tmem_ld32(t_acc + lane_base + b * kPC + h * 32, v);
+          tmem_ld_wait();
+          if (h == kPC / 32 - 1) { tc_fence_before(); mbar_arrive(acc_empty + b); }
+          const size_t p0 = (size_t)c * kPC + h * 32;
+          float* rh = a.R_hi + p0 * a.K_pad + plan;
+          float* rl = a.R_lo + p0 * a.K_pad + plan;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float d = __uint_as_float(v[j]);
+            const float lo = fminf(d - dlo, 0.f), hi = fmaxf(d - dhi, 0.f);
+            const float u = wlo * lo, w = whi * hi;
+            if (h * 32 + j < nv) f = fmaf(u, lo, fmaf(w, hi, f));
+            const float r = u + w;                                        // = dF/dd / 2
+            const float r_hi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);   // exact tf32 (truncated)
+            rh[(size_t)j * a.K_pad] = r_hi;
+            rl[(size_t)j * a.K_pad] = r - r_hi;
+          }
+          if (a.dose_dbg && plan < a.K) {
+            for (int j = 0; j < 32; ++j) {
+              if (h * 32 + j < nv) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[j]);
+            }
+          }
+        }
+      }
+    }
+    a.Fpart[((size_t)tile * a.segs + seg) * 128 + L] = f;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
+// point slabs [seg n_slabs / segs, (seg + 1) n_slabs / segs) of PS points each.
+template <int PS>
+__global__ void __launch_bounds__(kThreads, 1)
+k_grad_tc(const __grid_constant__ CUtensorMap tmR_hi, const __grid_constant__ CUtensorMap tmR_lo,
+          const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
+  if (a.gate && *a.gate == 0) return;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int G = a.A_pad >> 5;
+  constexpr int kRBytes = 4 * PS * 128;             // R part: 4 plan groups x PS points x 128 B
+  const int dBytes = G * PS * 128;                  // D part: G dwell groups x PS points x 128 B
+  const int stageBytes = 2 * kRBytes + 2 * dBytes;  // [R_hi | R_lo | D_hi | D_lo]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)a.n_stage * stageBytes);
+  uint64_t* full = bars;
+  uint64_t* empty = bars + a.n_stage;
+  uint64_t* acc_full = bars + 2 * a.n_stage;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int seg = blockIdx.x, tile = blockIdx.y;
+  const int s0 = (int)((long long)seg * a.n_slabs / a.segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / a.segs);
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    mbar_init(acc_full, 1);
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmR_hi); tma_prefetch_desc(&tmR_lo); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo);
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        mbar_wait(empty + st, ph ^ 1);
+        uint8_t* dst = smem + (size_t)st * stageBytes;
+        mbar_expect_tx(full + st, (uint32_t)stageBytes);
+        tma_load_3d(&tmR_hi, dst, full + st, 0, s * PS, tile * 4);
+        tma_load_3d(&tmR_lo, dst + kRBytes, full + st, 0, s * PS, tile * 4);
+        tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0);
+        tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0);
+        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && s1 > s0) {
+      // the accumulator is A_pad columns wide; one MMA covers at most 256 of them
+      const int n0 = a.A_pad <= 256 ? a.A_pad : 256, n1 = a.A_pad - n0;
+      const uint32_t idesc0 = instr_desc(n0, 1, 1), idesc1 = instr_desc(n1 > 0 ? n1 : 16, 1, 1);
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        mbar_wait(full + st, ph);
+        tc_fence_after();
+        const uint32_t base = smem_u32(smem + (size_t)st * stageBytes);
+#pragma unroll
+        for (int j = 0; j < PS / 8; ++j) {          // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
+          const uint64_t r_hi = smem_desc(base + j * 1024, PS * 128, 512, kSwz128Base32);
+          const uint64_t r_lo = smem_desc(base + kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+          const uint64_t d_hi = smem_desc(base + 2 * kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+          const uint64_t d_lo = smem_desc(base + 2 * kRBytes + dBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+          const uint32_t acc = (s > s0 || j > 0) ? 1u : 0u;
+          mma_ss(tmem, r_hi, d_hi, idesc0, acc);
+          mma_ss(tmem, r_hi, d_lo, idesc0, 1);
+          mma_ss(tmem, r_lo, d_hi, idesc0, 1);
+          if (n1 > 0) {                              // dwell groups 8.. : +8 groups of PS x 128 B
+            const uint64_t off = (uint64_t)((8 * PS * 128) >> 4);
+            mma_ss(tmem + 256, r_hi, d_hi + off, idesc1, acc);
+            mma_ss(tmem + 256, r_hi, d_lo + off, idesc1, 1);
+            mma_ss(tmem + 256, r_lo, d_hi + off, idesc1, 1);
+          }
+        }
+        tc_commit(empty + st);
+        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+      }
+      tc_commit(acc_full);
+    }
+  } else {
+    const int q = warp & 3;
+    const int L = q * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    float4* dst = reinterpret_cast<float4*>(a.Gpart + (((size_t)tile * a.segs + seg) * 128 + L) * a.A_pad);
+    if (s1 > s0) {
+      mbar_wait(acc_full, 0);
+      tc_fence_after();
+      for (int g = 0; g < G; ++g) {
+        uint32_t v[32];
+        tmem_ld32(tmem + lane_base + g * 32, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          dst[g * 8 + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                       __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+      }
+    } else {
+      for (int i = 0; i < a.A_pad / 4; ++i) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+PFN_cuTensorMapEncodeTiled get_encode() {
+  static PFN_cuTensorMapEncodeTiled fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(p);
+  }
+  return fn;
+}
+
+// fp32 matrix [rows][cols] (cols contiguous, cols % 32 == 0) viewed as {32, rows, cols / 32};
+// box = {32, box_rows, box_groups}: lands in smem as [group][row][128 B] with the given swizzle.
+bool make_map(CUtensorMap* m, const float* base, long long rows, long long cols, int box_rows, int box_groups,
+              CUtensorMapSwizzle swz) {
+  PFN_cuTensorMapEncodeTiled enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {32, (cuuint64_t)rows, (cuuint64_t)(cols / 32)};
+  cuuint64_t strides[2] = {(cuuint64_t)cols * 4, 128};
+  cuuint32_t box[3] = {32, (cuuint32_t)box_rows, (cuuint32_t)box_groups};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+struct TcPlan {
+  CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo;
+  CUtensorMap grad_R_hi, grad_R_lo, grad_D_hi, grad_D_lo;
+  int segs = 1, n_tiles = 0;
+  int dose_stages = 0, dose_smem = 0;
+  int grad_ps = 32, grad_stages = 0, grad_smem = 0;
+  int* tile_seg_dev = nullptr;
+  Thresholds thr{};
+};
+
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, char* err, int errlen) {
+  constexpr int kSmemMax = 227 * 1024;
+  if (c.A_pad > 384) { snprintf(err, errlen, "tensor path supports n_dwell <= 384 (use GMCO_PREC_SIMT_FP32)"); return nullptr; }
+  TcPlan* t = new TcPlan();
+  t->n_tiles = p.K_pad / kPlanTile;
+  t->segs = num_sms / t->n_tiles > 0 ? num_sms / t->n_tiles : 1;
+  for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
+  const int G = c.A_pad / 32;
+  // dose kernel: T_lo resident + as many ring stages as fit
+  const int fixed = G * kTloBox + 1024 /*alignment slack*/ + 512 /*barriers*/;
+  t->dose_stages = (kSmemMax - fixed) / (2 * kSlabBytes);
+  if (t->dose_stages > 8) t->dose_stages = 8;
+  if (t->dose_stages < 2) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
+  t->dose_smem = fixed + t->dose_stages * 2 * kSlabBytes;
+  // gradient kernel
+  t->grad_ps = c.A_pad <= 256 ? 32 : 16;
+  const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
+  t->grad_stages = (kSmemMax - 1024 - 512) / stage;
+  if (t->grad_stages > 6) t->grad_stages = 6;
+  if (t->grad_stages < 2) { snprintf(err, errlen, "shared memory too small for the gradient ring"); delete t; return nullptr; }
+  t->grad_smem = 1024 + 512 + t->grad_stages * stage;
+  const CUtensorMapSwizzle sK = CU_TENSOR_MAP_SWIZZLE_128B, sMN = CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
+  bool ok = make_map(&t->dose_D_hi, c.D_hi, c.N_alloc, c.A_pad, kPC, 1, sK) &&
+            make_map(&t->dose_D_lo, c.D_lo, c.N_alloc, c.A_pad, kPC, 1, sK) &&
+            make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK) &&
+            make_map(&t->grad_R_hi, p.R_hi, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
+            make_map(&t->grad_R_lo, p.R_lo, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
+            make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
+            make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
+  if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
+  cudaError_t e = cudaFuncSetAttribute(k_dose_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+  std::vector<int> seg(t->n_tiles + 1);
+  for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
+  if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&t->tile_seg_dev), seg.size() * sizeof(int));
+  if (e == cudaSuccess) e = cudaMemcpy(t->tile_seg_dev, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { snprintf(err, errlen, "tensor plan setup: %s", cudaGetErrorString(e)); tc_plan_destroy(t); return nullptr; }
+  return t;
+}
+
+void tc_plan_destroy(TcPlan* t) {
+  if (!t) return;
+  if (t->tile_seg_dev) cudaFree(t->tile_seg_dev);
+  delete t;
+}
+
+int tc_num_segments(const TcPlan* t) { return t->n_tiles * t->segs; }
+const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
+
+int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
+                   cudaStream_t st) {
+  dim3 grid(t->segs, t->n_tiles);
+  DoseArgs da{};
+  da.T_hi = p.T_hi; da.R_hi = p.R_hi; da.R_lo = p.R_lo; da.Fpart = p.Fpart; da.Weff = p.Weff;
+  da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
+  da.gate = gate; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = c.N_pad / kPC;
+  da.segs = t->segs; da.n_stage = t->dose_stages; da.thr = t->thr;
+  k_dose_tc<<<grid, kThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
+  if (cudaGetLastError() != cudaSuccess) return -1;
+  GradArgs ga{};
+  ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
+  ga.n_stage = t->grad_stages;
+  if (t->grad_ps == 32)
+    k_grad_tc<32><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R_hi, t->grad_R_lo, t->grad_D_hi, t->grad_D_lo, ga);
+  else
+    k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R_hi, t->grad_R_lo, t->grad_D_hi, t->grad_D_lo, ga);
+  return cudaGetLastError() == cudaSuccess ? 2 : -1;
+}
+
+}  // namespace gmco
