@@ -55,7 +55,8 @@ typedef enum gmco_status {
 
 /* Precision / pipe of the two contractions D t and D^T r. */
 typedef enum gmco_precision {
-  GMCO_PREC_TF32X3 = 0,     /* tcgen05 kind::tf32, 3-product split (fp32-equivalent), fused kernel */
+  GMCO_PREC_TF32X3 = 0,     /* tcgen05 kind::tf32, 3-product split (fp32-equivalent); cases with more than
+                               384 dwell positions do not fit the tensor layout and run as SIMT_FP32  */
   GMCO_PREC_SIMT_FP32 = 1   /* plain fp32 FMA kernels (reference datum and debug route)            */
 } gmco_precision;
 

@@ -154,9 +154,9 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
     // upper bound on stream-K segments: one per CTA plus one per plan tile
     const size_t nseg = (size_t)h->num_sms + p.K_pad / kPlanTile + 1;
     g_elems = nseg * kPlanTile * c.A_pad;
-    if (nseg * kPlanTile > f_elems) f_elems = nseg * kPlanTile;
-    p.R = nullptr; p.nG = 0;
-    p.R_hi = a.take<float>(kp * c.N_alloc); p.R_lo = a.take<float>(kp * c.N_alloc);
+    if (nseg * kPlanTile * 2 > f_elems) f_elems = nseg * kPlanTile * 2;
+    p.nG = 0;
+    p.R = a.take<float>(kp * c.N_alloc);             // [N_alloc][K_pad] on this route
   }
   p.Fpart = a.take<float>(f_elems); p.Gpart = a.take<float>(g_elems);
   p.res_terms = a.take<float>(kp * 2 * c.S); p.res_cnt = a.take<int>(kp * c.S);
@@ -197,7 +197,7 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
     sp.nG = p.nG; sp.g_slot_stride = (long long)p.K_pad * c.A_pad;
     sp.tile_local = 0; sp.tile_seg = nullptr;
   } else {
-    sp.nF = 0; sp.nFcomp = 1; sp.f_slot_stride = kPlanTile;
+    sp.nF = 0; sp.nFcomp = 2; sp.f_slot_stride = 2 * kPlanTile;
     sp.nG = 0; sp.g_slot_stride = (long long)kPlanTile * c.A_pad;
     sp.tile_local = 1; sp.tile_seg = tc_tile_seg_dev(h->tc);
   }
@@ -293,6 +293,9 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
       (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || o.reserved[0] || o.reserved[1])
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
+  // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
+  // the plain-fp32 kernels (the paper's largest N_act is 385)
+  if (o.precision == GMCO_PREC_TF32X3 && round_up(n_dwell, 32) > kMaxApadTensor) o.precision = GMCO_PREC_SIMT_FP32;
   long long tot = 0;
   for (int s = 0; s < n_structs; ++s) {
     const gmco_structure& g = structs[s];

@@ -15,6 +15,7 @@ constexpr int kStructAlign = 64;  // every structure is padded to a multiple of 
 constexpr int kRowAlloc = 256;    // D rows are allocated up to a multiple of this (tile over-reads stay in bounds)
 constexpr int kPlanTile = 128;    // plans per tensor tile = TMEM lanes
 constexpr int kMaxApad = 480;     // 512 TMEM columns - at least one 32-point chunk of dose accumulator
+constexpr int kMaxApadTensor = 384; // tensor route: T_hi (A_pad TMEM columns) + one 128-column accumulator pair
 constexpr int kMaxNpl = kMaxApad / 32;  // dwell elements per lane in the warp-per-plan kernels
 constexpr int kRoundLogCap = 8192;      // rounds whose running-plan count is logged (profiling aid)
 
@@ -60,8 +61,8 @@ struct PlanDev {
   int *round_log = nullptr;                                        // [kRoundLogCap] running plans at the start of round r
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
   // partial results of one evaluation round
-  float *Fpart = nullptr; float *Gpart = nullptr; float *R = nullptr;   // R [K_pad][N_alloc]: SIMT route
-  float *R_hi = nullptr, *R_lo = nullptr;                            // [N_alloc][K_pad] tf32 parts of dF/dd / 2: tensor route
+  float *Fpart = nullptr; float *Gpart = nullptr;
+  float *R = nullptr;               // SIMT route: dF/dd [K_pad][N_alloc]; tensor route: dF/dd / 2 [N_alloc][K_pad]
   int nF = 0, nFcomp = 1, nG = 0;                                  // SIMT: slot counts (uniform over plans)
   // result staging
   float *res_terms = nullptr;                                      // [K_pad][2*S]

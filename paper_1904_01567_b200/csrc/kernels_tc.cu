@@ -67,6 +67,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (++spins > kWatchdog) __trap();
   }
 }
+// one lane of a fully converged warp; the compiler keeps everything around it on the uniform datapath
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 __device__ __forceinline__ void tma_load_3d(const CUtensorMap* map, void* dst, uint64_t* bar, int c0, int c1, int c2) {
@@ -164,17 +170,20 @@ __host__ __device__ constexpr uint32_t instr_desc(int n, int a_mn_major, int b_m
 
 struct Thresholds { float d_lo[GMCO_MAX_STRUCTS], d_hi[GMCO_MAX_STRUCTS]; };
 
+constexpr int kDoseThreads = 320;       // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue (2 per TMEM lane quadrant)
+constexpr int kScratchBytes = 8 * 4096; // T_hi transposition scratch, one 32 x 128 B slab per epilogue warp
+
 struct DoseArgs {
   const float* T_hi;          // [K_pad][A_pad]
-  float *R_hi, *R_lo;         // [N_alloc][K_pad]
-  float* Fpart;               // [n_tiles * segs][128]
+  float* R;                   // [N_alloc][K_pad]  dF/dd / 2 (fp32; the gradient kernel splits it)
+  float* Fpart;               // [n_tiles * segs][128][2]
   const float* Weff;          // [K_pad][2S]
   const int* tile_struct;     // [N_alloc / 64]
   const int* tile_valid;      // [N_alloc / 64]
   const int* row_src;         // [N_alloc]
   float* dose_dbg;            // [N][K] or null
   const int* gate;
-  int A_pad, K_pad, K, S, n_chunks, segs, n_stage;
+  int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, tlo_resident;
   Thresholds thr;
 };
 
@@ -184,19 +193,27 @@ struct GradArgs {
   int A_pad, n_slabs, segs, n_stage;
 };
 
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------------
 // a2-a4 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point chunks [seg n_chunks / segs, (seg + 1) n_chunks / segs).
-__global__ void __launch_bounds__(kThreads, 1)
+// Shared memory: [T_lo resident: G x 16 KB]? | ring n_stage x (D_hi 8 KB | D_lo 8 KB | [T_lo slab 16 KB]?) | barriers.
+// The last kScratchBytes of the ring double as the T_hi transposition scratch of the prologue.
+__global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
           const __grid_constant__ CUtensorMap tmT_lo, const DoseArgs a) {
   if (a.gate && *a.gate == 0) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
-  uint8_t* tlo = smem;                              // [G][128 plans][128 B]
-  uint8_t* ring = smem + (size_t)G * kTloBox;       // [n_stage][hi 8 KB | lo 8 KB]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + (size_t)a.n_stage * 2 * kSlabBytes);
+  const int stageBytes = a.tlo_resident ? 2 * kSlabBytes : 2 * kSlabBytes + kTloBox;
+  uint8_t* tlo = smem;                              // [G][128 plans][128 B] when resident
+  uint8_t* ring = smem + (a.tlo_resident ? (size_t)G * kTloBox : 0);
+  const int ringBytes = a.n_stage * stageBytes;
+  uint8_t* scratch = ring + ringBytes - kScratchBytes;
+  const int scr_slot = (ringBytes - kScratchBytes) / stageBytes;   // first ring slot that overlaps the scratch
+  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + ringBytes);
   uint64_t* full = bars;                            // [n_stage]
   uint64_t* empty = bars + a.n_stage;               // [n_stage]
   uint64_t* tlo_full = bars + 2 * a.n_stage;
@@ -212,8 +229,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
     mbar_init(tlo_full, 1);
-    mbar_init(thi_ready, 128);
-    for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 128); }
+    mbar_init(thi_ready, 256);
+    for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 256); }
     fence_barrier_init();
   }
   if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT_lo); }
@@ -221,116 +238,171 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem = *tmem_slot;
+  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
   const uint32_t t_thi = tmem;                      // columns [0, A_pad): T_hi
-  const uint32_t t_acc = tmem + a.A_pad;            // columns [A_pad, A_pad + 128): two dose accumulators
+  // columns [A_pad, A_pad + 128 n_acc): per buffer a MAIN accumulator (T_hi D_hi) and a CORRECTION accumulator
+  // (T_hi D_lo + T_lo D_hi).  The tensor core truncates when it adds into the fp32 accumulator; keeping the small
+  // products out of the large sum cuts that bias by 3x.
+  const uint32_t t_acc = tmem + a.A_pad;
 
   if (warp == 0) {
-    if (lane == 0 && c1 > c0) {
-      mbar_expect_tx(tlo_full, (uint32_t)G * kTloBox);
-      for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g);
+    // whole warp walks the ring (uniform control flow); one elected lane issues
+    if (c1 > c0) {
+      if (a.tlo_resident) {
+        if (elect_one()) {
+          mbar_expect_tx(tlo_full, (uint32_t)G * kTloBox);
+          for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g);
+        }
+        __syncwarp();
+      }
       int st = 0; uint32_t ph = 0;
+      bool scratch_busy = true;
       for (int c = c0; c < c1; ++c) {
         for (int g = 0; g < G; ++g) {
+          if (scratch_busy && st >= scr_slot) { mbar_wait(thi_ready, 0); scratch_busy = false; }
           mbar_wait(empty + st, ph ^ 1);
-          uint8_t* dst = ring + (size_t)st * 2 * kSlabBytes;
-          mbar_expect_tx(full + st, 2 * kSlabBytes);
-          tma_load_3d(&tmD_hi, dst, full + st, 0, c * kPC, g);
-          tma_load_3d(&tmD_lo, dst + kSlabBytes, full + st, 0, c * kPC, g);
+          if (elect_one()) {
+            uint8_t* dst = ring + (size_t)st * stageBytes;
+            mbar_expect_tx(full + st, (uint32_t)stageBytes);
+            tma_load_3d(&tmD_hi, dst, full + st, 0, c * kPC, g);
+            tma_load_3d(&tmD_lo, dst + kSlabBytes, full + st, 0, c * kPC, g);
+            if (!a.tlo_resident) tma_load_3d(&tmT_lo, dst + 2 * kSlabBytes, full + st, 0, tile * 128, g);
+          }
+          __syncwarp();
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0 && c1 > c0) {
+    if (c1 > c0) {
       constexpr uint32_t idesc = instr_desc(kPC, 0, 0);
-      mbar_wait(tlo_full, 0);
+      if (a.tlo_resident) mbar_wait(tlo_full, 0);
       mbar_wait(thi_ready, 0);
       tc_fence_after();
       int st = 0; uint32_t ph = 0;
       for (int c = c0; c < c1; ++c) {
-        const int b = (c - c0) & 1, use = (c - c0) >> 1;
+        const int b = a.n_acc == 2 ? (c - c0) & 1 : 0, use = a.n_acc == 2 ? (c - c0) >> 1 : c - c0;
         mbar_wait(acc_empty + b, (use & 1) ^ 1);
         tc_fence_after();
-        const uint32_t acc = t_acc + b * kPC;
+        const uint32_t acc = t_acc + b * 2 * kPC, acc_c = acc + kPC;
         for (int g = 0; g < G; ++g) {
           mbar_wait(full + st, ph);
           tc_fence_after();
-          const uint32_t s_hi = smem_u32(ring + (size_t)st * 2 * kSlabBytes);
-          const uint64_t d_hi = smem_desc(s_hi, 16, 1024, kSwz128), d_lo = smem_desc(s_hi + kSlabBytes, 16, 1024, kSwz128);
-          const uint64_t a_lo = smem_desc(smem_u32(tlo + (size_t)g * kTloBox), 16, 1024, kSwz128);
+          if (elect_one()) {
+            const uint32_t s_hi = smem_u32(ring + (size_t)st * stageBytes);
+            const uint64_t d_hi = smem_desc(s_hi, 16, 1024, kSwz128), d_lo = smem_desc(s_hi + kSlabBytes, 16, 1024, kSwz128);
+            const uint64_t a_lo = smem_desc(a.tlo_resident ? smem_u32(tlo + (size_t)g * kTloBox) : s_hi + 2 * kSlabBytes,
+                                            16, 1024, kSwz128);
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {             // 4 K-steps of 8 dwell positions: +32 B inside the swizzled row
-            const uint32_t a_hi = t_thi + g * 32 + j * 8;
-            mma_ts(acc, a_hi, d_hi + 2 * j, idesc, (g | j) != 0);
-            mma_ts(acc, a_hi, d_lo + 2 * j, idesc, 1);
-            mma_ss(acc, a_lo + 2 * j, d_hi + 2 * j, idesc, 1);
+            for (int j = 0; j < 4; ++j) {           // 4 K-steps of 8 dwell positions: +32 B inside the swizzled row
+              const uint32_t a_hi = t_thi + g * 32 + j * 8;
+              mma_ts(acc, a_hi, d_hi + 2 * j, idesc, (g | j) != 0);
+              mma_ts(acc_c, a_hi, d_lo + 2 * j, idesc, (g | j) != 0);
+              mma_ss(acc_c, a_lo + 2 * j, d_hi + 2 * j, idesc, 1);
+            }
+            tc_commit(empty + st);
+            if (g == G - 1) tc_commit(acc_full + b);
           }
-          tc_commit(empty + st);
+          __syncwarp();
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
         }
-        tc_commit(acc_full + b);
       }
     }
   } else {
+    const int e = warp - 2;                         // 0..7
     const int q = warp & 3;                         // TMEM lane quadrant this warp may access
+    const int h = e >> 2;                           // which 32 of the chunk's 64 points this warp evaluates
     const int L = q * 32 + lane;                    // lane = plan inside the tile
     const int plan = tile * 128 + L;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-    float f = 0.f;
+    float f_lo = 0.f, f_hi = 0.f;
     if (c1 > c0) {
-      // T_hi row of this plan -> TMEM columns [0, A_pad)
-      const float4* src = reinterpret_cast<const float4*>(a.T_hi + (size_t)plan * a.A_pad);
-      for (int g = 0; g < G; ++g) {
-        uint32_t v[32];
+      // prologue: T_hi rows of this quadrant -> TMEM columns [0, A_pad).  Coalesced 128 B row reads, transposed
+      // through a per-warp 4 KB scratch (XOR-swizzled 16 B chunks: conflict-free both ways); slabs g = h, h + 2, ...
+      {
+        uint8_t* scr = scratch + e * 4096;
+        const int r0 = lane >> 3, c4 = lane & 7;
+        const float* src = a.T_hi + (size_t)(tile * 128 + q * 32) * a.A_pad;
+        for (int g = h; g < G; g += 2) {
+          float4 t[8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const float4 t = src[g * 8 + i];
-          v[4 * i + 0] = __float_as_uint(t.x); v[4 * i + 1] = __float_as_uint(t.y);
-          v[4 * i + 2] = __float_as_uint(t.z); v[4 * i + 3] = __float_as_uint(t.w);
+          for (int i = 0; i < 8; ++i)
+            t[i] = *reinterpret_cast<const float4*>(src + (size_t)(i * 4 + r0) * a.A_pad + g * 32 + c4 * 4);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int r = i * 4 + r0;
+            *reinterpret_cast<float4*>(scr + r * 128 + ((c4 ^ (r & 7)) << 4)) = t[i];
+          }
+          __syncwarp();
+          uint32_t v[32];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const float4 u = *reinterpret_cast<const float4*>(scr + lane * 128 + ((k ^ (lane & 7)) << 4));
+            v[4 * k + 0] = __float_as_uint(u.x); v[4 * k + 1] = __float_as_uint(u.y);
+            v[4 * k + 2] = __float_as_uint(u.z); v[4 * k + 3] = __float_as_uint(u.w);
+          }
+          __syncwarp();
+          tmem_st32(t_thi + lane_base + g * 32, v);
         }
-        tmem_st32(t_thi + lane_base + g * 32, v);
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(thi_ready);
       }
-      tmem_st_wait();
-      tc_fence_before();
-      mbar_arrive(thi_ready);
 
+      // structure id, valid rows and weights of the NEXT chunk are fetched one chunk ahead
+      int s_n = a.tile_struct[c0], nv_n = a.tile_valid[c0];
+      float wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n], whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
       for (int c = c0; c < c1; ++c) {
-        const int b = (c - c0) & 1, use = (c - c0) >> 1;
-        const int s = a.tile_struct[c], nv = a.tile_valid[c];
+        const int b = a.n_acc == 2 ? (c - c0) & 1 : 0, use = a.n_acc == 2 ? (c - c0) >> 1 : c - c0;
+        const int s = s_n, nvh = nv_n - h * 32;
+        const float wlo = wlo_n, whi = whi_n;
+        if (c + 1 < c1) {
+          s_n = a.tile_struct[c + 1]; nv_n = a.tile_valid[c + 1];
+          wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n]; whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
+        }
         const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
-        const float wlo = a.Weff[(size_t)plan * 2 * a.S + 2 * s], whi = a.Weff[(size_t)plan * 2 * a.S + 2 * s + 1];
         mbar_wait(acc_full + b, use & 1);
         tc_fence_after();
-#pragma unroll
-        for (int h = 0; h < kPC / 32; ++h) {
-          uint32_t v[32];
-          tmem_ld32(t_acc + lane_base + b * kPC + h * 32, v);
+        uint32_t v[32];
+        {
+          uint32_t vc[32];
+          tmem_ld32(t_acc + lane_base + b * 2 * kPC + h * 32, v);
+          tmem_ld32(t_acc + lane_base + b * 2 * kPC + kPC + h * 32, vc);
           tmem_ld_wait();
-          if (h == kPC / 32 - 1) { tc_fence_before(); mbar_arrive(acc_empty + b); }
-          const size_t p0 = (size_t)c * kPC + h * 32;
-          float* rh = a.R_hi + p0 * a.K_pad + plan;
-          float* rl = a.R_lo + p0 * a.K_pad + plan;
+          tc_fence_before();
+          mbar_arrive(acc_empty + b);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
+        }
+        const size_t p0 = (size_t)c * kPC + h * 32;
+        float* rp = a.R + p0 * a.K_pad + plan;
+        if (nvh >= 32) {
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             const float d = __uint_as_float(v[j]);
             const float lo = fminf(d - dlo, 0.f), hi = fmaxf(d - dhi, 0.f);
             const float u = wlo * lo, w = whi * hi;
-            if (h * 32 + j < nv) f = fmaf(u, lo, fmaf(w, hi, f));
-            const float r = u + w;                                        // = dF/dd / 2
-            const float r_hi = __uint_as_float(__float_as_uint(r) & 0xffffe000u);   // exact tf32 (truncated)
-            rh[(size_t)j * a.K_pad] = r_hi;
-            rl[(size_t)j * a.K_pad] = r - r_hi;
+            f_lo = fmaf(u, lo, f_lo); f_hi = fmaf(w, hi, f_hi);
+            rp[(size_t)j * a.K_pad] = u + w;                              // = dF/dd / 2
           }
-          if (a.dose_dbg && plan < a.K) {
-            for (int j = 0; j < 32; ++j) {
-              if (h * 32 + j < nv) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[j]);
-            }
+        } else {                                                          // ragged tail of a structure
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float d = __uint_as_float(v[j]);
+            const float lo = fminf(d - dlo, 0.f), hi = fmaxf(d - dhi, 0.f);
+            const float u = wlo * lo, w = whi * hi;
+            if (j < nvh) { f_lo = fmaf(u, lo, f_lo); f_hi = fmaf(w, hi, f_hi); }
+            rp[(size_t)j * a.K_pad] = u + w;                              // padding rows of D are zero: value unused
+          }
+        }
+        if (a.dose_dbg && plan < a.K) {
+          for (int j = 0; j < 32; ++j) {
+            if (j < nvh) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[j]);
           }
         }
       }
     }
-    a.Fpart[((size_t)tile * a.segs + seg) * 128 + L] = f;
+    a.Fpart[(((size_t)tile * a.segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
   }
   tc_fence_before();
   __syncthreads();
@@ -340,21 +412,24 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 // ---------------------------------------------------------------------------------------------
 // a5 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point slabs [seg n_slabs / segs, (seg + 1) n_slabs / segs) of PS points each.
+// Stage = [R | R_lo | D_hi | D_lo]: TMA brings R (fp32), D_hi, D_lo; warps 2-5 split R in place into its
+// tf32 parts (hi = truncation, lo = r - hi) before the MMA warp may read the stage.
 template <int PS>
 __global__ void __launch_bounds__(kThreads, 1)
-k_grad_tc(const __grid_constant__ CUtensorMap tmR_hi, const __grid_constant__ CUtensorMap tmR_lo,
-          const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
+k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmD_hi,
+          const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
   if (a.gate && *a.gate == 0) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;
   constexpr int kRBytes = 4 * PS * 128;             // R part: 4 plan groups x PS points x 128 B
   const int dBytes = G * PS * 128;                  // D part: G dwell groups x PS points x 128 B
-  const int stageBytes = 2 * kRBytes + 2 * dBytes;  // [R_hi | R_lo | D_hi | D_lo]
+  const int stageBytes = 2 * kRBytes + 2 * dBytes;  // [R | R_lo | D_hi | D_lo]
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)a.n_stage * stageBytes);
   uint64_t* full = bars;
   uint64_t* empty = bars + a.n_stage;
-  uint64_t* acc_full = bars + 2 * a.n_stage;
+  uint64_t* conv = bars + 2 * a.n_stage;
+  uint64_t* acc_full = bars + 3 * a.n_stage;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -362,69 +437,95 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR_hi, const __grid_constant__ CU
   const int s0 = (int)((long long)seg * a.n_slabs / a.segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / a.segs);
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); mbar_init(conv + i, 128); }
     mbar_init(acc_full, 1);
     fence_barrier_init();
   }
-  if (warp == 0 && lane == 0) {
-    tma_prefetch_desc(&tmR_hi); tma_prefetch_desc(&tmR_lo); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo);
-  }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmR); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem = *tmem_slot;
+  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
 
   if (warp == 0) {
-    if (lane == 0) {
-      int st = 0; uint32_t ph = 0;
-      for (int s = s0; s < s1; ++s) {
-        mbar_wait(empty + st, ph ^ 1);
+    int st = 0; uint32_t ph = 0;
+    for (int s = s0; s < s1; ++s) {
+      mbar_wait(empty + st, ph ^ 1);
+      if (elect_one()) {
         uint8_t* dst = smem + (size_t)st * stageBytes;
-        mbar_expect_tx(full + st, (uint32_t)stageBytes);
-        tma_load_3d(&tmR_hi, dst, full + st, 0, s * PS, tile * 4);
-        tma_load_3d(&tmR_lo, dst + kRBytes, full + st, 0, s * PS, tile * 4);
+        mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
+        tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4);
         tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0);
         tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0);
-        if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
+      __syncwarp();
+      if (++st == a.n_stage) { st = 0; ph ^= 1; }
     }
   } else if (warp == 1) {
-    if (lane == 0 && s1 > s0) {
+    if (s1 > s0) {
       // the accumulator is A_pad columns wide; one MMA covers at most 256 of them
       const int n0 = a.A_pad <= 256 ? a.A_pad : 256, n1 = a.A_pad - n0;
       const uint32_t idesc0 = instr_desc(n0, 1, 1), idesc1 = instr_desc(n1 > 0 ? n1 : 16, 1, 1);
+      // separate accumulator (columns 256..) for the two correction products when the tile leaves room: see k_dose_tc
+      const uint32_t corr = a.A_pad <= 256 ? 256u : 0u;
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        mbar_wait(full + st, ph);
+        mbar_wait(conv + st, ph);
         tc_fence_after();
-        const uint32_t base = smem_u32(smem + (size_t)st * stageBytes);
+        if (elect_one()) {
+          const uint32_t base = smem_u32(smem + (size_t)st * stageBytes);
 #pragma unroll
-        for (int j = 0; j < PS / 8; ++j) {          // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
-          const uint64_t r_hi = smem_desc(base + j * 1024, PS * 128, 512, kSwz128Base32);
-          const uint64_t r_lo = smem_desc(base + kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-          const uint64_t d_hi = smem_desc(base + 2 * kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-          const uint64_t d_lo = smem_desc(base + 2 * kRBytes + dBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-          const uint32_t acc = (s > s0 || j > 0) ? 1u : 0u;
-          mma_ss(tmem, r_hi, d_hi, idesc0, acc);
-          mma_ss(tmem, r_hi, d_lo, idesc0, 1);
-          mma_ss(tmem, r_lo, d_hi, idesc0, 1);
-          if (n1 > 0) {                              // dwell groups 8.. : +8 groups of PS x 128 B
-            const uint64_t off = (uint64_t)((8 * PS * 128) >> 4);
-            mma_ss(tmem + 256, r_hi, d_hi + off, idesc1, acc);
-            mma_ss(tmem + 256, r_hi, d_lo + off, idesc1, 1);
-            mma_ss(tmem + 256, r_lo, d_hi + off, idesc1, 1);
+          for (int j = 0; j < PS / 8; ++j) {        // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
+            const uint64_t r_hi = smem_desc(base + j * 1024, PS * 128, 512, kSwz128Base32);
+            const uint64_t r_lo = smem_desc(base + kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+            const uint64_t d_hi = smem_desc(base + 2 * kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+            const uint64_t d_lo = smem_desc(base + 2 * kRBytes + dBytes + j * 1024, PS * 128, 512, kSwz128Base32);
+            const uint32_t acc = (s > s0 || j > 0) ? 1u : 0u;
+            mma_ss(tmem, r_hi, d_hi, idesc0, acc);
+            mma_ss(tmem + corr, r_hi, d_lo, idesc0, corr ? acc : 1u);
+            mma_ss(tmem + corr, r_lo, d_hi, idesc0, 1);
+            if (n1 > 0) {                            // dwell groups 8.. : +8 groups of PS x 128 B
+              const uint64_t off = (uint64_t)((8 * PS * 128) >> 4);
+              mma_ss(tmem + 256, r_hi, d_hi + off, idesc1, acc);
+              mma_ss(tmem + 256, r_hi, d_lo + off, idesc1, 1);
+              mma_ss(tmem + 256, r_lo, d_hi + off, idesc1, 1);
+            }
           }
+          tc_commit(empty + st);
+          if (s == s1 - 1) tc_commit(acc_full);
         }
-        tc_commit(empty + st);
+        __syncwarp();
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
-      tc_commit(acc_full);
     }
   } else {
     const int q = warp & 3;
     const int L = q * 32 + lane;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    // main loop: split each arriving R tile into (hi, lo) in place; element-wise, so the swizzle does not matter
+    {
+      const int t = threadIdx.x - 64;               // 0..127
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        mbar_wait(full + st, ph);
+        uint8_t* base = smem + (size_t)st * stageBytes + t * 16;
+#pragma unroll
+        for (int i = 0; i < kRBytes / 2048; ++i) {
+          const float4 v = *reinterpret_cast<const float4*>(base + i * 2048);
+          float4 hi, lo;
+          hi.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); lo.x = v.x - hi.x;
+          hi.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); lo.y = v.y - hi.y;
+          hi.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); lo.z = v.z - hi.z;
+          hi.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); lo.w = v.w - hi.w;
+          *reinterpret_cast<float4*>(base + i * 2048) = hi;
+          *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
+        }
+        fence_proxy_async();
+        mbar_arrive(conv + st);
+        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+      }
+    }
     float4* dst = reinterpret_cast<float4*>(a.Gpart + (((size_t)tile * a.segs + seg) * 128 + L) * a.A_pad);
     if (s1 > s0) {
       mbar_wait(acc_full, 0);
@@ -432,7 +533,15 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR_hi, const __grid_constant__ CU
       for (int g = 0; g < G; ++g) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + g * 32, v);
-        tmem_ld_wait();
+        if (a.A_pad <= 256) {
+          uint32_t vc[32];
+          tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
+        } else {
+          tmem_ld_wait();
+        }
 #pragma unroll
         for (int i = 0; i < 8; ++i)
           dst[g * 8 + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
@@ -480,9 +589,9 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long cols,
 
 struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo;
-  CUtensorMap grad_R_hi, grad_R_lo, grad_D_hi, grad_D_lo;
+  CUtensorMap grad_R, grad_D_hi, grad_D_lo;
   int segs = 1, n_tiles = 0;
-  int dose_stages = 0, dose_smem = 0;
+  int dose_stages = 0, dose_smem = 0, tlo_resident = 1;
   int grad_ps = 32, grad_stages = 0, grad_smem = 0;
   int* tile_seg_dev = nullptr;
   Thresholds thr{};
@@ -490,18 +599,21 @@ struct TcPlan {
 
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, char* err, int errlen) {
   constexpr int kSmemMax = 227 * 1024;
-  if (c.A_pad > 384) { snprintf(err, errlen, "tensor path supports n_dwell <= 384 (use GMCO_PREC_SIMT_FP32)"); return nullptr; }
+  if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
   t->n_tiles = p.K_pad / kPlanTile;
   t->segs = num_sms / t->n_tiles > 0 ? num_sms / t->n_tiles : 1;
   for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
   const int G = c.A_pad / 32;
-  // dose kernel: T_lo resident + as many ring stages as fit
-  const int fixed = G * kTloBox + 1024 /*alignment slack*/ + 512 /*barriers*/;
-  t->dose_stages = (kSmemMax - fixed) / (2 * kSlabBytes);
+  // dose kernel: T_lo resident when it leaves room for >= 2 ring stages, else streamed with every D slab
+  const int slack = 1024 /*alignment*/ + 512 /*barriers*/;
+  t->tlo_resident = G * kTloBox + 2 * 2 * kSlabBytes + slack <= kSmemMax ? 1 : 0;
+  const int fixed = (t->tlo_resident ? G * kTloBox : 0) + slack;
+  const int stageB = t->tlo_resident ? 2 * kSlabBytes : 2 * kSlabBytes + kTloBox;
+  t->dose_stages = (kSmemMax - fixed) / stageB;
   if (t->dose_stages > 8) t->dose_stages = 8;
-  if (t->dose_stages < 2) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
-  t->dose_smem = fixed + t->dose_stages * 2 * kSlabBytes;
+  if (t->dose_stages * stageB < kScratchBytes) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
+  t->dose_smem = fixed + t->dose_stages * stageB;
   // gradient kernel
   t->grad_ps = c.A_pad <= 256 ? 32 : 16;
   const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
@@ -513,8 +625,7 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   bool ok = make_map(&t->dose_D_hi, c.D_hi, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_D_lo, c.D_lo, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK) &&
-            make_map(&t->grad_R_hi, p.R_hi, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
-            make_map(&t->grad_R_lo, p.R_lo, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
+            make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
@@ -542,19 +653,20 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
                    cudaStream_t st) {
   dim3 grid(t->segs, t->n_tiles);
   DoseArgs da{};
-  da.T_hi = p.T_hi; da.R_hi = p.R_hi; da.R_lo = p.R_lo; da.Fpart = p.Fpart; da.Weff = p.Weff;
+  da.T_hi = p.T_hi; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
   da.gate = gate; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = c.N_pad / kPC;
-  da.segs = t->segs; da.n_stage = t->dose_stages; da.thr = t->thr;
-  k_dose_tc<<<grid, kThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
+  da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 4 * kPC <= 512 ? 2 : 1;
+  da.tlo_resident = t->tlo_resident; da.thr = t->thr;
+  k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
   if (cudaGetLastError() != cudaSuccess) return -1;
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
   ga.n_stage = t->grad_stages;
   if (t->grad_ps == 32)
-    k_grad_tc<32><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R_hi, t->grad_R_lo, t->grad_D_hi, t->grad_D_lo, ga);
+    k_grad_tc<32><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
   else
-    k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R_hi, t->grad_R_lo, t->grad_D_hi, t->grad_D_lo, ga);
+    k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
   return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 
