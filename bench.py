@@ -56,6 +56,8 @@ class ClockSampler:
         self.index, self.period, self.rows, self.stop, self.t, self.h = index, period_s, [], False, None, None
 
     def __enter__(self):
+        if self.period <= 0:
+            return self
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -155,6 +157,7 @@ def main():
     ap.add_argument("--precision", default="tf32x3", choices=["tf32x3", "simt"])
     ap.add_argument("--ref-sample", type=int, default=32, help="plans per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--clock-period", type=float, default=0.02, help="seconds between NVML clock samples (0 = off)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -232,7 +235,7 @@ def main():
     for _ in range(args.warmup):
         step(False); step(True)
     barrier()
-    with ClockSampler(local) as clk:
+    with ClockSampler(local, args.clock_period) as clk:
         ms_dev = timed(False, args.steps)
         barrier()
     ms_dev = max_over_ranks(ms_dev)

@@ -44,8 +44,15 @@ struct gmco_handle {
   float *in_T0 = nullptr, *in_w = nullptr;
   float *out_T = nullptr, *out_F = nullptr, *out_dvh = nullptr, *out_terms = nullptr;
   int *out_iters = nullptr, *out_status = nullptr;
-  int* host_flags = nullptr;         // pinned [4]
+  int host_flags[4] = {0, 0, 0, 0};  // pageable: the copies into it are followed by a stream synchronise
   TcPlan* tc = nullptr;
+  // device-driven round loop: a CUDA graph whose only node is a WHILE conditional; its body is two rounds
+  // (parity 0, parity 1) and a kernel that keeps the loop going while a plan is still running
+  cudaGraph_t loop_graph = nullptr;
+  cudaGraphExec_t loop_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;  // capture only (the caller's stream may be the legacy stream, which cannot capture)
+  int loop_K = -1, loop_iters = -1, loop_launches_per_pair = 0;
+  bool used_graph = false;
   cudaStream_t stream = nullptr;
   int device = 0, num_sms = 0;
   HandleState state = ST_CREATED;
@@ -135,8 +142,9 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   p.F = a.take<float>(kp); p.gp = a.take<float>(kp); p.alpha = a.take<float>(kp);
   p.it_done = a.take<int>(kp); p.trials = a.take<int>(kp); p.hcount = a.take<int>(kp); p.hhead = a.take<int>(kp);
   p.status = a.take<int>(kp);
-  p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1);
+  p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1); p.rounds_done = a.take<int>(1);
   p.round_log = a.take<int>(kRoundLogCap);
+  p.tile_seg = a.take<int>(p.K_pad / kPlanTile + 1);
   // partials: the SIMT dose pass (also the final pass of gmco_result) needs [tiles][K_pad][2]
   const size_t f_simt = (size_t)(c.N_alloc / 64) * kp * 2;
   p.nFcomp = 2; p.nF = c.N_alloc / 64;
@@ -168,11 +176,14 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   (void)dose_stage_elems;
 }
 
+void destroy_loop_graph(gmco_handle* h);
+
 int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   if (h->plan_capacity_K == K && h->plan_arena.base && h->stream == st) {
     return GMCO_OK;
   }
   if (h->tc) { tc_plan_destroy(h->tc); h->tc = nullptr; }
+  destroy_loop_graph(h);
   arena_free(h->plan_arena, h->stream);
   carve_plans(h, K, 0);                       // measuring pass
   int rc = arena_alloc(h, h->plan_arena, st);
@@ -180,7 +191,7 @@ int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   carve_plans(h, K, 0);
   h->plan_capacity_K = K;
   if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
-    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->err, sizeof(h->err));
+    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, st, h->err, sizeof(h->err));
     if (!h->tc) return GMCO_E_UNSUPPORTED;
   }
   return GMCO_OK;
@@ -217,26 +228,74 @@ int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, cudaStream_t 
   return GMCO_OK;
 }
 
+// one round: every running plan has its trial point evaluated, then accepted or its step halved
+int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const StepParams& sp, cudaStream_t st) {
+  LN(h, launch_round_begin(h->p, parity, log_idx, st));
+  if (prof) {
+    while ((int)h->ev.size() < h->ev_used + 2) {
+      cudaEvent_t e;
+      CK(h, cudaEventCreate(&e));
+      h->ev.push_back(e);
+    }
+    CK(h, cudaEventRecord(h->ev[h->ev_used], st));
+  }
+  int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, st);
+  if (rc) return rc;
+  if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
+  LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
+  return GMCO_OK;
+}
+
+// host-driven rounds (profiling mode: per-round events need one launch per round)
 int enqueue_rounds(gmco_handle* h, int n, cudaStream_t st) {
   const StepParams sp = make_step_params(h, h->iters);
   for (int i = 0; i < n; ++i) {
-    const int parity = h->rounds_enqueued & 1;
-    LN(h, launch_round_begin(h->p, parity, h->rounds_enqueued, st));
     const bool prof = h->profile && h->rounds_enqueued < kRoundLogCap;
-    if (prof) {
-      while ((int)h->ev.size() < h->ev_used + 2) {
-        cudaEvent_t e;
-        CK(h, cudaEventCreate(&e));
-        h->ev.push_back(e);
-      }
-      CK(h, cudaEventRecord(h->ev[h->ev_used], st));
-    }
-    int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, st);
+    int rc = enqueue_round(h, h->rounds_enqueued & 1, h->rounds_enqueued, prof, sp, st);
     if (rc) return rc;
-    if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
-    LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
     h->rounds_enqueued++;
   }
+  return GMCO_OK;
+}
+
+void destroy_loop_graph(gmco_handle* h) {
+  if (h->loop_exec) cudaGraphExecDestroy(h->loop_exec);
+  if (h->loop_graph) cudaGraphDestroy(h->loop_graph);
+  h->loop_exec = nullptr; h->loop_graph = nullptr; h->loop_K = -1; h->loop_iters = -1;
+}
+
+long long max_rounds_of(const gmco_handle* h) { return 1 + (long long)h->iters * ((long long)h->opt.max_trials + 1); }
+
+// device-driven rounds: WHILE(conditional) { round(parity 0); round(parity 1); keep going while n_running[0] > 0 }
+int build_loop_graph(gmco_handle* h) {
+  if (h->loop_exec && h->loop_K == h->p.K && h->loop_iters == h->iters) return GMCO_OK;
+  destroy_loop_graph(h);
+  if (!h->cap_stream) CK(h, cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+  CK(h, cudaGraphCreate(&h->loop_graph, 0));
+  cudaGraphConditionalHandle cond;
+  CK(h, cudaGraphConditionalHandleCreate(&cond, h->loop_graph, 1, cudaGraphCondAssignDefault));
+  cudaGraphNodeParams np{};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = cond; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+  cudaGraphNode_t node;
+  CK(h, cudaGraphAddNode(&node, h->loop_graph, nullptr, 0, &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  CK(h, cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+  const StepParams sp = make_step_params(h, h->iters);
+  const int before = h->launches;
+  const long long mr = max_rounds_of(h);
+  int rc = enqueue_round(h, 0, kRoundLogCap, false, sp, h->cap_stream);
+  if (!rc) rc = enqueue_round(h, 1, kRoundLogCap, false, sp, h->cap_stream);
+  if (!rc && launch_loop_cond(cond, h->p, (int)(mr > 0x7fffffff ? 0x7fffffff : mr), h->cap_stream) < 0)
+    rc = fail(h, GMCO_E_CUDA, "loop condition kernel: %s", cudaGetErrorString(cudaGetLastError()));
+  h->loop_launches_per_pair = h->launches - before + 1;
+  h->launches = before;
+  cudaError_t e = cudaStreamEndCapture(h->cap_stream, nullptr);
+  if (rc) { destroy_loop_graph(h); return rc; }
+  if (e != cudaSuccess) { destroy_loop_graph(h); return fail(h, GMCO_E_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e)); }
+  e = cudaGraphInstantiate(&h->loop_exec, h->loop_graph, 0);
+  if (e != cudaSuccess) { destroy_loop_graph(h); return fail(h, GMCO_E_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+  h->loop_K = h->p.K; h->loop_iters = h->iters;
   return GMCO_OK;
 }
 
@@ -309,14 +368,16 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return fail(nullptr, GMCO_E_UNSUPPORTED, "no CUDA device: %s", cudaGetErrorString(e));
-  cudaDeviceProp prop{};
-  e = cudaGetDeviceProperties(&prop, dev);
-  if (e != cudaSuccess) return fail(nullptr, GMCO_E_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
-  if (prop.major != 10) return fail(nullptr, GMCO_E_UNSUPPORTED, "libgmco needs an sm_100 device (B200)%s");
+  // cudaDeviceGetAttribute, not cudaGetDeviceProperties: the latter takes about a millisecond per call
+  int cc_major = 0, n_sms = 0;
+  e = cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return fail(nullptr, GMCO_E_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+  if (cc_major != 10) return fail(nullptr, GMCO_E_UNSUPPORTED, "libgmco needs an sm_100 device (B200)%s");
 
   gmco_handle* h = new (std::nothrow) gmco_handle();
   if (!h) return fail(nullptr, GMCO_E_NOMEM, "host allocation failed%s");
-  h->opt = o; h->device = dev; h->num_sms = prop.multiProcessorCount;
+  h->opt = o; h->device = dev; h->num_sms = n_sms;
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   h->structs.assign(structs, structs + n_structs);
   cudaStream_t st = h->stream;
@@ -404,7 +465,6 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
     fail(nullptr, GMCO_E_CUDA, "case setup kernels: %s", cudaGetErrorString(cudaGetLastError()));
     arena_free(h->case_arena, st); delete h; return GMCO_E_CUDA;
   }
-  CKC(cudaMallocHost(reinterpret_cast<void**>(&h->host_flags), 4 * sizeof(int)));
 #undef CKC
   *out = h;
   return GMCO_OK;
@@ -421,9 +481,10 @@ void gmco_destroy(gmco_handle* h) {
   cudaStreamSynchronize(h->stream);
   for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   if (h->tc) tc_plan_destroy(h->tc);
+  destroy_loop_graph(h);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   arena_free(h->plan_arena, h->stream);
   arena_free(h->case_arena, h->stream);
-  if (h->host_flags) cudaFreeHost(h->host_flags);
   delete h;
 }
 
@@ -443,11 +504,19 @@ int gmco_optimize(gmco_handle* h, const float* T0, int32_t t0_broadcast, const f
   if (rc) return rc;
   LN(h, launch_init_plans(h->c, h->p, T0d, t0_broadcast ? 1 : 0, wd, h->struct_scale, st));
   // round 0 evaluates the start point; every further round is one trial step of every running plan.
-  // Backtracking plans need extra rounds: enqueue some slack now (rounds with nothing running return
-  // at once), gmco_result adds more if a plan is still running.
-  const int slack = iters > 0 ? (iters / 6 > 4 ? iters / 6 : 4) : 0;
-  rc = enqueue_rounds(h, 1 + iters + slack, st);
-  if (rc) return rc;
+  // Profiling mode drives the rounds from the host; backtracking plans need extra rounds, so it enqueues some
+  // slack now (rounds with nothing running return at once) and gmco_result adds more if a plan is still running.
+  h->used_graph = !h->profile;
+  if (h->used_graph) {
+    // the loop runs on the device until no plan is running: no slack rounds, no host polling
+    rc = build_loop_graph(h);
+    if (rc) return rc;
+    CK(h, cudaGraphLaunch(h->loop_exec, st));
+  } else {
+    const int slack = iters > 0 ? (iters / 6 > 4 ? iters / 6 : 4) : 0;
+    rc = enqueue_rounds(h, 1 + iters + slack, st);
+    if (rc) return rc;
+  }
   h->state = ST_OPTIMIZED;
   return GMCO_OK;
 }
@@ -466,13 +535,19 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
     return GMCO_OK;
   }
   if (h->state == ST_OPTIMIZED) {
-    const long long max_rounds = 1 + (long long)h->iters * ((long long)h->opt.max_trials + 1);
+    const long long max_rounds = max_rounds_of(h);
     for (;;) {
-      const int parity = h->rounds_enqueued & 1;          // counter the NEXT round would read
+      const int parity = h->used_graph ? 0 : h->rounds_enqueued & 1;   // counter the NEXT round would read
       CK(h, cudaMemcpyAsync(h->host_flags, p.n_running + parity, sizeof(int), cudaMemcpyDeviceToHost, st));
       CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(h, cudaMemcpyAsync(h->host_flags + 2, p.rounds_done, sizeof(int), cudaMemcpyDeviceToHost, st));
       CK(h, cudaStreamSynchronize(st));
       if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
+      if (h->used_graph) {
+        h->rounds_enqueued = h->host_flags[2];
+        h->launches += (h->host_flags[2] / 2) * h->loop_launches_per_pair;
+        break;
+      }
       if (h->host_flags[0] == 0 || h->rounds_enqueued >= max_rounds) break;
       int rc = enqueue_rounds(h, 8, st);
       if (rc) return rc;

@@ -58,7 +58,9 @@ struct PlanDev {
   float *F = nullptr, *gp = nullptr, *alpha = nullptr;             // [K_pad]
   int *it_done = nullptr, *trials = nullptr, *hcount = nullptr, *hhead = nullptr, *status = nullptr;
   int *n_running = nullptr;                                        // [2] ping-pong counter of RUNNING plans
+  int *tile_seg = nullptr;                                         // [K_pad / 128 + 1] partial-slot range of each plan tile (tensor route)
   int *round_log = nullptr;                                        // [kRoundLogCap] running plans at the start of round r
+  int *rounds_done = nullptr;                                      // [1] rounds executed by the device-driven loop
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
   // partial results of one evaluation round
   float *Fpart = nullptr; float *Gpart = nullptr;
@@ -91,6 +93,7 @@ int launch_simt_eval(const CaseDev& c, const PlanDev& p, bool write_R, float* do
                      bool dvh_mode, const float* dvh_thr /*[S] device*/, const int* gate, cudaStream_t st);
 int launch_simt_grad(const CaseDev& c, const PlanDev& p, const int* gate, cudaStream_t st);
 int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st);
+int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_rounds, cudaStream_t st);
 int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
                        cudaStream_t st);
 int launch_eval_finish_scaled(const CaseDev& c, const PlanDev& p, const StepParams& sp, float g_scale, float* F_out,
@@ -101,7 +104,8 @@ int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st);
 
 // tensor path (kernel_fused_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
-TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, char* err, int errlen);
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
+                       char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 const int* tc_tile_seg_dev(const TcPlan*);

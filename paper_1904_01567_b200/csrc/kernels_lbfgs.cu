@@ -74,6 +74,7 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
                       const float* struct_scale, cudaStream_t st) {
   if (p.K_pad == 0) return 0;
   cudaMemsetAsync(p.bad_input, 0, sizeof(int), st);
+  cudaMemsetAsync(p.rounds_done, 0, sizeof(int), st);
   k_init_plans<<<p.K_pad, 128, 0, st>>>(make_ptrs(p), p.K, c.A, c.A_pad, c.S, T0, t0_bcast, w_user, struct_scale,
                                         p.Weff);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
@@ -296,6 +297,19 @@ int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp,
 __global__ void k_round_begin(int* n_running, int parity, int* log_slot) {
   n_running[parity ^ 1] = 0;
   if (log_slot) *log_slot = n_running[parity];
+}
+
+// tail of the WHILE body (two rounds): loop again while a plan is running and the round budget lasts
+__global__ void k_loop_cond(cudaGraphConditionalHandle cond, const int* __restrict__ n_running, int* rounds_done,
+                            int max_rounds) {
+  const int r = *rounds_done + 2;
+  *rounds_done = r;
+  cudaGraphSetConditional(cond, (n_running[0] > 0 && r < max_rounds) ? 1u : 0u);
+}
+
+int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_rounds, cudaStream_t st) {
+  k_loop_cond<<<1, 1, 0, st>>>(cond, p.n_running, p.rounds_done, max_rounds);
+  return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
 int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st) {

@@ -597,7 +597,8 @@ struct TcPlan {
   Thresholds thr{};
 };
 
-TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, char* err, int errlen) {
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
+                       char* err, int errlen) {
   constexpr int kSmemMax = 227 * 1024;
   if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
@@ -634,15 +635,14 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   std::vector<int> seg(t->n_tiles + 1);
   for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
-  if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&t->tile_seg_dev), seg.size() * sizeof(int));
-  if (e == cudaSuccess) e = cudaMemcpy(t->tile_seg_dev, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice);
+  t->tile_seg_dev = p.tile_seg;                    // lives in the plan arena; pageable source: staged before the call returns
+  if (e == cudaSuccess) e = cudaMemcpyAsync(t->tile_seg_dev, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) { snprintf(err, errlen, "tensor plan setup: %s", cudaGetErrorString(e)); tc_plan_destroy(t); return nullptr; }
   return t;
 }
 
 void tc_plan_destroy(TcPlan* t) {
   if (!t) return;
-  if (t->tile_seg_dev) cudaFree(t->tile_seg_dev);
   delete t;
 }
 
