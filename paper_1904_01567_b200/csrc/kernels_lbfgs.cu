@@ -96,26 +96,73 @@ __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, in
   f = warp_sum(f);
 #pragma unroll
   for (int j = 0; j < NPL; ++j) G[j] = 0.f;
-  for (int s = g0; s < g1; ++s) {
-    const float* gp = sp.Gpart + (long long)s * sp.g_slot_stride + prow * sp.A_pad + lane;
+  // four slots' loads are issued before the first add (the loads are what costs time); the adds keep slot order
+  const float* gp = sp.Gpart + (long long)g0 * sp.g_slot_stride + prow * sp.A_pad + lane;
+  int s = g0;
+  for (; s + 4 <= g1; s += 4, gp += 4 * sp.g_slot_stride) {
+    float v[4][NPL];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * sp.g_slot_stride + 32 * j) : 0.f;
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
+  }
+  for (; s < g1; ++s, gp += sp.g_slot_stride) {
 #pragma unroll
     for (int j = 0; j < NPL; ++j)
-      if (j < npl) G[j] += gp[32 * j];
+      if (j < npl) G[j] += __ldcs(gp + 32 * j);
   }
   return f;
 }
 
 // ---------------------------------------------------------------------------------------------
+// The history of a plan (m pairs, 2 m A_pad floats) is staged in shared memory by bulk asynchronous copies issued
+// at the very start, so the 2 m dependent dot products of the two-loop recursion read shared memory instead of
+// paying one HBM/L2 latency each.  wpb warps (= plans) per CTA; dynamic smem = wpb * 2 m A_pad floats.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
 template <int NPL>
-__global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int parity, float g_scale) {
+__global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int parity, float g_scale, int wpb) {
+  extern __shared__ __align__(128) float s_hist[];
   __shared__ float s_a[4][GMCO_MAX_HISTORY];
+  __shared__ __align__(8) unsigned long long s_bar[4];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int k = blockIdx.x * 4 + warp;
+  const int k = blockIdx.x * wpb + warp;
   if (pp.n_running[parity] == 0) return;
   if (k >= sp.K || pp.status[k] != PLAN_RUNNING) return;
   const int npl = sp.A_pad >> 5;
   const long long row = (long long)k * sp.A_pad + lane;
   const long long hstride = (long long)pp.K_pad * sp.A_pad;
+  float* hS = s_hist + (size_t)warp * 2 * sp.m * sp.A_pad;     // [m][A_pad] s vectors, by ring slot
+  float* hY = hS + (size_t)sp.m * sp.A_pad;                    // [m][A_pad] y vectors
+  {
+    const uint32_t bar = smem_addr(&s_bar[warp]);
+    const uint32_t bytes = (uint32_t)sp.A_pad * 4u;
+    if (lane == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * 2u * (uint32_t)sp.m) : "memory");
+    }
+    __syncwarp();
+    for (int i = lane; i < 2 * sp.m; i += 32) {                // one 4 A_pad byte row per lane
+      const int slot = i < sp.m ? i : i - sp.m;
+      const float* src = (i < sp.m ? pp.Sh : pp.Yh) + slot * hstride + (long long)k * sp.A_pad;
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(smem_addr(hS + (size_t)i * sp.A_pad)), "l"(src), "r"(bytes), "r"(bar) : "memory");
+    }
+  }
+  // every path below waits for the copies before the warp may leave (the CTA's shared memory must outlive them)
+  auto hist_wait = [&]() {
+    const uint32_t bar = smem_addr(&s_bar[warp]);
+    uint32_t ok = 0;
+    while (!ok) {
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(ok) : "r"(bar) : "memory");
+    }
+  };
 
   float G[NPL], xt[NPL], gt[NPL], x[NPL], g[NPL];
   const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G);
@@ -161,12 +208,16 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         sy = fmaf(sv[j], yv[j], sy); ss = fmaf(sv[j], sv[j], ss); yy = fmaf(yv[j], yv[j], yy);
       }
       sy = warp_sum(sy); ss = warp_sum(ss); yy = warp_sum(yy);
+      hist_wait();                                           // the staged copy of slot hh is about to be replaced
       if (sy > 1e-10f * sqrtf(ss) * sqrtf(yy)) {             // curvature guard
         float* Sd = pp.Sh + hh * hstride + row;
         float* Yd = pp.Yh + hh * hstride + row;
 #pragma unroll
         for (int j = 0; j < NPL; ++j)
-          if (j < npl) { Sd[32 * j] = sv[j]; Yd[32 * j] = yv[j]; }
+          if (j < npl) {
+            Sd[32 * j] = sv[j]; Yd[32 * j] = yv[j];
+            hS[hh * sp.A_pad + lane + 32 * j] = sv[j]; hY[hh * sp.A_pad + lane + 32 * j] = yv[j];
+          }
         if (lane == 0) { pp.rho[(long long)hh * pp.K_pad + k] = 1.f / sy; pp.gam[(long long)hh * pp.K_pad + k] = sy / yy; }
         hh = hh + 1 == sp.m ? 0 : hh + 1;
         hc = min(hc + 1, sp.m);
@@ -211,10 +262,12 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
       float q[NPL];
 #pragma unroll
       for (int j = 0; j < NPL; ++j) q[j] = g[j];
+      hist_wait();
+      __syncwarp();
       for (int i = 0; i < hc; ++i) {
         int slot = hh - 1 - i; if (slot < 0) slot += sp.m;
-        const float* Sd = pp.Sh + slot * hstride + row;
-        const float* Yd = pp.Yh + slot * hstride + row;
+        const float* Sd = hS + slot * sp.A_pad + lane;
+        const float* Yd = hY + slot * sp.A_pad + lane;
         float sv[NPL], yv[NPL], d = 0.f;
 #pragma unroll
         for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
@@ -232,8 +285,8 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
       for (int j = 0; j < NPL; ++j) q[j] *= gamma;
       for (int i = hc - 1; i >= 0; --i) {
         int slot = hh - 1 - i; if (slot < 0) slot += sp.m;
-        const float* Sd = pp.Sh + slot * hstride + row;
-        const float* Yd = pp.Yh + slot * hstride + row;
+        const float* Sd = hS + slot * sp.A_pad + lane;
+        const float* Yd = hY + slot * sp.A_pad + lane;
         float sv[NPL], yv[NPL], d = 0.f;
 #pragma unroll
         for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
@@ -272,11 +325,21 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     if (status == PLAN_RUNNING) atomicAdd(&pp.n_running[parity ^ 1], 1);
     else pp.status[k] = status;
   }
+  hist_wait();
 }
 
 template <int NPL>
 static void step_launch(const PlanDev& p, const StepParams& sp, int parity, float g_scale, cudaStream_t st) {
-  k_step<NPL><<<(p.K + 3) / 4, 128, 0, st>>>(sp, make_ptrs(p), parity, g_scale);
+  const size_t per_plan = (size_t)2 * sp.m * sp.A_pad * sizeof(float);     // <= 2 * 16 * 480 * 4 = 61 KB
+  int wpb = (int)((200u << 10) / per_plan);
+  if (wpb > 4) wpb = 4;
+  const size_t smem = per_plan * wpb;
+  static size_t allowed = 0;                                               // per instantiation
+  if (smem > allowed) {
+    if (cudaFuncSetAttribute(k_step<NPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(200u << 10)) != cudaSuccess) return;
+    allowed = 200u << 10;
+  }
+  k_step<NPL><<<(p.K + wpb - 1) / wpb, 32 * wpb, smem, st>>>(sp, make_ptrs(p), parity, g_scale, wpb);
 }
 
 int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
