@@ -31,6 +31,9 @@ sys.path.insert(0, str(ROOT))
 import gmco_cases as gc  # noqa: E402
 
 METRIC, UNIT = "plans_per_s", "plans/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_dose_tc + one k_grad_tc launch, from the ncu --set full
+# capture summarised in profiles/r1_ncu_full_summary.md (a constant copied from that file, not measured here)
+NCU_TRAFFIC_BYTES = {"C3": None}
 
 
 def env_int(name, default):
@@ -292,10 +295,11 @@ def roofline(case, prec, g, prof, peaks):
     if prec == g.GMCO_PREC_TF32X3:
         peak = peaks["bf16_sustained"] * (1.1 / 2.25)
         issued = 3.0 * flops / (ms * 1e-3) / 1e12
-        return {"bound": "tensor", "kernel": "k_fused_tc (dose GEMM + penalty + gradient GEMM)",
+        return {"bound": "tensor", "kernel": "k_dose_tc + k_grad_tc (the two contractions of one round, timed as a pair)",
                 "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
                 "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["eval_launches"],
-                "peak_source": f"{peaks['source']} bf16 sustained x 1.1/2.25 (nominal tf32:bf16)", "traffic": None}
+                "peak_source": f"{peaks['source']} bf16 sustained x 1.1/2.25 (nominal tf32:bf16)",
+                "traffic": NCU_TRAFFIC_BYTES.get(case.name)}
     peak = 148 * 128 * 2 * 1.965e9 / 1e12
     ach = flops / (ms * 1e-3) / 1e12
     return {"bound": "alu", "kernel": "k_simt_dose + k_simt_grad", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
