@@ -139,6 +139,22 @@ def run_reference(args, case):
     }))
 
 
+def max_over_ranks_ms(ms: float, world: int, device) -> float:
+    """The slowest rank's time: one all-reduce(MAX) of a scalar, outside every timed region."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(plans_per_rank: int, world: int, steps: int, ms_max: float) -> float:
+    """Whole-job plans/s: every rank optimises its own pool (weak scaling), time = max over ranks."""
+    return world * plans_per_rank * steps / (ms_max * 1e-3)
+
+
 def workload_config(case, args, stats):
     cfg = {"workload": f"{case.name}: BASELINE.json configs[{['C1','C2','C3','C4'].index(case.name)}]",
            "n_points": case.n_points, "n_dwell": case.n_dwell, "plans_per_gpu": case.n_plans, "m": case.m,
@@ -229,11 +245,7 @@ def main():
         torch.cuda.synchronize()
 
     def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return max_over_ranks_ms(ms, world, "cuda")
 
     for _ in range(args.warmup):
         step(False); step(True)
@@ -253,8 +265,8 @@ def main():
         prof = dict(last["stats"])
     barrier()
 
-    value = world * K * args.steps / (ms_dev * 1e-3)
-    e2e_value = world * K * args.steps / (ms_e2e * 1e-3)
+    value = job_value(K, world, args.steps, ms_dev)
+    e2e_value = job_value(K, world, args.steps, ms_e2e)
     h2d = case.D.nbytes + case.T0.nbytes + case.weights.nbytes
     d2h = sum(v.numel() * v.element_size() for v in out_pin.values())
 

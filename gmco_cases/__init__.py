@@ -238,3 +238,13 @@ def shard_plans(n_plans: int, world_size: int, rank: int) -> tuple[int, int]:
     base, rem = divmod(n_plans, world_size)
     begin = rank * base + min(rank, rem)
     return begin, begin + base + (1 if rank < rem else 0)
+
+
+def sa_draws(n_dwell: int, n_chains: int, steps: int, seed: int):
+    """Random draws of the gSA chains (BASELINE.json configs[4]): the dwell index,
+    a standard normal and a uniform per (chain, step).  Inputs of BOTH sides; no method arithmetic."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    jdx = rng.integers(0, n_dwell, size=(n_chains, steps), dtype=np.int32)
+    z = rng.standard_normal(size=(n_chains, steps))
+    u = rng.random(size=(n_chains, steps))
+    return jdx, z, u

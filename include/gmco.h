@@ -40,7 +40,7 @@ extern "C" {
 #define GMCO_API
 #endif
 
-#define GMCO_VERSION 100          /* 0.1.0 */
+#define GMCO_VERSION 110          /* 0.1.1 */
 #define GMCO_MAX_STRUCTS 8
 #define GMCO_MAX_HISTORY 16
 
@@ -59,6 +59,12 @@ typedef enum gmco_precision {
                                384 dwell positions do not fit the tensor layout and run as SIMT_FP32  */
   GMCO_PREC_SIMT_FP32 = 1   /* plain fp32 FMA kernels (reference datum and debug route)            */
 } gmco_precision;
+
+/* Arithmetic of gmco_sa_run. */
+typedef enum gmco_sa_precision {
+  GMCO_SA_FP64 = 0,         /* dose, penalty differences and the accept test in fp64: the parity route   */
+  GMCO_SA_FP32 = 1          /* everything in fp32: the speed route                                       */
+} gmco_sa_precision;
 
 /* Per-plan exit status written by gmco_result. */
 typedef enum gmco_plan_status {
@@ -143,6 +149,27 @@ GMCO_API int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh,
  * synchronises only if an output is a host pointer.  Discards any optimisation state. */
 GMCO_API int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const float* weights,
                   int32_t K, float* dose, float* F, float* grad_x, void* cuda_stream);
+
+/* gSA -- K simulated-annealing chains on the case of `h`, the comparison method of the paper
+ * (PAPER.md:96-113 steps (ii)-(v); move / cooling / acceptance rule from
+ * BASELINE.json configs[4]).  Chain k starts at T0 and, at step n = 0..steps-1,
+ *   j = jdx[n];  sigma = max(0.1 t_j, 0.01 tau);  t' = max(t_j + sigma z[n], 0);
+ *   d' = d + (t' - t_j) D[:, j]  (incremental Eq. 1);  dF = F(d') - F(d)  (Eqs. 2, 4);
+ *   accept if dF <= 0, else if u[n] < exp(-dF / T_n),  T_n = temp0 * exp(n ln cooling).
+ * The random draws are INPUTS (the library owns no generator): jdx int32 in [0, n_dwell),
+ * z ~ N(0,1) and u ~ U[0,1) as fp64, each [K][steps] or, if draws_broadcast != 0, [steps] shared
+ * by all chains (host or device).  T0 / weights as in gmco_optimize.  tau: the scale of the move
+ * floor in seconds (>= 0).  precision: gmco_sa_precision.
+ * Outputs (host or device, any may be NULL): T [K][n_dwell] fp64 seconds; objective [K] fp64, summed
+ * afresh from the final dose; n_accepted [K] int64 accepted moves (dF = 0 counts as accepted).
+ * Enqueues on cuda_stream and synchronises it before returning.  Does not touch the state of
+ * gmco_optimize / gmco_result.  GMCO_E_UNSUPPORTED if the chain state does not fit one CTA
+ * (more than 12800 padded points in fp64, 25600 in fp32); GMCO_E_INVALID for an index outside
+ * [0, n_dwell) or negative / non-finite T0, weights. */
+GMCO_API int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, const float* weights, int32_t K,
+                int64_t steps, const int32_t* jdx, const double* z, const double* u, int32_t draws_broadcast,
+                double tau, double temp0, double cooling, int32_t precision, double* T, double* objective,
+                int64_t* n_accepted, void* cuda_stream);
 
 /* Counters of the last optimise/result pair.  GMCO_E_STATE before the first gmco_result. */
 GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);

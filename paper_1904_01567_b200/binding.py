@@ -9,6 +9,7 @@ import numpy as np
 _PKG = Path(__file__).resolve().parent
 GMCO_PREC_TF32X3, GMCO_PREC_SIMT_FP32 = 0, 1
 GMCO_MAX_STRUCTS = 8
+GMCO_SA_FP64, GMCO_SA_FP32 = 0, 1
 
 
 class GmcoError(RuntimeError):
@@ -59,6 +60,8 @@ def lib():
         L.gmco_optimize.argtypes = [vp, fp, i32, fp, i32, i32, vp]
         L.gmco_result.argtypes = [vp, fp, fp, fp, fp, vp, vp]
         L.gmco_evaluate.argtypes = [vp, fp, i32, fp, i32, fp, fp, fp, vp]
+        L.gmco_sa_run.argtypes = [vp, fp, i32, fp, i32, i64, vp, vp, vp, i32, C.c_double, C.c_double, C.c_double,
+                                  i32, vp, vp, vp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gmco_set_profiling.argtypes = [vp, i32]
         L.gmco_destroy.argtypes = [vp]
@@ -186,6 +189,36 @@ def gmco_evaluate(h: Handle, T, weights, want_dose=False, want_grad=True, host: 
     h.K = K
     _check(lib().gmco_evaluate(h.ptr, _ptr(T), bc, _ptr(weights), K, _ptr(dose), _ptr(F), _ptr(g), _stream(stream)), h)
     return dict(dose=dose, F=F, grad_x=g)
+
+
+def gmco_sa_run(h: Handle, T0, weights, jdx, z, u, tau: float, temp0: float = 1.0, cooling: float = 0.995,
+                precision: int = GMCO_SA_FP64, host: bool = False, stream=None) -> dict:
+    """K simulated-annealing chains (include/gmco.h gmco_sa_run).  jdx int32, z / u fp64, each [K][steps] or [steps]
+    (shared by all chains).  Returns dict(T [K][A] fp64, objective [K] fp64, n_accepted [K] int64)."""
+    T0, weights = _f32(T0), _f32(weights)
+    K = int(weights.shape[0])
+    bc = 1 if T0.ndim == 1 else 0
+    if isinstance(jdx, np.ndarray):
+        jdx = np.ascontiguousarray(jdx, dtype=np.int32)
+        z = np.ascontiguousarray(z, dtype=np.float64); u = np.ascontiguousarray(u, dtype=np.float64)
+    else:
+        import torch
+        jdx = jdx.to(torch.int32).contiguous(); z = z.to(torch.float64).contiguous(); u = u.to(torch.float64).contiguous()
+    dbc = 1 if jdx.ndim == 1 else 0
+    steps = int(jdx.shape[-1])
+    assert tuple(z.shape) == tuple(jdx.shape) == tuple(u.shape) and (dbc or int(jdx.shape[0]) == K)
+    A = h.n_dwell
+    if host:
+        T = np.empty((K, A), np.float64); F = np.empty(K, np.float64); na = np.empty(K, np.int64)
+    else:
+        import torch
+        dev = torch.device("cuda")
+        T = torch.empty((K, A), dtype=torch.float64, device=dev); F = torch.empty(K, dtype=torch.float64, device=dev)
+        na = torch.empty(K, dtype=torch.int64, device=dev)
+    _check(lib().gmco_sa_run(h.ptr, _ptr(T0), bc, _ptr(weights), K, steps, _ptr(jdx), _ptr(z), _ptr(u), dbc,
+                             float(tau), float(temp0), float(cooling), int(precision), _ptr(T), _ptr(F), _ptr(na),
+                             _stream(stream)), h)
+    return dict(T=T, objective=F, n_accepted=na)
 
 
 def gmco_get_stats(h: Handle) -> dict:

@@ -46,6 +46,7 @@ struct gmco_handle {
   int *out_iters = nullptr, *out_status = nullptr;
   int host_flags[4] = {0, 0, 0, 0};  // pageable: the copies into it are followed by a stream synchronise
   TcPlan* tc = nullptr;
+  float* sa_Dt = nullptr;            // gSA: transposed copy of D [A][N_alloc], built by the first gmco_sa_run
   // device-driven round loop: a CUDA graph whose only node is a WHILE conditional; its body is two rounds
   // (parity 0, parity 1) and a kernel that keeps the loop going while a plan is still running
   cudaGraph_t loop_graph = nullptr;
@@ -483,6 +484,7 @@ void gmco_destroy(gmco_handle* h) {
   if (h->tc) tc_plan_destroy(h->tc);
   destroy_loop_graph(h);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->sa_Dt) cudaFreeAsync(h->sa_Dt, h->stream);
   arena_free(h->plan_arena, h->stream);
   arena_free(h->case_arena, h->stream);
   delete h;
@@ -635,6 +637,85 @@ int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const flo
     CK(h, cudaStreamSynchronize(st));
     if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T or weights hold a negative, NaN or infinite value%s");
   }
+  return GMCO_OK;
+}
+
+int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, const float* weights, int32_t K, int64_t steps,
+                const int32_t* jdx, const double* z, const double* u, int32_t draws_broadcast, double tau,
+                double temp0, double cooling, int32_t precision, double* T, double* objective, int64_t* n_accepted,
+                void* cuda_stream) {
+  if (!h) return GMCO_E_INVALID;
+  if (K < 0 || steps < 0) return fail(h, GMCO_E_INVALID, "K and steps must be >= 0%s");
+  if (K == 0) return GMCO_OK;
+  if (!T0 || !weights) return fail(h, GMCO_E_INVALID, "T0 or weights is NULL%s");
+  if (steps > 0 && (!jdx || !z || !u)) return fail(h, GMCO_E_INVALID, "jdx, z or u is NULL%s");
+  if (precision != GMCO_SA_FP64 && precision != GMCO_SA_FP32) return fail(h, GMCO_E_INVALID, "unknown gmco_sa_precision%s");
+  if (!(tau >= 0.0) || !(temp0 >= 0.0) || !(cooling > 0.0) || isinf(tau) || isinf(temp0) || isinf(cooling))
+    return fail(h, GMCO_E_INVALID, "tau, temp0 must be finite and >= 0, cooling finite and > 0%s");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const CaseDev& c = h->c;
+  const int ppt = sa_points_per_thread(c);
+  const size_t smem = sa_smem_bytes(c, precision, ppt);
+  if (smem > 227 * 1024) return fail(h, GMCO_E_UNSUPPORTED, "gSA: the case has too many points for one CTA's shared memory%s");
+  h->launches = 0;
+  if (!h->sa_Dt) {
+    CK(h, cudaMallocAsync(reinterpret_cast<void**>(&h->sa_Dt), (size_t)c.A * c.N_alloc * sizeof(float), st));
+    LN(h, launch_sa_transpose(c, h->sa_Dt, st));
+  }
+  // one stream-ordered block for this call: staged host inputs and the outputs
+  const size_t nd = (size_t)(draws_broadcast ? 1 : K) * (size_t)steps;
+  const size_t nT0 = (size_t)(t0_broadcast ? 1 : K) * c.A, nw = (size_t)K * 2 * c.S;
+  const bool T0_host = !is_device_ptr(T0), w_host = !is_device_ptr(weights);
+  const bool j_host = steps > 0 && !is_device_ptr(jdx), z_host = steps > 0 && !is_device_ptr(z),
+             u_host = steps > 0 && !is_device_ptr(u);
+  Arena a;
+  char* blk = nullptr;
+  double *dT = nullptr, *dF = nullptr, *dFt = nullptr, *dz = nullptr, *du = nullptr;
+  long long* dn = nullptr; int *dbad = nullptr, *dj = nullptr; float *dT0 = nullptr, *dw = nullptr;
+  for (int pass = 0; pass < 2; ++pass) {
+    a.base = blk; a.used = 0;
+    dT = a.take<double>((size_t)K * c.A); dF = a.take<double>(K); dFt = a.take<double>(K);
+    dn = a.take<long long>(K); dbad = a.take<int>(1);
+    if (z_host) dz = a.take<double>(nd);
+    if (u_host) du = a.take<double>(nd);
+    if (j_host) dj = a.take<int>(nd);
+    if (T0_host) dT0 = a.take<float>(nT0);
+    if (w_host) dw = a.take<float>(nw);
+    if (pass == 0) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&blk), a.used, st));
+  }
+  int rc = GMCO_OK;
+  auto body = [&]() -> int {
+    CK(h, cudaMemsetAsync(dbad, 0, sizeof(int), st));
+    if (z_host) CK(h, cudaMemcpyAsync(dz, z, nd * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (u_host) CK(h, cudaMemcpyAsync(du, u, nd * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (j_host) CK(h, cudaMemcpyAsync(dj, jdx, nd * sizeof(int), cudaMemcpyHostToDevice, st));
+    if (T0_host) CK(h, cudaMemcpyAsync(dT0, T0, nT0 * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (w_host) CK(h, cudaMemcpyAsync(dw, weights, nw * sizeof(float), cudaMemcpyHostToDevice, st));
+    SaArgs sa{};
+    sa.Dt = h->sa_Dt; sa.ldt = c.N_alloc; sa.pt_lo = c.pt_lo; sa.pt_hi = c.pt_hi; sa.tile_struct = c.tile_struct;
+    sa.N_pad = c.N_pad; sa.A = c.A; sa.A_pad = c.A_pad; sa.S = c.S;
+    for (int s = 0; s < c.S; ++s) {
+      sa.wscale[2 * s] = (double)h->sh[s].w_lo / (double)h->sh[s].n_points;
+      sa.wscale[2 * s + 1] = (double)h->sh[s].w_hi / (double)h->sh[s].n_points;
+    }
+    sa.T0 = T0_host ? dT0 : T0; sa.t0_bcast = t0_broadcast ? 1 : 0; sa.w_user = w_host ? dw : weights;
+    sa.steps = steps; sa.jdx = j_host ? dj : jdx; sa.z = z_host ? dz : z; sa.u = u_host ? du : u;
+    sa.draws_bcast = draws_broadcast ? 1 : 0;
+    sa.tau = tau; sa.temp0 = temp0; sa.log_cooling = log(cooling);
+    sa.T_out = dT; sa.F_out = dF; sa.F_tracked = dFt; sa.n_accepted = dn; sa.bad_input = dbad;
+    LN(h, launch_sa_chains(c, sa, K, precision, st));
+    if (T) CK(h, cudaMemcpyAsync(T, dT, (size_t)K * c.A * sizeof(double), cudaMemcpyDefault, st));
+    if (objective) CK(h, cudaMemcpyAsync(objective, dF, (size_t)K * sizeof(double), cudaMemcpyDefault, st));
+    if (n_accepted) CK(h, cudaMemcpyAsync(n_accepted, dn, (size_t)K * sizeof(long long), cudaMemcpyDefault, st));
+    CK(h, cudaMemcpyAsync(h->host_flags + 2, dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    return GMCO_OK;
+  };
+  rc = body();
+  cudaFreeAsync(blk, st);
+  if (rc) return rc;
+  CK(h, cudaStreamSynchronize(st));
+  if (h->host_flags[2] & 1) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
+  if (h->host_flags[2] & 2) return fail(h, GMCO_E_INVALID, "jdx holds an index outside [0, n_dwell)%s");
   return GMCO_OK;
 }
 

@@ -102,6 +102,24 @@ int launch_result(const CaseDev& c, const PlanDev& p, const StructHost* sh, floa
                   float* dvh_out, float* terms_out, int* iters_out, int* status_out, cudaStream_t st);
 int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st);
 
+// gSA (kernels_sa.cu): one CTA of kSaThreads per chain, draws staged kSaBlock steps at a time
+constexpr int kSaThreads = 512;
+constexpr int kSaBlock = 128;
+struct SaArgs {
+  const float* Dt; long long ldt;             // transposed dose-rate matrix [A][ldt], ldt = N_alloc
+  const float *pt_lo, *pt_hi; const int* tile_struct;
+  int N_pad, A, A_pad, S;
+  double wscale[2 * GMCO_MAX_STRUCTS];        // base weight / n_points per (structure, side), fp64
+  const float* T0; int t0_bcast; const float* w_user;
+  long long steps; const int* jdx; const double *z, *u; int draws_bcast;
+  double tau, temp0, log_cooling;
+  double *T_out, *F_out, *F_tracked; long long* n_accepted; int* bad_input;
+};
+int launch_sa_transpose(const CaseDev& c, float* Dt, cudaStream_t st);
+size_t sa_smem_bytes(const CaseDev& c, int precision, int ppt);
+int sa_points_per_thread(const CaseDev& c);
+int launch_sa_chains(const CaseDev& c, const SaArgs& a, int K, int precision, cudaStream_t st);
+
 // tensor path (kernel_fused_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,

@@ -5,6 +5,7 @@
 // route that can hand dose to the caller (gmco_evaluate's debug output).  The production
 // contraction is the tcgen05 kernel in kernel_fused_tc.cu.
 #include "gmco_internal.cuh"
+#include "penalty.cuh"
 
 namespace gmco {
 
@@ -103,11 +104,7 @@ k_simt_dose(const float* __restrict__ D, const float* __restrict__ T, int A_pad,
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       const float d = acc[i][j];
-      const float lo = fminf(d - dl, 0.f), hi = fmaxf(d - dh, 0.f);
-      const float u = wlo[j] * lo, v = whi[j] * hi;
-      flo[j] = fmaf(u, lo, flo[j]);
-      fhi[j] = fmaf(v, hi, fhi[j]);
-      rv[i][j] = 2.f * (u + v);
+      rv[i][j] = 2.f * eq2_accumulate<float>(d, dl, dh, wlo[j], whi[j], flo[j], fhi[j]);
     }
     const int src = row_src[pr];
     if (dose_out && src >= 0) {

@@ -25,6 +25,7 @@
 #include <vector>
 
 #include "gmco_internal.cuh"
+#include "penalty.cuh"
 
 namespace gmco {
 
@@ -380,19 +381,15 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             const float d = __uint_as_float(v[j]);
-            const float lo = fminf(d - dlo, 0.f), hi = fmaxf(d - dhi, 0.f);
-            const float u = wlo * lo, w = whi * hi;
-            f_lo = fmaf(u, lo, f_lo); f_hi = fmaf(w, hi, f_hi);
-            rp[(size_t)j * a.K_pad] = u + w;                              // = dF/dd / 2
+            rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, f_lo, f_hi);  // = dF/dd / 2
           }
         } else {                                                          // ragged tail of a structure
 #pragma unroll
           for (int j = 0; j < 32; ++j) {
             const float d = __uint_as_float(v[j]);
-            const float lo = fminf(d - dlo, 0.f), hi = fmaxf(d - dhi, 0.f);
-            const float u = wlo * lo, w = whi * hi;
-            if (j < nvh) { f_lo = fmaf(u, lo, f_lo); f_hi = fmaf(w, hi, f_hi); }
-            rp[(size_t)j * a.K_pad] = u + w;                              // padding rows of D are zero: value unused
+            float t_lo = f_lo, t_hi = f_hi;
+            rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, t_lo, t_hi);  // padding rows: value unused
+            if (j < nvh) { f_lo = t_lo; f_hi = t_hi; }
           }
         }
         if (a.dose_dbg && plan < a.K) {
