@@ -20,6 +20,7 @@
 // warps 2-5 = epilogue (TMEM lane quadrant = warp_id % 4).  Pipelines are mbarrier rings.
 #include <cudaTypedefs.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -31,8 +32,10 @@ namespace gmco {
 
 namespace {
 
-constexpr int kPC = 64;                 // points per dose chunk (= MMA N of the dose contraction)
-constexpr int kSlabBytes = kPC * 128;   // one 32-dwell slab of a dose chunk, one part: 8 KB
+// Points per dose chunk = MMA N of the dose contraction.  128, not 64: a kind::tf32 M=128 K=8 MMA costs
+// max(~60, N/2) cycles on sm_100 (measured, profiles/r1_mma_rate.md), so N=64 runs the tensor pipe at half rate.
+constexpr int kPC = 128;
+constexpr int kSlabBytes = kPC * 128;   // one 32-dwell slab of a dose chunk, one part (hi or lo): 16 KB
 constexpr int kTloBox = 128 * 128;      // T_lo: 128 plans x 32 dwell: 16 KB
 constexpr int kThreads = 192;
 constexpr uint32_t kWatchdog = 1u << 26;
@@ -68,6 +71,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (++spins > kWatchdog) __trap();
   }
 }
+// the same on a shared-memory address that is already a 32-bit value
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity) {
+  uint32_t spins = 0, ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok && ++spins > kWatchdog) __trap();
+  } while (!ok);
+}
 // one lane of a fully converged warp; the compiler keeps everything around it on the uniform datapath
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
@@ -76,10 +89,22 @@ __device__ __forceinline__ bool elect_one() {
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
-__device__ __forceinline__ void tma_load_3d(const CUtensorMap* map, void* dst, uint64_t* bar, int c0, int c1, int c2) {
+// L2 eviction policies for the TMA streams: the dose-rate matrix is the operand every CTA and every
+// round re-reads and must stay in L2; R is dead once the gradient kernel has read it.
+__device__ __forceinline__ uint64_t l2_evict_last() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t l2_evict_first() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t l2_evict_normal() {
+  uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ void tma_load_3d(const CUtensorMap* map, void* dst, uint64_t* bar, int c0, int c1, int c2,
+                                            uint64_t policy) {
   asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;"
+      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
       : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
@@ -99,6 +124,9 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
 __device__ __forceinline__ void tc_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tc_commit_addr(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
 // D[tmem] (+)= A[smem] . B[smem]
 __device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
   asm volatile(
@@ -108,13 +136,29 @@ __device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_
       : "memory");
 }
 // D[tmem] (+)= A[tmem] . B[smem]
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
+
+// Lean forms for the issue loops: a shared-memory descriptor is passed as its two 32-bit halves.  Only the low half
+// (start address, 16 B units) changes from one MMA to the next, so the issuing warp does 32-bit adds on the uniform
+// datapath instead of rebuilding 64-bit descriptors (the issue loop, not the tensor pipe, was the bottleneck).
+__device__ __forceinline__ void mma_ts2(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc,
+                                        uint32_t acc) {
   asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc)
+      "{\n\t.reg .pred p;\n\t.reg .b64 bd;\n\tsetp.ne.b32 p, %5, 0;\n\tmov.b64 bd, {%2, %3};\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], bd, %4, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc)
       : "memory");
 }
+__device__ __forceinline__ void mma_ss2(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                        uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 ad, bd;\n\tsetp.ne.b32 p, %6, 0;\n\tmov.b64 ad, {%1, %2};\n\tmov.b64 bd, {%3, %4};\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], ad, bd, %5, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// the two halves of smem_desc(): lo = start address | LBO, hi = SBO | version | layout
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) { return ((saddr >> 4) & 0x3fff) | ((lbo_bytes >> 4) << 16); }
+__host__ __device__ constexpr uint32_t desc_hi(uint32_t sbo_bytes, uint32_t layout) { return (sbo_bytes >> 4) | (1u << 14) | (layout << 29); }
 
 #define GMCO_R32(v, o)                                                                                           \
   "=r"(v[o + 0]), "=r"(v[o + 1]), "=r"(v[o + 2]), "=r"(v[o + 3]), "=r"(v[o + 4]), "=r"(v[o + 5]), "=r"(v[o + 6]), \
@@ -199,7 +243,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // ---------------------------------------------------------------------------------------------
 // a2-a4 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point chunks [seg n_chunks / segs, (seg + 1) n_chunks / segs).
-// Shared memory: [T_lo resident: G x 16 KB]? | ring n_stage x (D_hi 8 KB | D_lo 8 KB | [T_lo slab 16 KB]?) | barriers.
+// Shared memory: [T_lo resident: G x 16 KB]? | ring of n_stage entries | barriers.  Ring entries alternate between
+// the D_hi slab and the D_lo slab of one (chunk, 32-dwell group): 16 KB each, so the ring is deep in entries although
+// a chunk is 128 points wide; when T_lo is streamed, its 16 KB slab rides behind the D_hi slab of its group.
 // The last kScratchBytes of the ring double as the T_hi transposition scratch of the prologue.
 __global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
@@ -208,7 +254,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
-  const int stageBytes = a.tlo_resident ? 2 * kSlabBytes : 2 * kSlabBytes + kTloBox;
+  const int stageBytes = a.tlo_resident ? kSlabBytes : kSlabBytes + kTloBox;
   uint8_t* tlo = smem;                              // [G][128 plans][128 B] when resident
   uint8_t* ring = smem + (a.tlo_resident ? (size_t)G * kTloBox : 0);
   const int ringBytes = a.n_stage * stageBytes;
@@ -241,9 +287,9 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   tc_fence_after();
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
   const uint32_t t_thi = tmem;                      // columns [0, A_pad): T_hi
-  // columns [A_pad, A_pad + 128 n_acc): per buffer a MAIN accumulator (T_hi D_hi) and a CORRECTION accumulator
-  // (T_hi D_lo + T_lo D_hi).  The tensor core truncates when it adds into the fp32 accumulator; keeping the small
-  // products out of the large sum cuts that bias by 3x.
+  // columns [A_pad, A_pad + 128 n_acc): one 128-point accumulator per buffer; the three products of the split
+  // accumulate into it in ring order (the tensor core truncates when it adds into the fp32 accumulator: measured
+  // dose error stays below 1e-5 relative).
   const uint32_t t_acc = tmem + a.A_pad;
 
   if (warp == 0) {
@@ -252,22 +298,24 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
       if (a.tlo_resident) {
         if (elect_one()) {
           mbar_expect_tx(tlo_full, (uint32_t)G * kTloBox);
-          for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g);
+          for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g, l2_evict_normal());
         }
         __syncwarp();
       }
+      const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
       int st = 0; uint32_t ph = 0;
       bool scratch_busy = true;
       for (int c = c0; c < c1; ++c) {
-        for (int g = 0; g < G; ++g) {
+        for (int g2 = 0; g2 < 2 * G; ++g2) {          // entry 2 g: D_hi (+ streamed T_lo), entry 2 g + 1: D_lo
+          const int g = g2 >> 1, lo = g2 & 1;
           if (scratch_busy && st >= scr_slot) { mbar_wait(thi_ready, 0); scratch_busy = false; }
           mbar_wait(empty + st, ph ^ 1);
           if (elect_one()) {
             uint8_t* dst = ring + (size_t)st * stageBytes;
-            mbar_expect_tx(full + st, (uint32_t)stageBytes);
-            tma_load_3d(&tmD_hi, dst, full + st, 0, c * kPC, g);
-            tma_load_3d(&tmD_lo, dst + kSlabBytes, full + st, 0, c * kPC, g);
-            if (!a.tlo_resident) tma_load_3d(&tmT_lo, dst + 2 * kSlabBytes, full + st, 0, tile * 128, g);
+            const bool with_t = !lo && !a.tlo_resident;
+            mbar_expect_tx(full + st, (uint32_t)(with_t ? kSlabBytes + kTloBox : kSlabBytes));
+            tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, c * kPC, g, polD);
+            if (with_t) tma_load_3d(&tmT_lo, dst + kSlabBytes, full + st, 0, tile * 128, g, polT);
           }
           __syncwarp();
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
@@ -276,36 +324,52 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
     }
   } else if (warp == 1) {
     if (c1 > c0) {
+      // Issue loop.  Everything is warp-uniform (uniform datapath); one elected lane issues.  Per ring entry: one wait, 8 or 4
+      // MMAs whose descriptors differ by 32-bit adds, one commit.
       constexpr uint32_t idesc = instr_desc(kPC, 0, 0);
+      constexpr uint32_t dhi = desc_hi(1024, kSwz128);
+      const int n_stage = a.n_stage, n_acc = a.n_acc;
+      const uint32_t ring_lo = desc_lo(smem_u32(ring), 16), ring_step = (uint32_t)stageBytes >> 4;
+      const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
+      const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
       if (a.tlo_resident) mbar_wait(tlo_full, 0);
       mbar_wait(thi_ready, 0);
       tc_fence_after();
       int st = 0; uint32_t ph = 0;
       for (int c = c0; c < c1; ++c) {
-        const int b = a.n_acc == 2 ? (c - c0) & 1 : 0, use = a.n_acc == 2 ? (c - c0) >> 1 : c - c0;
+        const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
         mbar_wait(acc_empty + b, (use & 1) ^ 1);
         tc_fence_after();
-        const uint32_t acc = t_acc + b * 2 * kPC, acc_c = acc + kPC;
-        for (int g = 0; g < G; ++g) {
-          mbar_wait(full + st, ph);
-          tc_fence_after();
+        const uint32_t acc = t_acc + b * kPC;
+        uint32_t thi = t_thi, alo = tlo_lo0;
+        for (int g = 0; g < G; ++g, thi += 32, alo += kTloBox >> 4) {
+          // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
+          mbar_wait_addr(full0 + 8 * st, ph);
           if (elect_one()) {
-            const uint32_t s_hi = smem_u32(ring + (size_t)st * stageBytes);
-            const uint64_t d_hi = smem_desc(s_hi, 16, 1024, kSwz128), d_lo = smem_desc(s_hi + kSlabBytes, 16, 1024, kSwz128);
-            const uint64_t a_lo = smem_desc(a.tlo_resident ? smem_u32(tlo + (size_t)g * kTloBox) : s_hi + 2 * kSlabBytes,
-                                            16, 1024, kSwz128);
+            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+            const uint32_t ad = a.tlo_resident ? alo : bd + (kSlabBytes >> 4);
+            mma_ts2(acc, thi, bd, dhi, idesc, g != 0);
+            mma_ss2(acc, ad, dhi, bd, dhi, idesc, 1);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {           // 4 K-steps of 8 dwell positions: +32 B inside the swizzled row
-              const uint32_t a_hi = t_thi + g * 32 + j * 8;
-              mma_ts(acc, a_hi, d_hi + 2 * j, idesc, (g | j) != 0);
-              mma_ts(acc_c, a_hi, d_lo + 2 * j, idesc, (g | j) != 0);
-              mma_ss(acc_c, a_lo + 2 * j, d_hi + 2 * j, idesc, 1);
+            for (int j = 1; j < 4; ++j) {           // K-steps of 8 dwell positions: +32 B inside the swizzled row
+              mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+              mma_ss2(acc, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
             }
-            tc_commit(empty + st);
+            tc_commit_addr(empty0 + 8 * st);
+          }
+          __syncwarp();
+          if (++st == n_stage) { st = 0; ph ^= 1; }
+          // entry 2 g + 1: D_lo slab: T_hi D_lo
+          mbar_wait_addr(full0 + 8 * st, ph);
+          if (elect_one()) {
+            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+            tc_commit_addr(empty0 + 8 * st);
             if (g == G - 1) tc_commit(acc_full + b);
           }
           __syncwarp();
-          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+          if (++st == n_stage) { st = 0; ph ^= 1; }
         }
       }
     }
@@ -350,51 +414,51 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         mbar_arrive(thi_ready);
       }
 
-      // structure id, valid rows and weights of the NEXT chunk are fetched one chunk ahead
-      int s_n = a.tile_struct[c0], nv_n = a.tile_valid[c0];
+      // This warp evaluates the 64-row tile 2 c + h of chunk c (one structure per 64-row tile by construction).
+      // Structure id, valid rows and weights of the NEXT chunk are fetched one chunk ahead.
+      int s_n = a.tile_struct[2 * c0 + h], nv_n = a.tile_valid[2 * c0 + h];
       float wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n], whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
       for (int c = c0; c < c1; ++c) {
         const int b = a.n_acc == 2 ? (c - c0) & 1 : 0, use = a.n_acc == 2 ? (c - c0) >> 1 : c - c0;
-        const int s = s_n, nvh = nv_n - h * 32;
+        const int s = s_n, nv = nv_n;
         const float wlo = wlo_n, whi = whi_n;
         if (c + 1 < c1) {
-          s_n = a.tile_struct[c + 1]; nv_n = a.tile_valid[c + 1];
+          s_n = a.tile_struct[2 * (c + 1) + h]; nv_n = a.tile_valid[2 * (c + 1) + h];
           wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n]; whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
         }
         const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
         mbar_wait(acc_full + b, use & 1);
         tc_fence_after();
-        uint32_t v[32];
-        {
-          uint32_t vc[32];
-          tmem_ld32(t_acc + lane_base + b * 2 * kPC + h * 32, v);
-          tmem_ld32(t_acc + lane_base + b * 2 * kPC + kPC + h * 32, vc);
-          tmem_ld_wait();
-          tc_fence_before();
-          mbar_arrive(acc_empty + b);
+        uint32_t v[2][32];
+        tmem_ld32(t_acc + lane_base + b * kPC + h * 64, v[0]);
+        tmem_ld32(t_acc + lane_base + b * kPC + h * 64 + 32, v[1]);
+        tmem_ld_wait();
+        tc_fence_before();
+        mbar_arrive(acc_empty + b);
 #pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
-        }
-        const size_t p0 = (size_t)c * kPC + h * 32;
-        float* rp = a.R + p0 * a.K_pad + plan;
-        if (nvh >= 32) {
+        for (int sub = 0; sub < 2; ++sub) {
+          const int nvh = nv - sub * 32;
+          const size_t p0 = (size_t)c * kPC + h * 64 + sub * 32;
+          float* rp = a.R + p0 * a.K_pad + plan;
+          if (nvh >= 32) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float d = __uint_as_float(v[j]);
-            rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, f_lo, f_hi);  // = dF/dd / 2
+            for (int j = 0; j < 32; ++j) {
+              const float d = __uint_as_float(v[sub][j]);
+              rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, f_lo, f_hi);  // = dF/dd / 2
+            }
+          } else {                                                          // ragged tail of a structure
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const float d = __uint_as_float(v[sub][j]);
+              float t_lo = f_lo, t_hi = f_hi;
+              rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, t_lo, t_hi);  // padding rows: value unused
+              if (j < nvh) { f_lo = t_lo; f_hi = t_hi; }
+            }
           }
-        } else {                                                          // ragged tail of a structure
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float d = __uint_as_float(v[j]);
-            float t_lo = f_lo, t_hi = f_hi;
-            rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, t_lo, t_hi);  // padding rows: value unused
-            if (j < nvh) { f_lo = t_lo; f_hi = t_hi; }
-          }
-        }
-        if (a.dose_dbg && plan < a.K) {
-          for (int j = 0; j < 32; ++j) {
-            if (j < nvh) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[j]);
+          if (a.dose_dbg && plan < a.K) {
+            for (int j = 0; j < 32; ++j) {
+              if (j < nvh) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[sub][j]);
+            }
           }
         }
       }
@@ -446,15 +510,16 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
 
   if (warp == 0) {
+    const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
     int st = 0; uint32_t ph = 0;
     for (int s = s0; s < s1; ++s) {
       mbar_wait(empty + st, ph ^ 1);
       if (elect_one()) {
         uint8_t* dst = smem + (size_t)st * stageBytes;
         mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
-        tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4);
-        tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0);
-        tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0);
+        tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
+        tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);
+        tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
       }
       __syncwarp();
       if (++st == a.n_stage) { st = 0; ph ^= 1; }
@@ -605,18 +670,19 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   const int G = c.A_pad / 32;
   // dose kernel: T_lo resident when it leaves room for >= 2 ring stages, else streamed with every D slab
   const int slack = 1024 /*alignment*/ + 512 /*barriers*/;
-  t->tlo_resident = G * kTloBox + 2 * 2 * kSlabBytes + slack <= kSmemMax ? 1 : 0;
+  t->tlo_resident = G * kTloBox + 4 * kSlabBytes + slack <= kSmemMax ? 1 : 0;
   const int fixed = (t->tlo_resident ? G * kTloBox : 0) + slack;
-  const int stageB = t->tlo_resident ? 2 * kSlabBytes : 2 * kSlabBytes + kTloBox;
+  const int stageB = t->tlo_resident ? kSlabBytes : kSlabBytes + kTloBox;
   t->dose_stages = (kSmemMax - fixed) / stageB;
-  if (t->dose_stages > 8) t->dose_stages = 8;
+  if (t->dose_stages > 12) t->dose_stages = 12;
   if (t->dose_stages * stageB < kScratchBytes) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
   t->dose_smem = fixed + t->dose_stages * stageB;
   // gradient kernel
   t->grad_ps = c.A_pad <= 256 ? 32 : 16;
+  if (const char* e = getenv("GMCO_GRAD_PS")) { const int v = atoi(e); if (v == 8 || v == 16 || v == 32) t->grad_ps = v; }
   const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
   t->grad_stages = (kSmemMax - 1024 - 512) / stage;
-  if (t->grad_stages > 6) t->grad_stages = 6;
+  if (t->grad_stages > 9) t->grad_stages = 9;
   if (t->grad_stages < 2) { snprintf(err, errlen, "shared memory too small for the gradient ring"); delete t; return nullptr; }
   t->grad_smem = 1024 + 512 + t->grad_stages * stage;
   const CUtensorMapSwizzle sK = CU_TENSOR_MAP_SWIZZLE_128B, sMN = CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
@@ -630,6 +696,7 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   cudaError_t e = cudaFuncSetAttribute(k_dose_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   std::vector<int> seg(t->n_tiles + 1);
   for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
   t->tile_seg_dev = p.tile_seg;                    // lives in the plan arena; pageable source: staged before the call returns
@@ -652,8 +719,8 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   DoseArgs da{};
   da.T_hi = p.T_hi; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
-  da.gate = gate; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = c.N_pad / kPC;
-  da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 4 * kPC <= 512 ? 2 : 1;
+  da.gate = gate; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
+  da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 2 * kPC <= 512 ? 2 : 1;
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
   k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
   if (cudaGetLastError() != cudaSuccess) return -1;
@@ -662,8 +729,10 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   ga.n_stage = t->grad_stages;
   if (t->grad_ps == 32)
     k_grad_tc<32><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
-  else
+  else if (t->grad_ps == 16)
     k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+  else
+    k_grad_tc<8><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
   return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 
