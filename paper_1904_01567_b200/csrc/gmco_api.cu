@@ -219,19 +219,21 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
 // SIMT kernels emit r = 2 w (d - D_lim) / n, the tensor kernel emits r / 2 (one multiply less per element)
 float g_scale_of(const gmco_handle* h) { return h->opt.precision == GMCO_PREC_SIMT_FP32 ? 2.f : 4.f; }
 
-int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, cudaStream_t st) {
+// zero_ctr / log_slot: start-of-round bookkeeping (reset the other parity's running-plan counter, log this round's).
+// The tensor route does it in its first kernel; the SIMT route launches k_round_begin.
+int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, int* zero_ctr, int* log_slot, cudaStream_t st) {
   if (h->opt.precision == GMCO_PREC_SIMT_FP32) {
+    if (zero_ctr) LN(h, launch_round_begin(zero_ctr, gate, log_slot, st));
     LN(h, launch_simt_eval(h->c, h->p, true, dose_dbg, false, nullptr, gate, st));
     LN(h, launch_simt_grad(h->c, h->p, gate, st));
   } else {
-    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, st));
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, st));
   }
   return GMCO_OK;
 }
 
 // one round: every running plan has its trial point evaluated, then accepted or its step halved
 int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const StepParams& sp, cudaStream_t st) {
-  LN(h, launch_round_begin(h->p, parity, log_idx, st));
   if (prof) {
     while ((int)h->ev.size() < h->ev_used + 2) {
       cudaEvent_t e;
@@ -240,7 +242,8 @@ int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const Step
     }
     CK(h, cudaEventRecord(h->ev[h->ev_used], st));
   }
-  int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, st);
+  int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, h->p.n_running + (parity ^ 1),
+                        log_idx < kRoundLogCap ? h->p.round_log + log_idx : nullptr, st);
   if (rc) return rc;
   if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
   LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
@@ -616,7 +619,7 @@ int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const flo
   float* dose_dev = dose;
   const bool dose_host = dose && !is_device_ptr(dose);
   if (dose_host) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dose_dev), (size_t)c.N * K * sizeof(float), st));
-  rc = enqueue_eval(h, dose_dev, nullptr, st);
+  rc = enqueue_eval(h, dose_dev, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   const StepParams sp = make_step_params(h, 0);
   float* Fd = F ? h->out_F : nullptr;
@@ -707,15 +710,15 @@ int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, const flo
     if (T) CK(h, cudaMemcpyAsync(T, dT, (size_t)K * c.A * sizeof(double), cudaMemcpyDefault, st));
     if (objective) CK(h, cudaMemcpyAsync(objective, dF, (size_t)K * sizeof(double), cudaMemcpyDefault, st));
     if (n_accepted) CK(h, cudaMemcpyAsync(n_accepted, dn, (size_t)K * sizeof(long long), cudaMemcpyDefault, st));
-    CK(h, cudaMemcpyAsync(h->host_flags + 2, dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(h, cudaMemcpyAsync(h->host_flags + 3, dbad, sizeof(int), cudaMemcpyDeviceToHost, st));
     return GMCO_OK;
   };
   rc = body();
   cudaFreeAsync(blk, st);
   if (rc) return rc;
   CK(h, cudaStreamSynchronize(st));
-  if (h->host_flags[2] & 1) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
-  if (h->host_flags[2] & 2) return fail(h, GMCO_E_INVALID, "jdx holds an index outside [0, n_dwell)%s");
+  if (h->host_flags[3] & 1) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
+  if (h->host_flags[3] & 2) return fail(h, GMCO_E_INVALID, "jdx holds an index outside [0, n_dwell)%s");
   return GMCO_OK;
 }
 

@@ -92,7 +92,7 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
 int launch_simt_eval(const CaseDev& c, const PlanDev& p, bool write_R, float* dose_out /*[N][K] or null*/,
                      bool dvh_mode, const float* dvh_thr /*[S] device*/, const int* gate, cudaStream_t st);
 int launch_simt_grad(const CaseDev& c, const PlanDev& p, const int* gate, cudaStream_t st);
-int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st);
+int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, cudaStream_t st);
 int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_rounds, cudaStream_t st);
 int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
                        cudaStream_t st);
@@ -128,6 +128,6 @@ void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 const int* tc_tile_seg_dev(const TcPlan*);
 int launch_tc_eval(const TcPlan* tp, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   cudaStream_t st);
+                   int* zero_ctr, int* log_slot, cudaStream_t st);
 
 }  // namespace gmco

@@ -96,17 +96,30 @@ __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, in
   f = warp_sum(f);
 #pragma unroll
   for (int j = 0; j < NPL; ++j) G[j] = 0.f;
-  // four slots' loads are issued before the first add (the loads are what costs time); the adds keep slot order
+  // The loads are what costs time (one L2/HBM round trip per batch): B slots' loads are issued before the first add,
+  // B = 9 while the registers last (two trips for the 18 segments of C3); the adds keep slot order (deterministic).
   const float* gp = sp.Gpart + (long long)g0 * sp.g_slot_stride + prow * sp.A_pad + lane;
   int s = g0;
-  for (; s + 4 <= g1; s += 4, gp += 4 * sp.g_slot_stride) {
-    float v[4][NPL];
+  constexpr int B = NPL <= 8 ? 9 : 4;
+  for (; s + B <= g1; s += B, gp += B * sp.g_slot_stride) {
+    float v[B][NPL];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int u = 0; u < B; ++u)
 #pragma unroll
       for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * sp.g_slot_stride + 32 * j) : 0.f;
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
+    for (int u = 0; u < B; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
+  }
+  for (; s + 3 <= g1; s += 3, gp += 3 * sp.g_slot_stride) {
+    float v[3][NPL];
+#pragma unroll
+    for (int u = 0; u < 3; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * sp.g_slot_stride + 32 * j) : 0.f;
+#pragma unroll
+    for (int u = 0; u < 3; ++u)
 #pragma unroll
       for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
   }
@@ -357,9 +370,9 @@ int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp,
 }
 
 // zero the "next round" counter; runs before the contraction kernels of a round
-__global__ void k_round_begin(int* n_running, int parity, int* log_slot) {
-  n_running[parity ^ 1] = 0;
-  if (log_slot) *log_slot = n_running[parity];
+__global__ void k_round_begin(int* zero_ctr, const int* gate, int* log_slot) {
+  *zero_ctr = 0;
+  if (log_slot) *log_slot = *gate;
 }
 
 // tail of the WHILE body (two rounds): loop again while a plan is running and the round budget lasts
@@ -375,8 +388,8 @@ int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-int launch_round_begin(const PlanDev& p, int parity, int round, cudaStream_t st) {
-  k_round_begin<<<1, 1, 0, st>>>(p.n_running, parity, round < kRoundLogCap ? p.round_log + round : nullptr);
+int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, cudaStream_t st) {
+  k_round_begin<<<1, 1, 0, st>>>(zero_ctr, gate, log_slot);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -20,7 +20,6 @@
 // warps 2-5 = epilogue (TMEM lane quadrant = warp_id % 4).  Pipelines are mbarrier rings.
 #include <cudaTypedefs.h>
 #include <stdio.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -228,6 +227,8 @@ struct DoseArgs {
   const int* row_src;         // [N_alloc]
   float* dose_dbg;            // [N][K] or null
   const int* gate;
+  int* zero_ctr;              // start-of-round bookkeeping, done by CTA (0, 0): *zero_ctr = 0, *log_slot = *gate
+  int* log_slot;
   int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, tlo_resident;
   Thresholds thr;
 };
@@ -250,6 +251,10 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
           const __grid_constant__ CUtensorMap tmT_lo, const DoseArgs a) {
+  if (a.zero_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+    *a.zero_ctr = 0;
+    if (a.log_slot) *a.log_slot = *a.gate;
+  }
   if (a.gate && *a.gate == 0) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -526,39 +531,39 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
     }
   } else if (warp == 1) {
     if (s1 > s0) {
-      // the accumulator is A_pad columns wide; one MMA covers at most 256 of them
+      // The accumulator is A_pad columns wide; one MMA covers at most 256 of them.  All three products of the split
+      // go into the same accumulator (as in k_dose_tc).  Lean issue loop: descriptors differ by 32-bit adds.
       const int n0 = a.A_pad <= 256 ? a.A_pad : 256, n1 = a.A_pad - n0;
       const uint32_t idesc0 = instr_desc(n0, 1, 1), idesc1 = instr_desc(n1 > 0 ? n1 : 16, 1, 1);
-      // separate accumulator (columns 256..) for the two correction products when the tile leaves room: see k_dose_tc
-      const uint32_t corr = a.A_pad <= 256 ? 256u : 0u;
+      constexpr uint32_t dhi = desc_hi(512, kSwz128Base32);
+      const int n_stage = a.n_stage;
+      const uint32_t base_lo = desc_lo(smem_u32(smem), PS * 128), stage_step = (uint32_t)stageBytes >> 4;
+      const uint32_t o_rlo = kRBytes >> 4, o_dhi = (2 * kRBytes) >> 4, o_dlo = (uint32_t)(2 * kRBytes + dBytes) >> 4;
+      const uint32_t o_n1 = (8 * PS * 128) >> 4;          // dwell groups 8.. : +8 groups of PS x 128 B
+      const uint32_t conv0 = smem_u32(conv), empty0 = smem_u32(empty);
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        mbar_wait(conv + st, ph);
+        mbar_wait_addr(conv0 + 8 * st, ph);
         tc_fence_after();
         if (elect_one()) {
-          const uint32_t base = smem_u32(smem + (size_t)st * stageBytes);
+          const uint32_t r = base_lo + (uint32_t)st * stage_step;
 #pragma unroll
           for (int j = 0; j < PS / 8; ++j) {        // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
-            const uint64_t r_hi = smem_desc(base + j * 1024, PS * 128, 512, kSwz128Base32);
-            const uint64_t r_lo = smem_desc(base + kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-            const uint64_t d_hi = smem_desc(base + 2 * kRBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-            const uint64_t d_lo = smem_desc(base + 2 * kRBytes + dBytes + j * 1024, PS * 128, 512, kSwz128Base32);
-            const uint32_t acc = (s > s0 || j > 0) ? 1u : 0u;
-            mma_ss(tmem, r_hi, d_hi, idesc0, acc);
-            mma_ss(tmem + corr, r_hi, d_lo, idesc0, corr ? acc : 1u);
-            mma_ss(tmem + corr, r_lo, d_hi, idesc0, 1);
-            if (n1 > 0) {                            // dwell groups 8.. : +8 groups of PS x 128 B
-              const uint64_t off = (uint64_t)((8 * PS * 128) >> 4);
-              mma_ss(tmem + 256, r_hi, d_hi + off, idesc1, acc);
-              mma_ss(tmem + 256, r_hi, d_lo + off, idesc1, 1);
-              mma_ss(tmem + 256, r_lo, d_hi + off, idesc1, 1);
+            const uint32_t rh = r + j * 64, rl = rh + o_rlo, dh = rh + o_dhi, dl = rh + o_dlo;
+            mma_ss2(tmem, rh, dhi, dh, dhi, idesc0, (s > s0 || j > 0) ? 1u : 0u);
+            mma_ss2(tmem, rh, dhi, dl, dhi, idesc0, 1);
+            mma_ss2(tmem, rl, dhi, dh, dhi, idesc0, 1);
+            if (n1 > 0) {
+              mma_ss2(tmem + 256, rh, dhi, dh + o_n1, dhi, idesc1, (s > s0 || j > 0) ? 1u : 0u);
+              mma_ss2(tmem + 256, rh, dhi, dl + o_n1, dhi, idesc1, 1);
+              mma_ss2(tmem + 256, rl, dhi, dh + o_n1, dhi, idesc1, 1);
             }
           }
-          tc_commit(empty + st);
+          tc_commit_addr(empty0 + 8 * st);
           if (s == s1 - 1) tc_commit(acc_full);
         }
         __syncwarp();
-        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        if (++st == n_stage) { st = 0; ph ^= 1; }
       }
     }
   } else {
@@ -588,28 +593,31 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
     }
-    float4* dst = reinterpret_cast<float4*>(a.Gpart + (((size_t)tile * a.segs + seg) * 128 + L) * a.A_pad);
+    // Epilogue: thread L owns plan L's row of the tile.  TMEM -> registers -> a padded row in shared memory (the ring is
+    // idle by now; pitch A_pad + 4 floats keeps 16 B stores conflict-free) -> ONE bulk asynchronous copy of the whole
+    // row (4 A_pad bytes, contiguous in Gpart) per thread.  No cross-thread hand-off: a thread copies what it wrote.
+    float* grow = a.Gpart + (((size_t)tile * a.segs + seg) * 128 + L) * a.A_pad;
     if (s1 > s0) {
       mbar_wait(acc_full, 0);
       tc_fence_after();
+      float* srow = reinterpret_cast<float*>(smem) + (size_t)L * (a.A_pad + 4);
       for (int g = 0; g < G; ++g) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + g * 32, v);
-        if (a.A_pad <= 256) {
-          uint32_t vc[32];
-          tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
-          tmem_ld_wait();
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
-        } else {
-          tmem_ld_wait();
-        }
+        tmem_ld_wait();
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          dst[g * 8 + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                                       __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+          *reinterpret_cast<float4*>(srow + g * 32 + 4 * i) =
+              make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                          __uint_as_float(v[4 * i + 3]));
       }
+      fence_proxy_async();
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(grow), "r"(smem_u32(srow)),
+                   "r"((uint32_t)a.A_pad * 4u) : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");      // shared memory may go once it has been read
     } else {
+      float4* dst = reinterpret_cast<float4*>(grow);
       for (int i = 0; i < a.A_pad / 4; ++i) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
@@ -678,8 +686,8 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   if (t->dose_stages * stageB < kScratchBytes) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
   t->dose_smem = fixed + t->dose_stages * stageB;
   // gradient kernel
-  t->grad_ps = c.A_pad <= 256 ? 32 : 16;
-  if (const char* e = getenv("GMCO_GRAD_PS")) { const int v = atoi(e); if (v == 8 || v == 16 || v == 32) t->grad_ps = v; }
+  // 16-point stages: the ring is deeper in stages than with 32 (C3: 4 x 48 KB instead of 2 x 96 KB), measured faster
+  t->grad_ps = 16;
   const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
   t->grad_stages = (kSmemMax - 1024 - 512) / stage;
   if (t->grad_stages > 9) t->grad_stages = 9;
@@ -694,9 +702,7 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
   cudaError_t e = cudaFuncSetAttribute(k_dose_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   std::vector<int> seg(t->n_tiles + 1);
   for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
   t->tile_seg_dev = p.tile_seg;                    // lives in the plan arena; pageable source: staged before the call returns
@@ -714,12 +720,12 @@ int tc_num_segments(const TcPlan* t) { return t->n_tiles * t->segs; }
 const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
 
 int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   cudaStream_t st) {
+                   int* zero_ctr, int* log_slot, cudaStream_t st) {
   dim3 grid(t->segs, t->n_tiles);
   DoseArgs da{};
   da.T_hi = p.T_hi; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
-  da.gate = gate; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
+  da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
   da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 2 * kPC <= 512 ? 2 : 1;
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
   k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
@@ -727,12 +733,7 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
   ga.n_stage = t->grad_stages;
-  if (t->grad_ps == 32)
-    k_grad_tc<32><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
-  else if (t->grad_ps == 16)
-    k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
-  else
-    k_grad_tc<8><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+  k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
   return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
 
