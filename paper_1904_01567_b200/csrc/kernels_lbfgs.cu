@@ -177,18 +177,27 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     }
   };
 
+  // Every global read of the plan's state is issued here, before the partial sums, so that the whole kernel pays
+  // about one memory round trip plus the two batches of the gradient partials (it is latency-bound, not
+  // bandwidth-bound).  rho / gamma of the m history pairs live in lanes 0..m-1 and are broadcast by shuffle in the
+  // two-loop recursion: a global load per recursion step would put 2 m dependent L2 latencies on the critical path.
   float G[NPL], xt[NPL], gt[NPL], x[NPL], g[NPL];
-  const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G);
 #pragma unroll
   for (int j = 0; j < NPL; ++j) {
     xt[j] = j < npl ? pp.xt[row + 32 * j] : 0.f;
-    gt[j] = g_scale * xt[j] * G[j];                          // Eq. 3 summed: g = 2 x o (D^T r)
+    x[j] = j < npl ? pp.x[row + 32 * j] : 0.f;
+    g[j] = j < npl ? pp.g[row + 32 * j] : 0.f;
   }
-
+  float rho_l = lane < sp.m ? pp.rho[(long long)lane * pp.K_pad + k] : 0.f;
+  float gam_l = lane < sp.m ? pp.gam[(long long)lane * pp.K_pad + k] : 0.f;
   int tr = pp.trials[k];
   float F = pp.F[k];
   int it = pp.it_done[k];
   int hc = pp.hcount[k], hh = pp.hhead[k];
+  const float alpha = pp.alpha[k], gp = pp.gp[k];
+  const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G);
+#pragma unroll
+  for (int j = 0; j < NPL; ++j) gt[j] = g_scale * xt[j] * G[j];   // Eq. 3 summed: g = 2 x o (D^T r)
   int status = PLAN_RUNNING;
   bool new_dir = false;
 
@@ -199,9 +208,6 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     new_dir = true;
     if (it >= sp.iters) status = GMCO_PLAN_ITERS;
   } else {
-    const float alpha = pp.alpha[k], gp = pp.gp[k];
-#pragma unroll
-    for (int j = 0; j < NPL; ++j) { x[j] = j < npl ? pp.x[row + 32 * j] : 0.f; g[j] = j < npl ? pp.g[row + 32 * j] : 0.f; }
     bool accept = Ft <= F + sp.c1 * alpha * gp;              // Armijo
     if (!accept && sp.eps_f > 0.f && Ft <= F + sp.eps_f * fabsf(F)) {
       // approximate test (reading A5b): F within its noise allowance and slope condition
@@ -231,7 +237,10 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
             Sd[32 * j] = sv[j]; Yd[32 * j] = yv[j];
             hS[hh * sp.A_pad + lane + 32 * j] = sv[j]; hY[hh * sp.A_pad + lane + 32 * j] = yv[j];
           }
-        if (lane == 0) { pp.rho[(long long)hh * pp.K_pad + k] = 1.f / sy; pp.gam[(long long)hh * pp.K_pad + k] = sy / yy; }
+        if (lane == hh) {
+          rho_l = 1.f / sy; gam_l = sy / yy;
+          pp.rho[(long long)hh * pp.K_pad + k] = rho_l; pp.gam[(long long)hh * pp.K_pad + k] = gam_l;
+        }
         hh = hh + 1 == sp.m ? 0 : hh + 1;
         hc = min(hc + 1, sp.m);
       }
@@ -286,14 +295,15 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
 #pragma unroll
         for (int j = 0; j < NPL; ++j) d = fmaf(sv[j], q[j], d);
-        const float a = pp.rho[(long long)slot * pp.K_pad + k] * warp_sum(d);
+        const float a = __shfl_sync(0xffffffffu, rho_l, slot) * warp_sum(d);
 #pragma unroll
         for (int j = 0; j < NPL; ++j) q[j] = fmaf(-a, yv[j], q[j]);
         if (lane == 0) s_a[warp][i] = a;
       }
       __syncwarp();
       int newest = hh - 1; if (newest < 0) newest += sp.m;
-      const float gamma = hc > 0 ? pp.gam[(long long)newest * pp.K_pad + k] : 1.f / gnorm;
+      const float gam_n = __shfl_sync(0xffffffffu, gam_l, newest);
+      const float gamma = hc > 0 ? gam_n : 1.f / gnorm;
 #pragma unroll
       for (int j = 0; j < NPL; ++j) q[j] *= gamma;
       for (int i = hc - 1; i >= 0; --i) {
@@ -305,7 +315,7 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         for (int j = 0; j < NPL; ++j) { sv[j] = j < npl ? Sd[32 * j] : 0.f; yv[j] = j < npl ? Yd[32 * j] : 0.f; }
 #pragma unroll
         for (int j = 0; j < NPL; ++j) d = fmaf(yv[j], q[j], d);
-        const float b = pp.rho[(long long)slot * pp.K_pad + k] * warp_sum(d);
+        const float b = __shfl_sync(0xffffffffu, rho_l, slot) * warp_sum(d);
         const float coef = s_a[warp][i] - b;
 #pragma unroll
         for (int j = 0; j < NPL; ++j) q[j] = fmaf(sv[j], coef, q[j]);

@@ -218,7 +218,7 @@ constexpr int kDoseThreads = 320;       // warp 0 TMA, warp 1 MMA, warps 2-9 epi
 constexpr int kScratchBytes = 8 * 4096; // T_hi transposition scratch, one 32 x 128 B slab per epilogue warp
 
 struct DoseArgs {
-  const float* T_hi;          // [K_pad][A_pad]
+  const float* T;             // [K_pad][A_pad] trial dwell times, fp32; split into tf32 (hi, lo) in the prologue
   float* R;                   // [N_alloc][K_pad]  dF/dd / 2 (fp32; the gradient kernel splits it)
   float* Fpart;               // [n_tiles * segs][128][2]
   const float* Weff;          // [K_pad][2S]
@@ -239,6 +239,11 @@ struct GradArgs {
   int A_pad, n_slabs, segs, n_stage;
 };
 
+__device__ __forceinline__ float tf32_rn(float v) {
+  uint32_t u;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
+  return __uint_as_float(u);
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------------
@@ -250,7 +255,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // The last kScratchBytes of the ring double as the T_hi transposition scratch of the prologue.
 __global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
-          const __grid_constant__ CUtensorMap tmT_lo, const DoseArgs a) {
+          const __grid_constant__ CUtensorMap tmT_lo, const __grid_constant__ CUtensorMap tmT, const DoseArgs a) {
   if (a.zero_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
     *a.zero_ctr = 0;
     if (a.log_slot) *a.log_slot = *a.gate;
@@ -268,9 +273,9 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   uint64_t* bars = reinterpret_cast<uint64_t*>(ring + ringBytes);
   uint64_t* full = bars;                            // [n_stage]
   uint64_t* empty = bars + a.n_stage;               // [n_stage]
-  uint64_t* tlo_full = bars + 2 * a.n_stage;
-  uint64_t* thi_ready = tlo_full + 1;
-  uint64_t* acc_full = thi_ready + 1;               // [2]
+  uint64_t* tg_ready = bars + 2 * a.n_stage;        // [kMaxApadTensor / 32]: T of dwell group g is in TMEM / smem
+  uint64_t* tin_full = tg_ready + kMaxApadTensor / 32;   // [kMaxApadTensor / 32]: fp32 T of group g has landed (TMA)
+  uint64_t* acc_full = tin_full + kMaxApadTensor / 32;   // [2]
   uint64_t* acc_empty = acc_full + 2;               // [2]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
@@ -280,12 +285,11 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
-    mbar_init(tlo_full, 1);
-    mbar_init(thi_ready, 256);
+    for (int i = 0; i < kMaxApadTensor / 32; ++i) { mbar_init(tg_ready + i, 128); mbar_init(tin_full + i, 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 256); }
     fence_barrier_init();
   }
-  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT_lo); }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT_lo); tma_prefetch_desc(&tmT); }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
   tc_fence_before();
   __syncthreads();
@@ -300,20 +304,25 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   if (warp == 0) {
     // whole warp walks the ring (uniform control flow); one elected lane issues
     if (c1 > c0) {
-      if (a.tlo_resident) {
+      const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
+      if (a.tlo_resident) {                         // fp32 T of the tile lands where its lo part will live
         if (elect_one()) {
-          mbar_expect_tx(tlo_full, (uint32_t)G * kTloBox);
-          for (int g = 0; g < G; ++g) tma_load_3d(&tmT_lo, tlo + (size_t)g * kTloBox, tlo_full, 0, tile * 128, g, l2_evict_normal());
+          for (int g = 0; g < G; ++g) {
+            mbar_expect_tx(tin_full + g, (uint32_t)kTloBox);
+            tma_load_3d(&tmT, tlo + (size_t)g * kTloBox, tin_full + g, 0, tile * 128, g, polT);
+          }
         }
         __syncwarp();
       }
-      const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
       int st = 0; uint32_t ph = 0;
-      bool scratch_busy = true;
+      bool scratch_busy = !a.tlo_resident;          // resident mode transposes through the T_lo area itself
       for (int c = c0; c < c1; ++c) {
         for (int g2 = 0; g2 < 2 * G; ++g2) {          // entry 2 g: D_hi (+ streamed T_lo), entry 2 g + 1: D_lo
           const int g = g2 >> 1, lo = g2 & 1;
-          if (scratch_busy && st >= scr_slot) { mbar_wait(thi_ready, 0); scratch_busy = false; }
+          if (scratch_busy && st >= scr_slot) {       // the prologue's transposition scratch overlaps these slots
+            for (int i = 0; i < G; ++i) mbar_wait(tg_ready + i, 0);
+            scratch_busy = false;
+          }
           mbar_wait(empty + st, ph ^ 1);
           if (elect_one()) {
             uint8_t* dst = ring + (size_t)st * stageBytes;
@@ -337,9 +346,6 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
       const uint32_t ring_lo = desc_lo(smem_u32(ring), 16), ring_step = (uint32_t)stageBytes >> 4;
       const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
       const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
-      if (a.tlo_resident) mbar_wait(tlo_full, 0);
-      mbar_wait(thi_ready, 0);
-      tc_fence_after();
       int st = 0; uint32_t ph = 0;
       for (int c = c0; c < c1; ++c) {
         const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
@@ -349,6 +355,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         uint32_t thi = t_thi, alo = tlo_lo0;
         for (int g = 0; g < G; ++g, thi += 32, alo += kTloBox >> 4) {
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
+          if (c == c0) { mbar_wait(tg_ready + g, 0); tc_fence_after(); }   // first chunk overlaps the prologue
           mbar_wait_addr(full0 + 8 * st, ph);
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
@@ -387,12 +394,41 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     float f_lo = 0.f, f_hi = 0.f;
     if (c1 > c0) {
-      // prologue: T_hi rows of this quadrant -> TMEM columns [0, A_pad).  Coalesced 128 B row reads, transposed
-      // through a per-warp 4 KB scratch (XOR-swizzled 16 B chunks: conflict-free both ways); slabs g = h, h + 2, ...
-      {
+      // Prologue: the tile's trial dwell times T (fp32, read ONCE) are split here into tf32 parts: hi -> TMEM columns
+      // [0, A_pad) (the A operand of T_hi D), lo -> shared memory (the A operand of T_lo D_hi).  Slabs g = h, h + 2, ...;
+      // each slab has its own ready barrier, so the first chunk's MMAs start while later slabs are still on their way.
+      if (a.tlo_resident) {
+        // TMA has put slab g of T where T_lo will live, in the SWIZZLE_128B K-major layout of the MMA descriptor.
+        // Thread = plan row: it reads its own 128 B row (8 swizzled 16 B chunks), keeps hi for TMEM and writes lo
+        // back in place -- no cross-thread hand-off, no transposition scratch.
+        const int row = q * 32 + lane;
+        for (int g = h; g < G; g += 2) {
+          uint8_t* base = tlo + (size_t)g * kTloBox + row * 128;
+          mbar_wait(tin_full + g, 0);
+          uint32_t v[32];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            float4* cell = reinterpret_cast<float4*>(base + ((k ^ (row & 7)) << 4));
+            const float4 t = *cell;
+            float4 hi, lo;
+            hi.x = tf32_rn(t.x); hi.y = tf32_rn(t.y); hi.z = tf32_rn(t.z); hi.w = tf32_rn(t.w);
+            lo.x = tf32_rn(t.x - hi.x); lo.y = tf32_rn(t.y - hi.y); lo.z = tf32_rn(t.z - hi.z); lo.w = tf32_rn(t.w - hi.w);
+            *cell = lo;
+            v[4 * k + 0] = __float_as_uint(hi.x); v[4 * k + 1] = __float_as_uint(hi.y);
+            v[4 * k + 2] = __float_as_uint(hi.z); v[4 * k + 3] = __float_as_uint(hi.w);
+          }
+          tmem_st32(t_thi + lane_base + g * 32, v);
+          tmem_st_wait();
+          tc_fence_before();
+          fence_proxy_async();                      // the lo stores above are read by the MMA (async proxy)
+          mbar_arrive(tg_ready + g);
+        }
+      } else {
+        // streamed-T_lo mode (more than 320 dwell positions): T_lo comes from global memory with every D_hi slab;
+        // hi is read from T with coalesced 128 B row loads and transposed through the tail of the ring.
         uint8_t* scr = scratch + e * 4096;
         const int r0 = lane >> 3, c4 = lane & 7;
-        const float* src = a.T_hi + (size_t)(tile * 128 + q * 32) * a.A_pad;
+        const float* src = a.T + (size_t)(tile * 128 + q * 32) * a.A_pad;
         for (int g = h; g < G; g += 2) {
           float4 t[8];
 #pragma unroll
@@ -401,7 +437,9 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const int r = i * 4 + r0;
-            *reinterpret_cast<float4*>(scr + r * 128 + ((c4 ^ (r & 7)) << 4)) = t[i];
+            float4 hi;
+            hi.x = tf32_rn(t[i].x); hi.y = tf32_rn(t[i].y); hi.z = tf32_rn(t[i].z); hi.w = tf32_rn(t[i].w);
+            *reinterpret_cast<float4*>(scr + r * 128 + ((c4 ^ (r & 7)) << 4)) = hi;
           }
           __syncwarp();
           uint32_t v[32];
@@ -413,10 +451,10 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           }
           __syncwarp();
           tmem_st32(t_thi + lane_base + g * 32, v);
+          tmem_st_wait();
+          tc_fence_before();
+          mbar_arrive(tg_ready + g);
         }
-        tmem_st_wait();
-        tc_fence_before();
-        mbar_arrive(thi_ready);
       }
 
       // This warp evaluates the 64-row tile 2 c + h of chunk c (one structure per 64-row tile by construction).
@@ -658,7 +696,7 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long cols,
 }  // namespace
 
 struct TcPlan {
-  CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo;
+  CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
   int segs = 1, n_tiles = 0;
   int dose_stages = 0, dose_smem = 0, tlo_resident = 1;
@@ -697,6 +735,7 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   bool ok = make_map(&t->dose_D_hi, c.D_hi, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_D_lo, c.D_lo, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK) &&
+            make_map(&t->dose_T, p.T, p.K_pad, c.A_pad, 128, 1, sK) &&
             make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
@@ -723,12 +762,12 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
                    int* zero_ctr, int* log_slot, cudaStream_t st) {
   dim3 grid(t->segs, t->n_tiles);
   DoseArgs da{};
-  da.T_hi = p.T_hi; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
+  da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
   da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
   da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 2 * kPC <= 512 ? 2 : 1;
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
-  k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, da);
+  k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
   if (cudaGetLastError() != cudaSuccess) return -1;
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
