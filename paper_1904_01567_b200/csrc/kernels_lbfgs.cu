@@ -82,53 +82,46 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
 
 // ---------------------------------------------------------------------------------------------
 // Fixed-order reduction of the contraction kernels' partial results for plan k.
+// The loads are what costs time (one L2/HBM round trip per dependent batch), so they are issued in as few batches as
+// the registers allow -- the objective partials and up to 18 gradient slots (all of C3's) before the first add; the
+// adds keep slot order, so the result does not depend on scheduling.
+template <int NPL, int B>
+__device__ __forceinline__ void add_slots(const float*& gp, int& s, int g1, long long stride, int npl, float (&G)[NPL]) {
+  for (; s + B <= g1; s += B, gp += B * stride) {
+    float v[B][NPL];
+#pragma unroll
+    for (int u = 0; u < B; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * stride + 32 * j) : 0.f;
+#pragma unroll
+    for (int u = 0; u < B; ++u)
+#pragma unroll
+      for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
+  }
+}
+
 template <int NPL>
 __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, int lane, int npl, float (&G)[NPL]) {
   int f0 = 0, f1 = sp.nF, g0 = 0, g1 = sp.nG;
   long long prow = k;
   if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
-  float f = 0.f;
   const int nfe = (f1 - f0) * sp.nFcomp;                   // SIMT: (lo, hi) pairs per slot
-  for (int i = lane; i < nfe; i += 32) {
+  auto f_at = [&](int i) {
     const int slot = f0 + i / sp.nFcomp, comp = i % sp.nFcomp;
-    f += sp.Fpart[(long long)slot * sp.f_slot_stride + prow * sp.nFcomp + comp];
-  }
-  f = warp_sum(f);
+    return sp.Fpart[(long long)slot * sp.f_slot_stride + prow * sp.nFcomp + comp];
+  };
+  // objective partials: the first two per lane are in flight together with the first gradient batch
+  const float fa = lane < nfe ? f_at(lane) : 0.f, fb = lane + 32 < nfe ? f_at(lane + 32) : 0.f;
 #pragma unroll
   for (int j = 0; j < NPL; ++j) G[j] = 0.f;
-  // The loads are what costs time (one L2/HBM round trip per batch): B slots' loads are issued before the first add,
-  // B = 9 while the registers last (two trips for the 18 segments of C3); the adds keep slot order (deterministic).
   const float* gp = sp.Gpart + (long long)g0 * sp.g_slot_stride + prow * sp.A_pad + lane;
   int s = g0;
-  constexpr int B = NPL <= 8 ? 9 : 4;
-  for (; s + B <= g1; s += B, gp += B * sp.g_slot_stride) {
-    float v[B][NPL];
-#pragma unroll
-    for (int u = 0; u < B; ++u)
-#pragma unroll
-      for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * sp.g_slot_stride + 32 * j) : 0.f;
-#pragma unroll
-    for (int u = 0; u < B; ++u)
-#pragma unroll
-      for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
-  }
-  for (; s + 3 <= g1; s += 3, gp += 3 * sp.g_slot_stride) {
-    float v[3][NPL];
-#pragma unroll
-    for (int u = 0; u < 3; ++u)
-#pragma unroll
-      for (int j = 0; j < NPL; ++j) v[u][j] = j < npl ? __ldcs(gp + u * sp.g_slot_stride + 32 * j) : 0.f;
-#pragma unroll
-    for (int u = 0; u < 3; ++u)
-#pragma unroll
-      for (int j = 0; j < NPL; ++j) G[j] += v[u][j];
-  }
-  for (; s < g1; ++s, gp += sp.g_slot_stride) {
-#pragma unroll
-    for (int j = 0; j < NPL; ++j)
-      if (j < npl) G[j] += __ldcs(gp + 32 * j);
-  }
-  return f;
+  add_slots<NPL, (NPL <= 8 ? 18 : 6)>(gp, s, g1, sp.g_slot_stride, npl, G);
+  add_slots<NPL, 6>(gp, s, g1, sp.g_slot_stride, npl, G);
+  add_slots<NPL, 1>(gp, s, g1, sp.g_slot_stride, npl, G);
+  float f = fa + fb;
+  for (int i = lane + 64; i < nfe; i += 32) f += f_at(i);
+  return warp_sum(f);
 }
 
 // ---------------------------------------------------------------------------------------------
