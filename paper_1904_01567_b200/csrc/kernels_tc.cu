@@ -36,6 +36,7 @@ namespace {
 constexpr int kPC = 128;
 constexpr int kSlabBytes = kPC * 128;   // one 32-dwell slab of a dose chunk, one part (hi or lo): 16 KB
 constexpr int kTloBox = 128 * 128;      // T_lo: 128 plans x 32 dwell: 16 KB
+constexpr int kTmemGroups = 8;          // dwell groups of T_hi kept in TMEM (256 columns)
 constexpr int kThreads = 192;
 constexpr uint32_t kWatchdog = 1u << 26;
 
@@ -229,7 +230,7 @@ struct DoseArgs {
   const int* gate;
   int* zero_ctr;              // start-of-round bookkeeping, done by CTA (0, 0): *zero_ctr = 0, *log_slot = *gate
   int* log_slot;
-  int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, tlo_resident;
+  int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, sep_corr, tlo_resident;
   Thresholds thr;
 };
 
@@ -253,6 +254,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // the D_hi slab and the D_lo slab of one (chunk, 32-dwell group): 16 KB each, so the ring is deep in entries although
 // a chunk is 128 points wide; when T_lo is streamed, its 16 KB slab rides behind the D_hi slab of its group.
 // The last kScratchBytes of the ring double as the T_hi transposition scratch of the prologue.
+template <bool kResident>   // T_lo resident in shared memory (at most 256 dwell positions) or streamed with D_hi
 __global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
           const __grid_constant__ CUtensorMap tmT_lo, const __grid_constant__ CUtensorMap tmT, const DoseArgs a) {
@@ -264,9 +266,12 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
-  const int stageBytes = a.tlo_resident ? kSlabBytes : kSlabBytes + kTloBox;
-  uint8_t* tlo = smem;                              // [G][128 plans][128 B] when resident
-  uint8_t* ring = smem + (a.tlo_resident ? (size_t)G * kTloBox : 0);
+  const int stageBytes = kResident ? kSlabBytes : kSlabBytes + kTloBox;
+  // TMEM holds T_hi of the first kTmemGroups dwell groups (256 columns); with more groups the rest of T_hi lives in
+  // shared memory (the "tail", SS MMAs) so that both accumulators always fit.
+  const int Gs = kResident ? 0 : (G > kTmemGroups ? G - kTmemGroups : 0);
+  uint8_t* tlo = smem;                              // resident: T_lo [G][128 plans][128 B]; streamed: T_hi tail [Gs][..]
+  uint8_t* ring = smem + (size_t)(kResident ? G : Gs) * kTloBox;
   const int ringBytes = a.n_stage * stageBytes;
   uint8_t* scratch = ring + ringBytes - kScratchBytes;
   const int scr_slot = (ringBytes - kScratchBytes) / stageBytes;   // first ring slot that overlaps the scratch
@@ -296,16 +301,19 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   tc_fence_after();
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
   const uint32_t t_thi = tmem;                      // columns [0, A_pad): T_hi
-  // columns [A_pad, A_pad + 128 n_acc): one 128-point accumulator per buffer; the three products of the split
-  // accumulate into it in ring order (the tensor core truncates when it adds into the fp32 accumulator: measured
-  // dose error stays below 1e-5 relative).
-  const uint32_t t_acc = tmem + a.A_pad;
+  // columns [A_pad, ...): per buffer a MAIN accumulator (T_hi D_hi) and, when the columns last (A_pad <= 256), a
+  // separate CORRECTION accumulator (T_hi D_lo + T_lo D_hi), 128 points each.  The tensor core truncates when it adds
+  // into the fp32 accumulator; keeping the 64 small products of a chunk out of the large sum cuts that one-sided error
+  // from ~1e-5 to ~2e-6 of the dose, and the dose error is what the gradient feels near a threshold (r = d - D_lim
+  // cancels).  With both accumulators there is room for one buffer only: the epilogue frees it as soon as the values
+  // are in registers, the penalty arithmetic and the R stores still overlap the next chunk's MMAs.
+  const uint32_t t_acc = tmem + (G < kTmemGroups ? G : kTmemGroups) * 32;
 
   if (warp == 0) {
     // whole warp walks the ring (uniform control flow); one elected lane issues
     if (c1 > c0) {
       const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
-      if (a.tlo_resident) {                         // fp32 T of the tile lands where its lo part will live
+      if (kResident) {                         // fp32 T of the tile lands where its lo part will live
         if (elect_one()) {
           for (int g = 0; g < G; ++g) {
             mbar_expect_tx(tin_full + g, (uint32_t)kTloBox);
@@ -315,7 +323,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         __syncwarp();
       }
       int st = 0; uint32_t ph = 0;
-      bool scratch_busy = !a.tlo_resident;          // resident mode transposes through the T_lo area itself
+      bool scratch_busy = !kResident;          // resident mode transposes through the T_lo area itself
       for (int c = c0; c < c1; ++c) {
         for (int g2 = 0; g2 < 2 * G; ++g2) {          // entry 2 g: D_hi (+ streamed T_lo), entry 2 g + 1: D_lo
           const int g = g2 >> 1, lo = g2 & 1;
@@ -326,7 +334,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           mbar_wait(empty + st, ph ^ 1);
           if (elect_one()) {
             uint8_t* dst = ring + (size_t)st * stageBytes;
-            const bool with_t = !lo && !a.tlo_resident;
+            const bool with_t = !lo && !kResident;
             mbar_expect_tx(full + st, (uint32_t)(with_t ? kSlabBytes + kTloBox : kSlabBytes));
             tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, c * kPC, g, polD);
             if (with_t) tma_load_3d(&tmT_lo, dst + kSlabBytes, full + st, 0, tile * 128, g, polT);
@@ -351,21 +359,29 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
         mbar_wait(acc_empty + b, (use & 1) ^ 1);
         tc_fence_after();
-        const uint32_t acc = t_acc + b * kPC;
-        uint32_t thi = t_thi, alo = tlo_lo0;
-        for (int g = 0; g < G; ++g, thi += 32, alo += kTloBox >> 4) {
+        const uint32_t acc = t_acc + b * (a.sep_corr ? 2 * kPC : kPC), acc_c = a.sep_corr ? acc + kPC : acc;
+        uint32_t thi = t_thi, alo = tlo_lo0;   // alo: resident T_lo slab g, or (streamed) T_hi tail slab g - kTmemGroups
+        for (int g = 0; g < G; thi += 32, alo += (kResident || g >= kTmemGroups) ? kTloBox >> 4 : 0, ++g) {
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
           if (c == c0) { mbar_wait(tg_ready + g, 0); tc_fence_after(); }   // first chunk overlaps the prologue
           mbar_wait_addr(full0 + 8 * st, ph);
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
-            const uint32_t ad = a.tlo_resident ? alo : bd + (kSlabBytes >> 4);
-            mma_ts2(acc, thi, bd, dhi, idesc, g != 0);
-            mma_ss2(acc, ad, dhi, bd, dhi, idesc, 1);
+            const uint32_t ad = kResident ? alo : bd + (kSlabBytes >> 4);
+            if (kResident || g < kTmemGroups) {
+              mma_ts2(acc, thi, bd, dhi, idesc, g != 0);
+              mma_ss2(acc_c, ad, dhi, bd, dhi, idesc, (a.sep_corr && g == 0) ? 0u : 1u);
 #pragma unroll
-            for (int j = 1; j < 4; ++j) {           // K-steps of 8 dwell positions: +32 B inside the swizzled row
-              mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
-              mma_ss2(acc, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+              for (int j = 1; j < 4; ++j) {         // K-steps of 8 dwell positions: +32 B inside the swizzled row
+                mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+                mma_ss2(acc_c, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+              }
+            } else {                                // T_hi of this group is in the shared-memory tail
+#pragma unroll
+              for (int j = 0; j < 4; ++j) {
+                mma_ss2(acc, alo + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+                mma_ss2(acc_c, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+              }
             }
             tc_commit_addr(empty0 + 8 * st);
           }
@@ -375,8 +391,13 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           mbar_wait_addr(full0 + 8 * st, ph);
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+            if (kResident || g < kTmemGroups) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+              for (int j = 0; j < 4; ++j) mma_ts2(acc_c, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) mma_ss2(acc_c, alo + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+            }
             tc_commit_addr(empty0 + 8 * st);
             if (g == G - 1) tc_commit(acc_full + b);
           }
@@ -397,7 +418,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
       // Prologue: the tile's trial dwell times T (fp32, read ONCE) are split here into tf32 parts: hi -> TMEM columns
       // [0, A_pad) (the A operand of T_hi D), lo -> shared memory (the A operand of T_lo D_hi).  Slabs g = h, h + 2, ...;
       // each slab has its own ready barrier, so the first chunk's MMAs start while later slabs are still on their way.
-      if (a.tlo_resident) {
+      if (kResident) {
         // TMA has put slab g of T where T_lo will live, in the SWIZZLE_128B K-major layout of the MMA descriptor.
         // Thread = plan row: it reads its own 128 B row (8 swizzled 16 B chunks), keeps hi for TMEM and writes lo
         // back in place -- no cross-thread hand-off, no transposition scratch.
@@ -434,6 +455,19 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 #pragma unroll
           for (int i = 0; i < 8; ++i)
             t[i] = *reinterpret_cast<const float4*>(src + (size_t)(i * 4 + r0) * a.A_pad + g * 32 + c4 * 4);
+          if (g >= kTmemGroups) {                    // tail group: hi goes to shared memory in the operand layout
+            uint8_t* dstg = tlo + (size_t)(g - kTmemGroups) * kTloBox + q * 4096;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const int r = i * 4 + r0;
+              float4 hi;
+              hi.x = tf32_rn(t[i].x); hi.y = tf32_rn(t[i].y); hi.z = tf32_rn(t[i].z); hi.w = tf32_rn(t[i].w);
+              *reinterpret_cast<float4*>(dstg + r * 128 + ((c4 ^ (r & 7)) << 4)) = hi;
+            }
+            fence_proxy_async();
+            mbar_arrive(tg_ready + g);
+            continue;
+          }
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const int r = i * 4 + r0;
@@ -473,9 +507,21 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         mbar_wait(acc_full + b, use & 1);
         tc_fence_after();
         uint32_t v[2][32];
-        tmem_ld32(t_acc + lane_base + b * kPC + h * 64, v[0]);
-        tmem_ld32(t_acc + lane_base + b * kPC + h * 64 + 32, v[1]);
-        tmem_ld_wait();
+        const uint32_t t_main = t_acc + lane_base + b * (a.sep_corr ? 2 * kPC : kPC) + h * 64;
+        tmem_ld32(t_main, v[0]);
+        tmem_ld32(t_main + 32, v[1]);
+        if (a.sep_corr) {
+#pragma unroll
+          for (int sub = 0; sub < 2; ++sub) {
+            uint32_t vc[32];
+            tmem_ld32(t_main + kPC + sub * 32, vc);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[sub][j] = __float_as_uint(__uint_as_float(v[sub][j]) + __uint_as_float(vc[j]));
+          }
+        } else {
+          tmem_ld_wait();
+        }
         tc_fence_before();
         mbar_arrive(acc_empty + b);
 #pragma unroll
@@ -524,12 +570,13 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
           const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
   if (a.gate && *a.gate == 0) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem0 = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = smem0 + 1024;                     // [barriers 1 KB | ring | (epilogue row staging may run past the ring)]
   const int G = a.A_pad >> 5;
   constexpr int kRBytes = 4 * PS * 128;             // R part: 4 plan groups x PS points x 128 B
   const int dBytes = G * PS * 128;                  // D part: G dwell groups x PS points x 128 B
   const int stageBytes = 2 * kRBytes + 2 * dBytes;  // [R | R_lo | D_hi | D_lo]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)a.n_stage * stageBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem0);
   uint64_t* full = bars;
   uint64_t* empty = bars + a.n_stage;
   uint64_t* conv = bars + 2 * a.n_stage;
@@ -569,11 +616,13 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
     }
   } else if (warp == 1) {
     if (s1 > s0) {
-      // The accumulator is A_pad columns wide; one MMA covers at most 256 of them.  All three products of the split
-      // go into the same accumulator (as in k_dose_tc).  Lean issue loop: descriptors differ by 32-bit adds.
+      // The accumulator is A_pad columns wide; one MMA covers at most 256 of them.  When the columns last (A_pad <= 256)
+      // the two correction products go into a separate accumulator at column 256 (see k_dose_tc: the tensor core's
+      // accumulate truncates).  Lean issue loop: descriptors differ by 32-bit adds.
       const int n0 = a.A_pad <= 256 ? a.A_pad : 256, n1 = a.A_pad - n0;
       const uint32_t idesc0 = instr_desc(n0, 1, 1), idesc1 = instr_desc(n1 > 0 ? n1 : 16, 1, 1);
       constexpr uint32_t dhi = desc_hi(512, kSwz128Base32);
+      const uint32_t corr = a.A_pad <= 256 ? 256u : 0u;
       const int n_stage = a.n_stage;
       const uint32_t base_lo = desc_lo(smem_u32(smem), PS * 128), stage_step = (uint32_t)stageBytes >> 4;
       const uint32_t o_rlo = kRBytes >> 4, o_dhi = (2 * kRBytes) >> 4, o_dlo = (uint32_t)(2 * kRBytes + dBytes) >> 4;
@@ -588,9 +637,10 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
 #pragma unroll
           for (int j = 0; j < PS / 8; ++j) {        // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
             const uint32_t rh = r + j * 64, rl = rh + o_rlo, dh = rh + o_dhi, dl = rh + o_dlo;
-            mma_ss2(tmem, rh, dhi, dh, dhi, idesc0, (s > s0 || j > 0) ? 1u : 0u);
-            mma_ss2(tmem, rh, dhi, dl, dhi, idesc0, 1);
-            mma_ss2(tmem, rl, dhi, dh, dhi, idesc0, 1);
+            const uint32_t first = (s > s0 || j > 0) ? 1u : 0u;
+            mma_ss2(tmem, rh, dhi, dh, dhi, idesc0, first);
+            mma_ss2(tmem + corr, rh, dhi, dl, dhi, idesc0, corr ? first : 1u);
+            mma_ss2(tmem + corr, rl, dhi, dh, dhi, idesc0, 1);
             if (n1 > 0) {
               mma_ss2(tmem + 256, rh, dhi, dh + o_n1, dhi, idesc1, (s > s0 || j > 0) ? 1u : 0u);
               mma_ss2(tmem + 256, rh, dhi, dl + o_n1, dhi, idesc1, 1);
@@ -642,7 +692,15 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
       for (int g = 0; g < G; ++g) {
         uint32_t v[32];
         tmem_ld32(tmem + lane_base + g * 32, v);
-        tmem_ld_wait();
+        if (a.A_pad <= 256) {
+          uint32_t vc[32];
+          tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
+        } else {
+          tmem_ld_wait();
+        }
 #pragma unroll
         for (int i = 0; i < 8; ++i)
           *reinterpret_cast<float4*>(srow + g * 32 + 4 * i) =
@@ -716,8 +774,8 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   const int G = c.A_pad / 32;
   // dose kernel: T_lo resident when it leaves room for >= 2 ring stages, else streamed with every D slab
   const int slack = 1024 /*alignment*/ + 512 /*barriers*/;
-  t->tlo_resident = G * kTloBox + 4 * kSlabBytes + slack <= kSmemMax ? 1 : 0;
-  const int fixed = (t->tlo_resident ? G * kTloBox : 0) + slack;
+  t->tlo_resident = (G <= kTmemGroups && G * kTloBox + 4 * kSlabBytes + slack <= kSmemMax) ? 1 : 0;
+  const int fixed = (t->tlo_resident ? G : (G > kTmemGroups ? G - kTmemGroups : 0)) * kTloBox + slack;
   const int stageB = t->tlo_resident ? kSlabBytes : kSlabBytes + kTloBox;
   t->dose_stages = (kSmemMax - fixed) / stageB;
   if (t->dose_stages > 12) t->dose_stages = 12;
@@ -727,10 +785,11 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   // 16-point stages: the ring is deeper in stages than with 32 (C3: 4 x 48 KB instead of 2 x 96 KB), measured faster
   t->grad_ps = 16;
   const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
-  t->grad_stages = (kSmemMax - 1024 - 512) / stage;
+  const int staging = 128 * (c.A_pad + 4) * 4;     // epilogue: one padded accumulator row per plan
+  t->grad_stages = (kSmemMax - 2048) / stage;
   if (t->grad_stages > 9) t->grad_stages = 9;
   if (t->grad_stages < 2) { snprintf(err, errlen, "shared memory too small for the gradient ring"); delete t; return nullptr; }
-  t->grad_smem = 1024 + 512 + t->grad_stages * stage;
+  t->grad_smem = 2048 + (t->grad_stages * stage > staging ? t->grad_stages * stage : staging);
   const CUtensorMapSwizzle sK = CU_TENSOR_MAP_SWIZZLE_128B, sMN = CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
   bool ok = make_map(&t->dose_D_hi, c.D_hi, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_D_lo, c.D_lo, c.N_alloc, c.A_pad, kPC, 1, sK) &&
@@ -740,7 +799,8 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
-  cudaError_t e = cudaFuncSetAttribute(k_dose_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
+  cudaError_t e = t->tlo_resident ? cudaFuncSetAttribute(k_dose_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem)
+                                   : cudaFuncSetAttribute(k_dose_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   std::vector<int> seg(t->n_tiles + 1);
   for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
@@ -765,9 +825,11 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
   da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
-  da.segs = t->segs; da.n_stage = t->dose_stages; da.n_acc = c.A_pad + 2 * kPC <= 512 ? 2 : 1;
+  da.segs = t->segs; da.n_stage = t->dose_stages; da.sep_corr = 1;                                // T_hi takes at most 256 TMEM columns: both accumulators always fit
+  da.n_acc = 1;
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
-  k_dose_tc<<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+  if (t->tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+  else k_dose_tc<false><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
   if (cudaGetLastError() != cudaSuccess) return -1;
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
