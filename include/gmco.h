@@ -40,9 +40,11 @@ extern "C" {
 #define GMCO_API
 #endif
 
-#define GMCO_VERSION 110          /* 0.1.1 */
+#define GMCO_VERSION 120          /* 0.1.2 */
 #define GMCO_MAX_STRUCTS 8
 #define GMCO_MAX_HISTORY 16
+#define GMCO_MAX_CRITERIA 8
+#define GMCO_MAX_OBJECTIVES 16
 
 typedef enum gmco_status {
   GMCO_OK = 0,
@@ -170,6 +172,38 @@ GMCO_API int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, 
                 int64_t steps, const int32_t* jdx, const double* z, const double* u, int32_t draws_broadcast,
                 double tau, double temp0, double cooling, int32_t precision, double* T, double* objective,
                 int64_t* n_accepted, void* cuda_stream);
+
+/* One DVH acceptance criterion (RTOG 0924 and the stricter RTOG+ set). */
+typedef struct gmco_criterion {
+  int32_t structure;      /* index into the structure table: the criterion reads dvh[k][structure]               */
+  int32_t sense;          /* +1: index >= limit (target coverage, V100 >= 90 %);  -1: index < limit (D10 < 118 %) */
+  float limit_rtog;       /* in the units of that DVH index (the caller turns "1 cc" into % of the organ's points) */
+  float limit_rtog_plus;  /* RTOG+ differs from RTOG only in the target coverage (95 %)                           */
+  int32_t role;           /* 0 target: its index ranks the valid plans (highest wins)
+                             1 must hold for a fallback plan (urethra)
+                             2 organ at risk whose indices are summed to rank the fallback plans (bladder, rectum) */
+} gmco_criterion;
+
+/* Plan evaluation and selection from a pool (readings A22-A23).
+ * dvh: [K][n_structs] as written by gmco_result (host or device).  Class of a plan: 2 = meets every RTOG+ limit,
+ * 1 = meets every RTOG limit, 0 = violates at least one.  Selected plan, in descending priority: the RTOG+ plan
+ * with the highest target index; else the RTOG plan with the highest target index; else, among the plans that meet
+ * the RTOG limits of roles 0 and 1 (all plans if there is none), the one with the lowest sum of the role-2 indices
+ * (fp32, summed in criterion order).  Ties go to the lowest plan index.
+ * Outputs (host or device, any may be NULL): plan_class [K]; selected [1] (-1 if K = 0);
+ * class_counts [3] = plans of class 0, 1, 2.  Enqueues on cuda_stream and synchronises it. */
+GMCO_API int gmco_select_plan(gmco_handle* h, const float* dvh, int32_t K, const gmco_criterion* criteria,
+                     int32_t n_criteria, int32_t* plan_class, int32_t* selected, int32_t* class_counts,
+                     void* cuda_stream);
+
+/* Pareto filter: plan a dominates plan b if objectives[a][m] <= objectives[b][m] for every m and
+ * < for at least one m; a plan is non-dominated if no plan dominates it (equal plans do not dominate each other).
+ * objectives: [K][M] fp32, every column minimised, 1 <= M <= GMCO_MAX_OBJECTIVES (host or device) -- e.g.
+ * gmco_result's objective_terms viewed as [K][2 n_structs].  Outputs (host or device, any may be NULL):
+ * nondominated [K] bytes (1 / 0); n_nondominated [1].  NaN compares false both ways: a plan with a NaN objective
+ * neither dominates nor is dominated.  Enqueues on cuda_stream and synchronises it. */
+GMCO_API int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t K, int32_t M,
+                      uint8_t* nondominated, int32_t* n_nondominated, void* cuda_stream);
 
 /* Counters of the last optimise/result pair.  GMCO_E_STATE before the first gmco_result. */
 GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);

@@ -169,3 +169,61 @@ def sa_chain(D, structures, w, T0, tau, jdx, z, u, temp0=1.0, cooling=0.995, wan
                        _p(jdx, C.c_int32), _p(z), _p(u), C.c_double(temp0), C.c_double(cooling),
                        _p(t), _p(d), C.byref(F), C.byref(na))
     return dict(t=t, dose=d, F=F.value, n_accepted=na.value)
+
+
+def pareto_front(objectives):
+    """Non-dominated plans (a solution is Pareto optimal "if no solution that improves any individual
+    objective value without worsening at least one of the other individual objective values exists").
+    objectives [K, M], every column minimised.  The definition written out as a double loop: plan a dominates plan b
+    if a_m <= b_m for every m and a_m < b_m for at least one m.  Comparisons only, on the fp32 values as given."""
+    obj = np.asarray(objectives, dtype=np.float32).reshape(len(objectives), -1)
+    K = obj.shape[0]
+    nondom = np.ones(K, dtype=bool)
+    for b in range(K):
+        for a in range(K):
+            if np.all(obj[a] <= obj[b]) and np.any(obj[a] < obj[b]):
+                nondom[b] = False
+                break
+    return nondom
+
+
+def select_plan(dvh, criteria):
+    """Plan evaluation and selection (PAPER.md:132-143 criteria; PAPER.md:147-151 selection; A22-A23).
+    dvh [K, S]; criteria: sequence of (structure, sense, limit_rtog, limit_rtog_plus, role) with sense +1 ("index >=
+    limit") or -1 ("index < limit") and role 0 target / 1 must-hold / 2 organ at risk.
+    Returns (selected index or -1, plan_class [K] with 2 = RTOG+, 1 = RTOG, 0 = invalid, class_counts [3]).
+    fp32 comparisons; the fallback's sum of the role-2 indices is an fp32 sum in criterion order."""
+    dvh = np.asarray(dvh, dtype=np.float32)
+    K = dvh.shape[0]
+    cls = np.zeros(K, dtype=np.int32)
+    target = np.zeros(K, dtype=np.float32); oar = np.zeros(K, dtype=np.float32); core = np.ones(K, dtype=bool)
+    for k in range(K):
+        rtog = plus = True
+        s = np.float32(0.0)
+        for (st, sense, lim, lim_plus, role) in criteria:
+            v = dvh[k, st]
+            ok = (v >= np.float32(lim)) if sense > 0 else (v < np.float32(lim))
+            okp = (v >= np.float32(lim_plus)) if sense > 0 else (v < np.float32(lim_plus))
+            rtog = rtog and ok
+            plus = plus and okp
+            if role == 0:
+                target[k] = v
+            if role != 2:
+                core[k] = core[k] and ok
+            if role == 2:
+                s = np.float32(s + v)
+        oar[k] = s
+        cls[k] = 2 if (rtog and plus) else (1 if rtog else 0)
+    counts = np.array([(cls == 0).sum(), (cls == 1).sum(), (cls == 2).sum()], dtype=np.int32)
+    if K == 0:
+        return -1, cls, counts
+
+    def argbest(mask, key):                 # highest key, ties to the lowest index
+        idx = np.flatnonzero(mask)
+        return int(idx[np.argmax(key[idx])]) if idx.size else -1   # np.argmax returns the first maximum
+
+    for mask, key in ((cls == 2, target), (cls >= 1, target), (core, -oar), (np.ones(K, bool), -oar)):
+        sel = argbest(mask, key)
+        if sel >= 0:
+            return sel, cls, counts
+    return -1, cls, counts

@@ -28,6 +28,11 @@ class Options(C.Structure):
                 ("precision", C.c_int32), ("eps_f", C.c_float), ("reserved", C.c_int32 * 2)]
 
 
+class Criterion(C.Structure):
+    _fields_ = [("structure", C.c_int32), ("sense", C.c_int32), ("limit_rtog", C.c_float),
+                ("limit_rtog_plus", C.c_float), ("role", C.c_int32)]
+
+
 class Stats(C.Structure):
     _fields_ = [("device_bytes", C.c_int64), ("rounds", C.c_int32), ("kernel_launches", C.c_int32),
                 ("plans_iters", C.c_int32), ("plans_converged", C.c_int32), ("plans_stalled", C.c_int32),
@@ -62,6 +67,8 @@ def lib():
         L.gmco_evaluate.argtypes = [vp, fp, i32, fp, i32, fp, fp, fp, vp]
         L.gmco_sa_run.argtypes = [vp, fp, i32, fp, i32, i64, vp, vp, vp, i32, C.c_double, C.c_double, C.c_double,
                                   i32, vp, vp, vp, vp]
+        L.gmco_select_plan.argtypes = [vp, fp, i32, C.POINTER(Criterion), i32, vp, vp, vp, vp]
+        L.gmco_pareto_front.argtypes = [vp, fp, i32, i32, vp, vp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.gmco_set_profiling.argtypes = [vp, i32]
         L.gmco_destroy.argtypes = [vp]
@@ -219,6 +226,27 @@ def gmco_sa_run(h: Handle, T0, weights, jdx, z, u, tau: float, temp0: float = 1.
                              float(tau), float(temp0), float(cooling), int(precision), _ptr(T), _ptr(F), _ptr(na),
                              _stream(stream)), h)
     return dict(T=T, objective=F, n_accepted=na)
+
+
+def gmco_select_plan(h: Handle, dvh, criteria, stream=None) -> dict:
+    """criteria: sequence of (structure, sense, limit_rtog, limit_rtog_plus, role).  Returns dict(selected, plan_class
+    [K] int32 numpy, class_counts [3])."""
+    dvh = _f32(dvh)
+    K = int(dvh.shape[0])
+    arr = (Criterion * len(criteria))(*[Criterion(int(c[0]), int(c[1]), float(c[2]), float(c[3]), int(c[4])) for c in criteria])
+    cls = np.empty(K, np.int32); sel = np.empty(1, np.int32); cnt = np.empty(3, np.int32)
+    _check(lib().gmco_select_plan(h.ptr, _ptr(dvh), K, arr, len(criteria), _ptr(cls), _ptr(sel), _ptr(cnt),
+                                  _stream(stream)), h)
+    return dict(selected=int(sel[0]), plan_class=cls, class_counts=cnt)
+
+
+def gmco_pareto_front(h: Handle, objectives, stream=None) -> dict:
+    """objectives [K][M] (every column minimised).  Returns dict(nondominated [K] bool numpy, n_nondominated)."""
+    obj = _f32(objectives)
+    K = int(obj.shape[0]); M = int(np.prod(obj.shape[1:])) if K else int(np.prod(obj.shape[1:]) or 1)
+    mask = np.empty(K, np.uint8); n = np.empty(1, np.int32)
+    _check(lib().gmco_pareto_front(h.ptr, _ptr(obj), K, M, _ptr(mask), _ptr(n), _stream(stream)), h)
+    return dict(nondominated=mask.astype(bool), n_nondominated=int(n[0]))
 
 
 def gmco_get_stats(h: Handle) -> dict:

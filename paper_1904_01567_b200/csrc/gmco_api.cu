@@ -326,6 +326,19 @@ int copy_inputs(gmco_handle* h, const float* T0, int bcast, const float* w, int 
 
 }  // namespace
 
+namespace {
+// stage a host array on the device (stream-ordered scratch), or pass a device pointer through
+template <class T>
+int stage_in(gmco_handle* h, const T* src, size_t n, T** scratch, const T** dev, cudaStream_t st) {
+  *scratch = nullptr;
+  if (is_device_ptr(src)) { *dev = src; return GMCO_OK; }
+  CK(h, cudaMallocAsync(reinterpret_cast<void**>(scratch), n * sizeof(T), st));
+  CK(h, cudaMemcpyAsync(*scratch, src, n * sizeof(T), cudaMemcpyHostToDevice, st));
+  *dev = *scratch;
+  return GMCO_OK;
+}
+}  // namespace
+
 extern "C" {
 
 int gmco_version(void) { return GMCO_VERSION; }
@@ -719,6 +732,72 @@ int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, const flo
   CK(h, cudaStreamSynchronize(st));
   if (h->host_flags[3] & 1) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
   if (h->host_flags[3] & 2) return fail(h, GMCO_E_INVALID, "jdx holds an index outside [0, n_dwell)%s");
+  return GMCO_OK;
+}
+
+int gmco_select_plan(gmco_handle* h, const float* dvh, int32_t K, const gmco_criterion* criteria, int32_t n_criteria,
+                     int32_t* plan_class, int32_t* selected, int32_t* class_counts, void* cuda_stream) {
+  if (!h) return GMCO_E_INVALID;
+  if (K < 0 || n_criteria < 1 || n_criteria > GMCO_MAX_CRITERIA || !criteria)
+    return fail(h, GMCO_E_INVALID, "K < 0, or n_criteria outside 1..GMCO_MAX_CRITERIA, or criteria is NULL%s");
+  SelectArgs sa{};
+  sa.n = n_criteria;
+  int n_target = 0;
+  for (int i = 0; i < n_criteria; ++i) {
+    const gmco_criterion& q = criteria[i];
+    if (q.structure < 0 || q.structure >= h->c.S || (q.sense != 1 && q.sense != -1) || q.role < 0 || q.role > 2 ||
+        isnan(q.limit_rtog) || isnan(q.limit_rtog_plus))
+      return fail(h, GMCO_E_INVALID, "criterion with a bad structure index, sense, role or limit%s");
+    n_target += q.role == 0;
+    sa.structure[i] = q.structure; sa.sense[i] = q.sense; sa.role[i] = q.role;
+    sa.limit_rtog[i] = q.limit_rtog; sa.limit_plus[i] = q.limit_rtog_plus;
+  }
+  if (n_target != 1) return fail(h, GMCO_E_INVALID, "exactly one criterion must have role 0 (target)%s");
+  int host_out[4] = {-1, 0, 0, 0};
+  if (K > 0) {
+    if (!dvh) return fail(h, GMCO_E_INVALID, "dvh is NULL%s");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float* scr = nullptr; const float* ddvh = nullptr;
+    int rc = stage_in(h, dvh, (size_t)K * h->c.S, &scr, &ddvh, st);
+    if (rc) return rc;
+    int* dout = nullptr;
+    CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dout), ((size_t)K + 4) * sizeof(int), st));
+    h->launches = 0;
+    LN(h, launch_select(ddvh, K, h->c.S, sa, plan_class ? dout + 4 : nullptr, dout, st));
+    CK(h, cudaMemcpyAsync(host_out, dout, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (plan_class) CK(h, cudaMemcpyAsync(plan_class, dout + 4, (size_t)K * sizeof(int), cudaMemcpyDefault, st));
+    cudaFreeAsync(dout, st);
+    if (scr) cudaFreeAsync(scr, st);
+    CK(h, cudaStreamSynchronize(st));
+  }
+  if (selected) CK(h, cudaMemcpy(selected, host_out, sizeof(int), cudaMemcpyDefault));
+  if (class_counts) CK(h, cudaMemcpy(class_counts, host_out + 1, 3 * sizeof(int), cudaMemcpyDefault));
+  return GMCO_OK;
+}
+
+int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t K, int32_t M, uint8_t* nondominated,
+                      int32_t* n_nondominated, void* cuda_stream) {
+  if (!h) return GMCO_E_INVALID;
+  if (K < 0 || M < 1 || M > GMCO_MAX_OBJECTIVES) return fail(h, GMCO_E_INVALID, "K < 0 or M outside 1..GMCO_MAX_OBJECTIVES%s");
+  int host_n = 0;
+  if (K > 0) {
+    if (!objectives) return fail(h, GMCO_E_INVALID, "objectives is NULL%s");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float* scr = nullptr; const float* dobj = nullptr;
+    int rc = stage_in(h, objectives, (size_t)K * M, &scr, &dobj, st);
+    if (rc) return rc;
+    unsigned char* dmask = nullptr;
+    CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dmask), (size_t)K + 16, st));
+    int* dcount = reinterpret_cast<int*>(dmask + (((size_t)K + 3) & ~size_t(3)));
+    h->launches = 0;
+    LN(h, launch_pareto(dobj, K, M, dmask, dcount, st));
+    CK(h, cudaMemcpyAsync(&host_n, dcount, sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (nondominated) CK(h, cudaMemcpyAsync(nondominated, dmask, (size_t)K, cudaMemcpyDefault, st));
+    cudaFreeAsync(dmask, st);
+    if (scr) cudaFreeAsync(scr, st);
+    CK(h, cudaStreamSynchronize(st));
+  }
+  if (n_nondominated) CK(h, cudaMemcpy(n_nondominated, &host_n, sizeof(int), cudaMemcpyDefault));
   return GMCO_OK;
 }
 

@@ -120,6 +120,15 @@ size_t sa_smem_bytes(const CaseDev& c, int precision, int ppt);
 int sa_points_per_thread(const CaseDev& c);
 int launch_sa_chains(const CaseDev& c, const SaArgs& a, int K, int precision, cudaStream_t st);
 
+// plan-pool post-processing (kernels_pool.cu)
+struct SelectArgs {
+  int n;
+  int structure[GMCO_MAX_CRITERIA], sense[GMCO_MAX_CRITERIA], role[GMCO_MAX_CRITERIA];
+  float limit_rtog[GMCO_MAX_CRITERIA], limit_plus[GMCO_MAX_CRITERIA];
+};
+int launch_pareto(const float* obj, int K, int M, unsigned char* nondom, int* count, cudaStream_t st);
+int launch_select(const float* dvh, int K, int S, const SelectArgs& c, int* plan_class, int* out, cudaStream_t st);
+
 // tensor path (kernel_fused_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,

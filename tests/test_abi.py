@@ -23,7 +23,8 @@ def _declared_functions():
 def test_header_declares_the_three_calls_of_the_north_star():
     names = _declared_functions()
     for required in ("gmco_create", "gmco_optimize", "gmco_result", "gmco_evaluate", "gmco_destroy",
-                     "gmco_last_error", "gmco_version", "gmco_default_options", "gmco_get_stats", "gmco_sa_run"):
+                     "gmco_last_error", "gmco_version", "gmco_default_options", "gmco_get_stats", "gmco_sa_run", "gmco_select_plan",
+                     "gmco_pareto_front"):
         assert required in names
 
 
@@ -35,7 +36,7 @@ def test_library_exports_every_declared_symbol(built_lib):
 
 def test_version_and_default_options(built_lib):
     import paper_1904_01567_b200 as g
-    assert g.gmco_version() == 110
+    assert g.gmco_version() == 120
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
@@ -44,6 +45,7 @@ def test_version_and_default_options(built_lib):
 def test_struct_layouts_match_the_header(built_lib):
     import paper_1904_01567_b200.binding as b
     assert ctypes.sizeof(b._Structure) == 28 and ctypes.sizeof(b.Options) == 32 and ctypes.sizeof(b.Stats) == 40
+    assert ctypes.sizeof(b.Criterion) == 20
 
 
 def test_argument_errors_are_reported_without_a_gpu(built_lib):
