@@ -45,6 +45,7 @@ extern "C" {
 #define GMCO_MAX_HISTORY 16
 #define GMCO_MAX_CRITERIA 8
 #define GMCO_MAX_OBJECTIVES 16
+#define GMCO_MAX_RADIAL_COEF 8
 
 typedef enum gmco_status {
   GMCO_OK = 0,
@@ -172,6 +173,18 @@ GMCO_API int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, 
                 int64_t steps, const int32_t* jdx, const double* z, const double* u, int32_t draws_broadcast,
                 double tau, double temp0, double cooling, int32_t precision, double* T, double* objective,
                 int64_t* n_accepted, void* cuda_stream);
+
+/* Step (i) -- the dose-rate matrix ("dose rate matrix calculation (repeated for N_pnt dose calculation
+ * points x N_act dwell positions)"; the model is BASELINE.json configs[0]'s TG-43 point-source approximation):
+ *   D[i][l] = sk_lambda * g(r) / r^2,   r = |points[i] - dwell[l]| / 10 (mm -> cm), r = max(r, r_floor_cm),
+ *   g(r) = sum_c g_coef[c] r^c  (radial dose function as a polynomial in r [cm]; coefficients are inputs).
+ * points [n_points][3], dwell [n_dwell][3]: fp32 millimetres (host or device); g_coef: HOST array of n_coef
+ * (1..GMCO_MAX_RADIAL_COEF) doubles, lowest power first; D: [n_points][ldD] fp32, ldD >= n_dwell (host or device),
+ * Gy/s per unit dwell weight.  fp64 arithmetic, rounded once to fp32.  Needs no handle; errors are reported through
+ * gmco_last_error(NULL).  Enqueues on cuda_stream; synchronises it if any argument is a host pointer. */
+GMCO_API int gmco_dose_rate_matrix(const float* points, int64_t n_points, const float* dwell, int64_t n_dwell,
+                          const double* g_coef, int32_t n_coef, double sk_lambda, double r_floor_cm, float* D,
+                          int64_t ldD, void* cuda_stream);
 
 /* One DVH acceptance criterion (RTOG 0924 and the stricter RTOG+ set). */
 typedef struct gmco_criterion {

@@ -227,3 +227,16 @@ def select_plan(dvh, criteria):
         if sel >= 0:
             return sel, cls, counts
     return -1, cls, counts
+
+
+def dose_rate_matrix(points_mm, dwell_mm, g_coef, sk_lambda, r_floor_cm):
+    """Step (i): D [N, A] fp32 from point and dwell coordinates in mm (orc_dose_rate)."""
+    p = _f32(points_mm).reshape(-1, 3); q = _f32(dwell_mm).reshape(-1, 3)
+    coef = np.ascontiguousarray(g_coef, dtype=np.float64)
+    D = np.empty((p.shape[0], q.shape[0]), np.float32)
+    rc = lib().orc_dose_rate(_p(p, C.c_float), C.c_int64(p.shape[0]), _p(q, C.c_float), C.c_int64(q.shape[0]),
+                             _p(coef), C.c_int32(coef.size), C.c_double(sk_lambda), C.c_double(r_floor_cm),
+                             _p(D, C.c_float))
+    if rc != 0:
+        raise ValueError("orc_dose_rate: bad arguments")
+    return D

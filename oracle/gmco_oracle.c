@@ -393,3 +393,28 @@ int orc_sa_chain(const float* D, int64_t N, int64_t A, const orc_struct* st, int
   free(t); free(d); free(dn);
   return 0;
 }
+
+/* ------------------------------------------------------------------------------------
+ * Step (i): dose-rate matrix (PAPER.md:97 names the step; the model is BASELINE.json configs[0]'s TG-43
+ * point-source approximation, A14-A15):  D_il = sk_lambda g(r) / r^2,  r = |p_i - q_l| in cm floored at
+ * r_floor,  g(r) = sum_c coef[c] r^c.  Plain loops, fp64, one rounding to fp32.
+ * Pins (tests/test_oracle_doserate.py): D = sk_lambda g(1) at r = 1 cm exactly; inverse-square law with g = 1;
+ * the floor; translation / rotation invariance; the numpy recipe of gmco_cases (independent code).            */
+int orc_dose_rate(const float* pts /* [N][3] mm */, int64_t N, const float* dwell /* [A][3] mm */, int64_t A,
+                  const double* coef, int32_t n_coef, double sk_lambda, double r_floor_cm, float* D /* [N][A] */) {
+  if (n_coef < 1 || r_floor_cm <= 0.0) return -1;
+  for (int64_t i = 0; i < N; ++i)
+    for (int64_t l = 0; l < A; ++l) {
+      double r2 = 0.0;
+      for (int a = 0; a < 3; ++a) {
+        const double d = ((double)pts[3 * i + a] - (double)dwell[3 * l + a]) / 10.0;
+        r2 += d * d;
+      }
+      double r = sqrt(r2);
+      if (r < r_floor_cm) r = r_floor_cm;
+      double g = 0.0, rp = 1.0;
+      for (int32_t c = 0; c < n_coef; ++c) { g += coef[c] * rp; rp *= r; }      /* the polynomial as written */
+      D[i * A + l] = (float)(sk_lambda * g / (r * r));
+    }
+  return 0;
+}

@@ -67,6 +67,7 @@ def lib():
         L.gmco_evaluate.argtypes = [vp, fp, i32, fp, i32, fp, fp, fp, vp]
         L.gmco_sa_run.argtypes = [vp, fp, i32, fp, i32, i64, vp, vp, vp, i32, C.c_double, C.c_double, C.c_double,
                                   i32, vp, vp, vp, vp]
+        L.gmco_dose_rate_matrix.argtypes = [fp, i64, fp, i64, C.POINTER(C.c_double), i32, C.c_double, C.c_double, fp, i64, vp]
         L.gmco_select_plan.argtypes = [vp, fp, i32, C.POINTER(Criterion), i32, vp, vp, vp, vp]
         L.gmco_pareto_front.argtypes = [vp, fp, i32, i32, vp, vp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -226,6 +227,21 @@ def gmco_sa_run(h: Handle, T0, weights, jdx, z, u, tau: float, temp0: float = 1.
                              float(tau), float(temp0), float(cooling), int(precision), _ptr(T), _ptr(F), _ptr(na),
                              _stream(stream)), h)
     return dict(T=T, objective=F, n_accepted=na)
+
+
+def gmco_dose_rate_matrix(points_mm, dwell_mm, g_coef, sk_lambda: float, r_floor_cm: float, host: bool = False, stream=None):
+    """Step (i): D [N, A] fp32 (device tensor, or numpy when host=True) from coordinates in millimetres."""
+    p, q = _f32(points_mm), _f32(dwell_mm)
+    N, A = int(p.shape[0]), int(q.shape[0])
+    coef = (C.c_double * len(g_coef))(*[float(c) for c in g_coef])
+    if host:
+        D = np.empty((N, A), np.float32)
+    else:
+        import torch
+        D = torch.empty((N, A), dtype=torch.float32, device="cuda")
+    _check(lib().gmco_dose_rate_matrix(_ptr(p), N, _ptr(q), A, coef, len(g_coef), float(sk_lambda), float(r_floor_cm),
+                                       _ptr(D), A, _stream(stream)))
+    return D
 
 
 def gmco_select_plan(h: Handle, dvh, criteria, stream=None) -> dict:

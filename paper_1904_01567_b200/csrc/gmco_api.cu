@@ -735,6 +735,44 @@ int gmco_sa_run(gmco_handle* h, const float* T0, int32_t t0_broadcast, const flo
   return GMCO_OK;
 }
 
+int gmco_dose_rate_matrix(const float* points, int64_t n_points, const float* dwell, int64_t n_dwell,
+                          const double* g_coef, int32_t n_coef, double sk_lambda, double r_floor_cm, float* D, int64_t ldD,
+                          void* cuda_stream) {
+  gmco_handle* h = nullptr;                           // errors go to the create-error slot
+  if (n_points < 0 || n_dwell < 0 || n_dwell > (1 << 20) || ldD < n_dwell || n_coef < 1 || n_coef > GMCO_MAX_RADIAL_COEF ||
+      !g_coef || !(sk_lambda >= 0.0) || !(r_floor_cm > 0.0) || isinf(sk_lambda) || isinf(r_floor_cm))
+    return fail(h, GMCO_E_INVALID, "bad sizes, ldD < n_dwell, n_coef outside 1..GMCO_MAX_RADIAL_COEF, or r_floor_cm <= 0%s");
+  if (n_points == 0 || n_dwell == 0) return GMCO_OK;
+  if (!points || !dwell || !D) return fail(h, GMCO_E_INVALID, "points, dwell or D is NULL%s");
+  DoseRateArgs m{};
+  for (int c = 0; c < n_coef; ++c) { if (isnan(g_coef[c]) || isinf(g_coef[c])) return fail(h, GMCO_E_INVALID, "g_coef not finite%s"); m.coef[c] = g_coef[c]; }
+  m.n_coef = n_coef; m.sk_lambda = sk_lambda; m.r_floor_cm = r_floor_cm;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  float *sp = nullptr, *sq = nullptr, *dD = D;
+  const float *dp = nullptr, *dq = nullptr;
+  const bool D_host = !is_device_ptr(D);
+  auto body = [&]() -> int {
+    int rc = stage_in(h, points, (size_t)n_points * 3, &sp, &dp, st);
+    if (!rc) rc = stage_in(h, dwell, (size_t)n_dwell * 3, &sq, &dq, st);
+    if (rc) return rc;
+    long long ld = ldD;
+    if (D_host) { CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dD), (size_t)n_points * n_dwell * sizeof(float), st)); ld = n_dwell; }
+    if (launch_dose_rate(dp, n_points, dq, (int)n_dwell, m, dD, ld, st) < 0)
+      return fail(h, GMCO_E_CUDA, "k_dose_rate: %s", cudaGetErrorString(cudaGetLastError()));
+    if (D_host)
+      CK(h, cudaMemcpy2DAsync(D, (size_t)ldD * sizeof(float), dD, (size_t)n_dwell * sizeof(float),
+                              (size_t)n_dwell * sizeof(float), (size_t)n_points, cudaMemcpyDeviceToHost, st));
+    return GMCO_OK;
+  };
+  const int rc = body();
+  if (sp) cudaFreeAsync(sp, st);
+  if (sq) cudaFreeAsync(sq, st);
+  if (D_host && dD != D && dD) cudaFreeAsync(dD, st);
+  if (rc) return rc;
+  if (D_host || sp || sq) CK(h, cudaStreamSynchronize(st));
+  return GMCO_OK;
+}
+
 int gmco_select_plan(gmco_handle* h, const float* dvh, int32_t K, const gmco_criterion* criteria, int32_t n_criteria,
                      int32_t* plan_class, int32_t* selected, int32_t* class_counts, void* cuda_stream) {
   if (!h) return GMCO_E_INVALID;

@@ -120,6 +120,11 @@ size_t sa_smem_bytes(const CaseDev& c, int precision, int ppt);
 int sa_points_per_thread(const CaseDev& c);
 int launch_sa_chains(const CaseDev& c, const SaArgs& a, int K, int precision, cudaStream_t st);
 
+// dose-rate matrix (kernels_doserate.cu)
+struct DoseRateArgs { double coef[GMCO_MAX_RADIAL_COEF]; int n_coef; double sk_lambda, r_floor_cm; };
+int launch_dose_rate(const float* pts, long long N, const float* dwell, int A, const DoseRateArgs& m, float* D,
+                     long long ldD, cudaStream_t st);
+
 // plan-pool post-processing (kernels_pool.cu)
 struct SelectArgs {
   int n;

@@ -24,7 +24,7 @@ def test_header_declares_the_three_calls_of_the_north_star():
     names = _declared_functions()
     for required in ("gmco_create", "gmco_optimize", "gmco_result", "gmco_evaluate", "gmco_destroy",
                      "gmco_last_error", "gmco_version", "gmco_default_options", "gmco_get_stats", "gmco_sa_run", "gmco_select_plan",
-                     "gmco_pareto_front"):
+                     "gmco_pareto_front", "gmco_dose_rate_matrix"):
         assert required in names
 
 
