@@ -97,7 +97,11 @@ typedef struct gmco_options {
                          step that fails Armijo is still accepted when F+ <= F + eps_f |F| and
                          g+.p <= (2 c1 - 1) g.p (Hager & Zhang 2005; reading A5b).
                          0 = Armijo only                                      default 1e-6        */
-  int32_t reserved[2];/* must be 0                                                                */
+  int32_t compaction; /* 1: the tensor route packs the plans that are still running into the leading
+                         128-plan tiles every round, so a round costs what the RUNNING plans cost
+                         (plans stop at different rounds: eps > 0, or unequal numbers of
+                         step halvings); 0: every plan keeps its tile            default 1        */
+  int32_t reserved[1];/* must be 0                                                                */
 } gmco_options;
 
 /* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */
@@ -108,7 +112,7 @@ typedef struct gmco_stats {
   int32_t plans_iters, plans_converged, plans_stalled;
   int32_t eval_launches;    /* profiling only: contraction launches that had work (see gmco_set_profiling) */
   float eval_ms;            /* profiling only: summed device time of those launches, CUDA events  */
-  int32_t reserved[1];
+  int32_t eval_plans;       /* profiling only: plan-evaluations those launches did (running plans, summed over rounds) */
 } gmco_stats;
 
 typedef struct gmco_handle gmco_handle;

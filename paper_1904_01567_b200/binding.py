@@ -25,7 +25,7 @@ class _Structure(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
-                ("precision", C.c_int32), ("eps_f", C.c_float), ("reserved", C.c_int32 * 2)]
+                ("precision", C.c_int32), ("eps_f", C.c_float), ("compaction", C.c_int32), ("reserved", C.c_int32 * 1)]
 
 
 class Criterion(C.Structure):
@@ -36,7 +36,7 @@ class Criterion(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("device_bytes", C.c_int64), ("rounds", C.c_int32), ("kernel_launches", C.c_int32),
                 ("plans_iters", C.c_int32), ("plans_converged", C.c_int32), ("plans_stalled", C.c_int32),
-                ("eval_launches", C.c_int32), ("eval_ms", C.c_float), ("reserved", C.c_int32 * 1)]
+                ("eval_launches", C.c_int32), ("eval_ms", C.c_float), ("eval_plans", C.c_int32)]
 
 
 def lib_path() -> Path:
@@ -124,12 +124,14 @@ def _stream(stream):
     return getattr(stream, "cuda_stream", stream)
 
 
-def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None) -> Options:
+def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None, compaction=None) -> Options:
     o = Options()
     lib().gmco_default_options(C.byref(o))
     o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
     if eps_f is not None:
         o.eps_f = eps_f
+    if compaction is not None:
+        o.compaction = int(compaction)
     return o
 
 

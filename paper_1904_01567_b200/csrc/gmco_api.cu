@@ -139,7 +139,7 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   p.T = a.take<float>(ka); p.T_hi = a.take<float>(ka); p.T_lo = a.take<float>(ka);
   p.Sh = a.take<float>(ka * p.m); p.Yh = a.take<float>(ka * p.m);
   p.rho = a.take<float>(kp * p.m); p.gam = a.take<float>(kp * p.m);
-  p.Weff = a.take<float>(kp * 2 * c.S);
+  p.Weff = a.take<float>(kp * 2 * c.S); p.WeffC = a.take<float>(kp * 2 * c.S); p.slot = a.take<int>(kp);
   p.F = a.take<float>(kp); p.gp = a.take<float>(kp); p.alpha = a.take<float>(kp);
   p.it_done = a.take<int>(kp); p.trials = a.take<int>(kp); p.hcount = a.take<int>(kp); p.hhead = a.take<int>(kp);
   p.status = a.take<int>(kp);
@@ -160,8 +160,9 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
     g_elems = (size_t)ns * ka;
     p.R = a.take<float>(kp * c.N_alloc);
   } else {
-    // upper bound on stream-K segments: one per CTA plus one per plan tile
-    const size_t nseg = (size_t)h->num_sms + p.K_pad / kPlanTile + 1;
+    // one partial slot per CTA of the tensor kernels' grid (plan tiles x point segments)
+    const int n_tiles = p.K_pad / kPlanTile;
+    const size_t nseg = n_tiles > 0 ? (size_t)n_tiles * tc_choose_segs(n_tiles, c.N_pad, h->num_sms) : 1;
     g_elems = nseg * kPlanTile * c.A_pad;
     if (nseg * kPlanTile * 2 > f_elems) f_elems = nseg * kPlanTile * 2;
     p.nG = 0;
@@ -212,7 +213,9 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
     sp.nF = 0; sp.nFcomp = 2; sp.f_slot_stride = 2 * kPlanTile;
     sp.nG = 0; sp.g_slot_stride = (long long)kPlanTile * c.A_pad;
     sp.tile_local = 1; sp.tile_seg = tc_tile_seg_dev(h->tc);
+    if (h->opt.compaction) { sp.compact_cap = tc_compact_cap(h->tc); sp.total_ctas = tc_num_segments(h->tc); }
   }
+  sp.S = c.S;
   return sp;
 }
 
@@ -227,7 +230,7 @@ int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, int* zero_ctr
     LN(h, launch_simt_eval(h->c, h->p, true, dose_dbg, false, nullptr, gate, st));
     LN(h, launch_simt_grad(h->c, h->p, gate, st));
   } else {
-    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, st));
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, gate && h->opt.compaction, st));
   }
   return GMCO_OK;
 }
@@ -346,7 +349,7 @@ int gmco_version(void) { return GMCO_VERSION; }
 void gmco_default_options(gmco_options* o) {
   if (!o) return;
   memset(o, 0, sizeof(*o));
-  o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f;
+  o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f; o->compaction = 1;
 }
 
 const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
@@ -367,7 +370,8 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   if (opt) o = *opt;
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
-      (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || o.reserved[0] || o.reserved[1])
+      (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || (o.compaction != 0 && o.compaction != 1) ||
+      o.reserved[0])
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
   // the plain-fp32 kernels (the paper's largest N_act is 385)
@@ -604,7 +608,7 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
         if (log[r] <= 0) continue;                         // nothing was running: the launch returned at once
         float t = 0.f;
         CK(h, cudaEventElapsedTime(&t, h->ev[2 * r], h->ev[2 * r + 1]));
-        ms += t; s.eval_launches++;
+        ms += t; s.eval_launches++; s.eval_plans += log[r];
       }
       s.eval_ms = (float)ms;
     }
@@ -634,7 +638,8 @@ int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const flo
   if (dose_host) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dose_dev), (size_t)c.N * K * sizeof(float), st));
   rc = enqueue_eval(h, dose_dev, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
-  const StepParams sp = make_step_params(h, 0);
+  StepParams sp = make_step_params(h, 0);
+  sp.compact_cap = 0;                                    // one evaluation of every plan in place: no slots
   float* Fd = F ? h->out_F : nullptr;
   float* gd = grad_x ? h->out_T : nullptr;
   LN(h, launch_eval_finish_scaled(c, p, sp, g_scale_of(h), Fd, gd, st));

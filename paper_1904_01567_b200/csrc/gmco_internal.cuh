@@ -55,6 +55,8 @@ struct PlanDev {
   float *Sh = nullptr, *Yh = nullptr;                              // [m][K_pad][A_pad] history
   float *rho = nullptr, *gam = nullptr;                            // [m][K_pad] 1/(s.y) and (s.y)/(y.y)
   float *Weff = nullptr;                                           // [K_pad][2*S] weights * base / n_s
+  float *WeffC = nullptr;                                          // [K_pad][2*S] the same by tile SLOT (compaction)
+  int *slot = nullptr;                                             // [K_pad] row of the plan in T / R / the partials
   float *F = nullptr, *gp = nullptr, *alpha = nullptr;             // [K_pad]
   int *it_done = nullptr, *trials = nullptr, *hcount = nullptr, *hhead = nullptr, *status = nullptr;
   int *n_running = nullptr;                                        // [2] ping-pong counter of RUNNING plans
@@ -81,6 +83,8 @@ struct StepParams {
   const float* Gpart; int nG; long long g_slot_stride;
   int tile_local;                     // 1: partial rows are indexed by plan % 128 and slots come from tile_seg
   const int* tile_seg;                // [n_tiles + 1] slot range of each plan tile (tensor path)
+  int compact_cap, total_ctas;        // compaction (tensor path): segment cap per tile and CTAs per grid; 0 = off
+  int S;
 };
 
 // ---- kernel launchers (each returns the number of kernels it launched, or < 0 on CUDA error) ----
@@ -140,8 +144,10 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
                        char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
+int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms);
 const int* tc_tile_seg_dev(const TcPlan*);
+int tc_compact_cap(const TcPlan*);
 int launch_tc_eval(const TcPlan* tp, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   int* zero_ctr, int* log_slot, cudaStream_t st);
+                   int* zero_ctr, int* log_slot, bool compact, cudaStream_t st);
 
 }  // namespace gmco

@@ -27,6 +27,8 @@ struct PlanPtrs {
   float *x, *g, *p, *xt, *T, *T_hi, *T_lo, *Sh, *Yh, *rho, *gam, *F, *gp, *alpha;
   int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input;
   int K_pad;
+  float *Weff, *WeffC;        // [K_pad][2S] effective weights by plan / by slot
+  int* slot;                  // [K_pad] row of plan k in T, R and the partials (= k without compaction)
 };
 
 static PlanPtrs make_ptrs(const PlanDev& p) {
@@ -35,6 +37,7 @@ static PlanPtrs make_ptrs(const PlanDev& p) {
   q.Sh = p.Sh; q.Yh = p.Yh; q.rho = p.rho; q.gam = p.gam; q.F = p.F; q.gp = p.gp; q.alpha = p.alpha;
   q.it_done = p.it_done; q.trials = p.trials; q.hcount = p.hcount; q.hhead = p.hhead; q.status = p.status;
   q.n_running = p.n_running; q.bad_input = p.bad_input; q.K_pad = p.K_pad;
+  q.Weff = p.Weff; q.WeffC = p.WeffC; q.slot = p.slot;
   return q;
 }
 
@@ -59,12 +62,13 @@ __global__ void k_init_plans(PlanPtrs pp, int K, int A, int A_pad, int S, const 
     float w = 0.f;
     if (k < K) { w = w_user[(long long)k * 2 * S + j]; if (!(w >= 0.f) || isinf(w)) { bad = 1; w = 0.f; } }
     Weff[(long long)k * 2 * S + j] = w * scale[j];
+    pp.WeffC[(long long)k * 2 * S + j] = w * scale[j];
   }
   if (bad) atomicExch(pp.bad_input, 1);
   if (threadIdx.x == 0) {
     pp.F[k] = 0.f; pp.gp[k] = 0.f; pp.alpha[k] = 1.f;
     pp.it_done[k] = 0; pp.trials[k] = -1;                 // -1: the start point itself is being evaluated
-    pp.hcount[k] = 0; pp.hhead[k] = 0;
+    pp.hcount[k] = 0; pp.hhead[k] = 0; pp.slot[k] = k;
     pp.status[k] = k < K ? PLAN_RUNNING : GMCO_PLAN_ITERS;
     if (k == 0) { pp.n_running[0] = K; pp.n_running[1] = 0; }
   }
@@ -101,10 +105,15 @@ __device__ __forceinline__ void add_slots(const float*& gp, int& s, int g1, long
 }
 
 template <int NPL>
-__device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, int lane, int npl, float (&G)[NPL]) {
+__device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, int lane, int npl, float (&G)[NPL],
+                                                 int row = -1, int n_running = 0) {
   int f0 = 0, f1 = sp.nF, g0 = 0, g1 = sp.nG;
   long long prow = k;
-  if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
+  if (row >= 0) {                                          // compaction: the split the tensor kernels derived (compact_remap)
+    int sa = sp.total_ctas / ((n_running + 127) >> 7);
+    if (sa > sp.compact_cap) sa = sp.compact_cap;
+    f0 = g0 = (row >> 7) * sa; f1 = g1 = f0 + sa; prow = row & 127;
+  } else if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
   const int nfe = (f1 - f0) * sp.nFcomp;                   // SIMT: (lo, hi) pairs per slot
   auto f_at = [&](int i) {
     const int slot = f0 + i / sp.nFcomp, comp = i % sp.nFcomp;
@@ -137,8 +146,10 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
   __shared__ __align__(8) unsigned long long s_bar[4];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int k = blockIdx.x * wpb + warp;
-  if (pp.n_running[parity] == 0) return;
+  const int n_run = pp.n_running[parity];
+  if (n_run == 0) return;
   if (k >= sp.K || pp.status[k] != PLAN_RUNNING) return;
+  const int cur = sp.compact_cap ? pp.slot[k] : -1;            // where this round's partials of the plan are
   const int npl = sp.A_pad >> 5;
   const long long row = (long long)k * sp.A_pad + lane;
   const long long hstride = (long long)pp.K_pad * sp.A_pad;
@@ -188,11 +199,23 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
   int it = pp.it_done[k];
   int hc = pp.hcount[k], hh = pp.hhead[k];
   const float alpha = pp.alpha[k], gp = pp.gp[k];
-  const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G);
+  const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G, cur, n_run);
 #pragma unroll
   for (int j = 0; j < NPL; ++j) gt[j] = g_scale * xt[j] * G[j];   // Eq. 3 summed: g = 2 x o (D^T r)
   int status = PLAN_RUNNING;
   bool new_dir = false;
+  // A plan that goes on to another round counts itself and, with compaction, takes the count as its slot: the running
+  // plans fill rows [0, n_running) of T, and the contraction kernels touch the leading tiles only.  Which slot a plan
+  // gets depends on scheduling; its numbers do not (every row of a tile is summed the same way).
+  auto claim_row = [&]() -> long long {
+    int s = 0;
+    if (lane == 0) s = atomicAdd(&pp.n_running[parity ^ 1], 1);
+    if (!sp.compact_cap) return row;
+    s = __shfl_sync(0xffffffffu, s, 0);
+    if (lane == 0) pp.slot[k] = s;
+    if (lane < 2 * sp.S) pp.WeffC[(long long)s * 2 * sp.S + lane] = pp.Weff[(long long)k * 2 * sp.S + lane];
+    return (long long)s * sp.A_pad + lane;
+  };
 
   if (tr < 0) {                                              // start point: nothing to compare against
 #pragma unroll
@@ -251,12 +274,13 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         status = GMCO_PLAN_STALLED;
       } else {
         const float a2 = alpha * 0.5f;
+        const long long trow = claim_row();
 #pragma unroll
         for (int j = 0; j < NPL; ++j)
           if (j < npl) {
             const float pv = pp.p[row + 32 * j];
             const float xn = fmaf(a2, pv, x[j]), t = xn * xn, hi = tf32_rn_(t);
-            pp.xt[row + 32 * j] = xn; pp.T[row + 32 * j] = t; pp.T_hi[row + 32 * j] = hi; pp.T_lo[row + 32 * j] = tf32_rn_(t - hi);
+            pp.xt[row + 32 * j] = xn; pp.T[trow + 32 * j] = t; pp.T_hi[trow + 32 * j] = hi; pp.T_lo[trow + 32 * j] = tf32_rn_(t - hi);
           }
         if (lane == 0) { pp.alpha[k] = a2; pp.trials[k] = tr; }
       }
@@ -325,22 +349,20 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         for (int j = 0; j < NPL; ++j) { q[j] = g[j] * inv; gpn = fmaf(g[j], -q[j], gpn); }
         gpn = warp_sum(gpn);
       }
+      const long long trow = claim_row();
 #pragma unroll
       for (int j = 0; j < NPL; ++j)
         if (j < npl) {
           const float pv = -q[j];
           const float xn = x[j] + pv, t = xn * xn, hi = tf32_rn_(t);
           pp.p[row + 32 * j] = pv; pp.xt[row + 32 * j] = xn;
-          pp.T[row + 32 * j] = t; pp.T_hi[row + 32 * j] = hi; pp.T_lo[row + 32 * j] = tf32_rn_(t - hi);
+          pp.T[trow + 32 * j] = t; pp.T_hi[trow + 32 * j] = hi; pp.T_lo[trow + 32 * j] = tf32_rn_(t - hi);
         }
       if (lane == 0) { pp.gp[k] = gpn; pp.alpha[k] = 1.f; pp.trials[k] = 0; }
     }
     if (lane == 0) { pp.F[k] = F; pp.it_done[k] = it; pp.hcount[k] = hc; pp.hhead[k] = hh; }
   }
-  if (lane == 0) {
-    if (status == PLAN_RUNNING) atomicAdd(&pp.n_running[parity ^ 1], 1);
-    else pp.status[k] = status;
-  }
+  if (lane == 0 && status != PLAN_RUNNING) pp.status[k] = status;
   hist_wait();
 }
 

@@ -231,14 +231,29 @@ struct DoseArgs {
   int* zero_ctr;              // start-of-round bookkeeping, done by CTA (0, 0): *zero_ctr = 0, *log_slot = *gate
   int* log_slot;
   int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, sep_corr, tlo_resident;
+  int compact_cap;            // > 0: plans are packed by slot; the CTAs re-split over the tiles that hold running plans
   Thresholds thr;
 };
 
 struct GradArgs {
   float* Gpart;               // [n_tiles * segs][128][A_pad]
   const int* gate;
-  int A_pad, n_slabs, segs, n_stage;
+  int A_pad, n_slabs, segs, n_stage, compact_cap;
 };
+
+// Compaction (gmco_options.compaction): k_step packs the running plans into slots [0, n_running), so only the first
+// ceil(n_running / 128) tiles hold work.  The grid is fixed (it lives in a captured graph), so its CTAs are re-dealt:
+// with `ta` active tiles every tile gets min(CTAs / ta, cap) point segments.  All tiles get the same split, and the
+// split depends on n_running only, so a plan's sums do not depend on which slot it was given.
+__device__ __forceinline__ bool compact_remap(int n_running, int cap, int& seg, int& tile, int& segs) {
+  const int ta = (n_running + 127) >> 7;
+  const int total = (int)(gridDim.x * gridDim.y);
+  int sa = total / ta;
+  if (sa > cap) sa = cap;
+  const int c = (int)(blockIdx.y * gridDim.x + blockIdx.x);
+  tile = c / sa; seg = c - tile * sa; segs = sa;
+  return tile < ta;
+}
 
 __device__ __forceinline__ float tf32_rn(float v) {
   uint32_t u;
@@ -263,6 +278,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
     if (a.log_slot) *a.log_slot = *a.gate;
   }
   if (a.gate && *a.gate == 0) return;
+  int seg = blockIdx.x, tile = blockIdx.y, segs = a.segs;
+  if (a.compact_cap && !compact_remap(*a.gate, a.compact_cap, seg, tile, segs)) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
@@ -285,8 +302,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int seg = blockIdx.x, tile = blockIdx.y;
-  const int c0 = (int)((long long)seg * a.n_chunks / a.segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / a.segs);
+  const int c0 = (int)((long long)seg * a.n_chunks / segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / segs);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
@@ -552,7 +568,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         }
       }
     }
-    a.Fpart[(((size_t)tile * a.segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
+    a.Fpart[(((size_t)tile * segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
   }
   tc_fence_before();
   __syncthreads();
@@ -569,6 +585,8 @@ __global__ void __launch_bounds__(kThreads, 1)
 k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmD_hi,
           const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
   if (a.gate && *a.gate == 0) return;
+  int seg = blockIdx.x, tile = blockIdx.y, segs = a.segs;
+  if (a.compact_cap && !compact_remap(*a.gate, a.compact_cap, seg, tile, segs)) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem0 = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* smem = smem0 + 1024;                     // [barriers 1 KB | ring | (epilogue row staging may run past the ring)]
@@ -584,8 +602,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int seg = blockIdx.x, tile = blockIdx.y;
-  const int s0 = (int)((long long)seg * a.n_slabs / a.segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / a.segs);
+  const int s0 = (int)((long long)seg * a.n_slabs / segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / segs);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); mbar_init(conv + i, 128); }
@@ -684,7 +701,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
     // Epilogue: thread L owns plan L's row of the tile.  TMEM -> registers -> a padded row in shared memory (the ring is
     // idle by now; pitch A_pad + 4 floats keeps 16 B stores conflict-free) -> ONE bulk asynchronous copy of the whole
     // row (4 A_pad bytes, contiguous in Gpart) per thread.  No cross-thread hand-off: a thread copies what it wrote.
-    float* grow = a.Gpart + (((size_t)tile * a.segs + seg) * 128 + L) * a.A_pad;
+    float* grow = a.Gpart + (((size_t)tile * segs + seg) * 128 + L) * a.A_pad;
     if (s1 > s0) {
       mbar_wait(acc_full, 0);
       tc_fence_after();
@@ -763,13 +780,30 @@ struct TcPlan {
   Thresholds thr{};
 };
 
+// Point segments per plan tile.  Up to num_sms / n_tiles the grid is one wave of CTAs.  With many tiles one wave leaves
+// SMs idle (79 tiles of a 10 000-plan pool: 79 of 148) or unevenly loaded (C4: 32 tiles x 4 = 128 CTAs), so the grid
+// may run to several waves of shorter CTAs when this model says it pays: time ~ waves x (chunks per CTA + 1), the
+// "+ 1" standing for a CTA's prologue and tail (about one 128-point chunk's worth).
+int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms) {
+  const int n_chunks = (n_pad_points + kPC - 1) / kPC;
+  auto cost = [&](int s) {
+    const int waves = (n_tiles * s + num_sms - 1) / num_sms;
+    return waves * ((n_chunks + s - 1) / s + 1);
+  };
+  const int s0 = num_sms / n_tiles > 0 ? num_sms / n_tiles : 1;
+  int best = s0;
+  for (int s = s0 + 1; s <= 36 && s <= n_chunks; ++s)
+    if (cost(s) < cost(best) && 100 * cost(s) < 95 * cost(s0)) best = s;
+  return best;
+}
+
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
                        char* err, int errlen) {
   constexpr int kSmemMax = 227 * 1024;
   if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
   t->n_tiles = p.K_pad / kPlanTile;
-  t->segs = num_sms / t->n_tiles > 0 ? num_sms / t->n_tiles : 1;
+  t->segs = tc_choose_segs(t->n_tiles, c.N_pad, num_sms);
   for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
   const int G = c.A_pad / 32;
   // dose kernel: T_lo resident when it leaves room for >= 2 ring stages, else streamed with every D slab
@@ -818,11 +852,16 @@ void tc_plan_destroy(TcPlan* t) {
 int tc_num_segments(const TcPlan* t) { return t->n_tiles * t->segs; }
 const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
 
+// at least the static split (a single tile keeps all its CTAs), at most 36 segments: k_step reads one gradient partial
+// per segment, two batches of 18 (kernels_lbfgs.cu)
+int tc_compact_cap(const TcPlan* t) { return t->segs > 36 ? t->segs : 36; }
+
 int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   int* zero_ctr, int* log_slot, cudaStream_t st) {
+                   int* zero_ctr, int* log_slot, bool compact, cudaStream_t st) {
   dim3 grid(t->segs, t->n_tiles);
   DoseArgs da{};
-  da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = p.Weff;
+  da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = compact ? p.WeffC : p.Weff;
+  da.compact_cap = compact ? tc_compact_cap(t) : 0;
   da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
   da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
   da.segs = t->segs; da.n_stage = t->dose_stages; da.sep_corr = 1;                                // T_hi takes at most 256 TMEM columns: both accumulators always fit
@@ -833,7 +872,7 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   if (cudaGetLastError() != cudaSuccess) return -1;
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
-  ga.n_stage = t->grad_stages;
+  ga.n_stage = t->grad_stages; ga.compact_cap = da.compact_cap;
   k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
   return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
