@@ -33,7 +33,7 @@ import gmco_cases as gc  # noqa: E402
 METRIC, UNIT = "plans_per_s", "plans/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_dose_tc + one k_grad_tc launch, from the ncu --set full
 # capture summarised in profiles/r1_ncu_full_summary.md (a constant copied from that file, not measured here)
-NCU_TRAFFIC_BYTES = {"C3": int((26.053888 + 3.481600 + 74.337536 + 3.237632) * 1e6)}   # cold-cache capture: ncu flushes L2 per kernel
+NCU_TRAFFIC_BYTES = {"C3": int((26.053888 + 3.508736 + 74.339328 + 4.086272) * 1e6)}   # cold-cache capture: ncu flushes L2 per kernel
 
 
 def env_int(name, default):
@@ -176,7 +176,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4"])
     ap.add_argument("--precision", default="tf32x3", choices=["tf32x3", "simt"])
-    ap.add_argument("--ref-sample", type=int, default=32, help="plans per oracle step (bounded sample)")
+    ap.add_argument("--ref-sample", type=int, default=256, help="plans per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-gsa", action="store_true", help="skip the gSA-vs-gL-BFGS comparison leg (C5)")
     ap.add_argument("--clock-period", type=float, default=0.02, help="seconds between NVML clock samples (0 = off)")
