@@ -214,6 +214,7 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
     sp.nG = 0; sp.g_slot_stride = (long long)kPlanTile * c.A_pad;
     sp.tile_local = 1; sp.tile_seg = tc_tile_seg_dev(h->tc);
     if (h->opt.compaction) { sp.compact_cap = tc_compact_cap(h->tc); sp.total_ctas = tc_num_segments(h->tc); }
+    sp.dose_pair = tc_dose_pair(h->tc);
   }
   sp.S = c.S;
   return sp;

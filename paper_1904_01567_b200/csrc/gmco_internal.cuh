@@ -84,6 +84,7 @@ struct StepParams {
   int tile_local;                     // 1: partial rows are indexed by plan % 128 and slots come from tile_seg
   const int* tile_seg;                // [n_tiles + 1] slot range of each plan tile (tensor path)
   int compact_cap, total_ctas;        // compaction (tensor path): segment cap per tile and CTAs per grid; 0 = off
+  int dose_pair;                      // the objective partials follow the CTA-pair split (kernels_tc.cu compact_remap_pair)
   int S;
 };
 
@@ -144,6 +145,7 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
                        char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
+int tc_dose_pair(const TcPlan*);           // 1: the dose kernel runs as CTA pairs (its compaction split is per tile PAIR)
 int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms);
 const int* tc_tile_seg_dev(const TcPlan*);
 int tc_compact_cap(const TcPlan*);

@@ -110,9 +110,15 @@ __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, in
   int f0 = 0, f1 = sp.nF, g0 = 0, g1 = sp.nG;
   long long prow = k;
   if (row >= 0) {                                          // compaction: the split the tensor kernels derived (compact_remap)
-    int sa = sp.total_ctas / ((n_running + 127) >> 7);
+    const int ta = (n_running + 127) >> 7;
+    int sa = sp.total_ctas / ta;
     if (sa > sp.compact_cap) sa = sp.compact_cap;
-    f0 = g0 = (row >> 7) * sa; f1 = g1 = f0 + sa; prow = row & 127;
+    g0 = (row >> 7) * sa; g1 = g0 + sa; prow = row & 127;
+    if (sp.dose_pair) {                                    // compact_remap_pair: CTA pairs over tile pairs
+      sa = (sp.total_ctas >> 1) / ((ta + 1) >> 1);
+      if (sa > sp.compact_cap) sa = sp.compact_cap;
+    }
+    f0 = (row >> 7) * sa; f1 = f0 + sa;
   } else if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
   const int nfe = (f1 - f0) * sp.nFcomp;                   // SIMT: (lo, hi) pairs per slot
   auto f_at = [&](int i) {

@@ -20,6 +20,7 @@
 // warps 2-5 = epilogue (TMEM lane quadrant = warp_id % 4).  Pipelines are mbarrier rings.
 #include <cudaTypedefs.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -576,6 +577,335 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 }
 
 // ---------------------------------------------------------------------------------------------
+// a2-a4 on tensor cores, CTA-PAIR variant (tcgen05 cta_group::2).  The two CTAs of a cluster (2, 1, 1) own two adjacent
+// plan tiles and the SAME point chunks.  One MMA spans both: M = 256 plans (128 TMEM lanes in each CTA, each CTA's own
+// T_hi in its TMEM and T_lo in its shared memory), N = 128 points whose D slab is split between the two CTAs'
+// shared memories (64 points = 8 KB each).  Every CTA therefore loads HALF of each D slab: the operand stream from L2,
+// which is what kept k_dose_tc off the MMA floor, halves, and the same ring bytes hold twice as many
+// entries.  Only the leader (cluster rank 0) issues MMAs; its `full` barriers collect the bytes of both CTAs' TMA
+// loads, its tg_ready / acc_empty barriers the arrivals of both CTAs' epilogue threads; MMA completion is committed
+// to both CTAs' `empty` / `acc_full` barriers by multicast.  Resident-T_lo layout only (at most 256 dwell positions).
+constexpr int kHalfPC = kPC / 2;
+constexpr int kHalfSlab = kHalfPC * 128;   // 8 KB: 64 points x 32 dwell of one part (hi or lo)
+constexpr int kPairEntry = 2 * kHalfSlab;  // ring entry: TWO dwell groups of a half slab (8 MMAs per barrier round trip:
+                                           // the issuing warp's instruction stream, not the tensor pipe, is the limiter)
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same variable in the pair's leader CTA
+__device__ __forceinline__ uint32_t leader_addr(const void* p) {
+  uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, 0;" : "=r"(r) : "r"(smem_u32(p))); return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {   // acquires remote arrivals
+  uint32_t spins = 0, ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (!ok && ++spins > kWatchdog) __trap();
+  } while (!ok);
+}
+// this CTA's half of a D slab; the bytes are counted on the LEADER's barrier (a shared::cluster address)
+__device__ __forceinline__ void tma_load_3d_pair(const CUtensorMap* map, void* dst, uint32_t leader_bar, int c0, int c1,
+                                                 int c2, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;"
+      ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(leader_bar), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t* dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(dst_smem)), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// completion of all MMAs issued so far arrives on the barrier at this offset in BOTH CTAs of the pair
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void mma_ts2_pair(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc,
+                                             uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 bd;\n\tsetp.ne.b32 p, %5, 0;\n\tmov.b64 bd, {%2, %3};\n\t"
+      "tcgen05.mma.cta_group::2.kind::tf32 [%0], [%1], bd, %4, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc)
+      : "memory");
+}
+__device__ __forceinline__ void mma_ss2_pair(uint32_t d_tmem, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi,
+                                             uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 ad, bd;\n\tsetp.ne.b32 p, %6, 0;\n\tmov.b64 ad, {%1, %2};\n\tmov.b64 bd, {%3, %4};\n\t"
+      "tcgen05.mma.cta_group::2.kind::tf32 [%0], ad, bd, %5, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "r"(acc)
+      : "memory");
+}
+// kind::tf32, fp32 accumulator, M = 256 across the pair
+__host__ __device__ constexpr uint32_t instr_desc_pair(int n) {
+  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+}
+// compaction with pairs: the grid's CTA PAIRS are re-dealt over the active tile pairs (cf. compact_remap)
+__device__ __forceinline__ bool compact_remap_pair(int n_running, int cap, int rank, int& seg, int& tile, int& segs) {
+  const int tap = (((n_running + 127) >> 7) + 1) >> 1;
+  const int total = (int)(gridDim.y * (gridDim.x >> 1));
+  int sa = total / tap;
+  if (sa > cap) sa = cap;
+  const int c = (int)(blockIdx.y * (gridDim.x >> 1) + (blockIdx.x >> 1));
+  const int pt = c / sa;
+  tile = 2 * pt + rank; seg = c - pt * sa; segs = sa;
+  return pt < tap;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kDoseThreads, 1)
+k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
+               const __grid_constant__ CUtensorMap tmT, const DoseArgs a) {
+  if (a.zero_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+    *a.zero_ctr = 0;
+    if (a.log_slot) *a.log_slot = *a.gate;
+  }
+  if (a.gate && *a.gate == 0) return;                 // both CTAs of a pair take every early exit together
+  const int rank = (int)cluster_ctarank();
+  const bool leader = rank == 0;
+  int seg = blockIdx.y, tile = blockIdx.x, segs = a.segs;   // grid (tiles, segs): a 2-CTA MMA pair must be adjacent in x
+  if (a.compact_cap && !compact_remap_pair(*a.gate, a.compact_cap, rank, seg, tile, segs)) return;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int G = a.A_pad >> 5;                         // 32-dwell groups, at most kTmemGroups
+  uint8_t* tlo = smem;                                // T_lo [G][128 plans][128 B]
+  uint8_t* ring = smem + (size_t)G * kTloBox;         // n_stage entries of two half slabs
+  const int ringBytes = a.n_stage * kPairEntry;
+  const int Gp = (G + 1) >> 1;                        // entries per pass over the dwell groups (a missing odd group is zero-filled)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + ringBytes);
+  uint64_t* full = bars;                              // [n_stage]  used in the leader: both CTAs' bytes
+  uint64_t* empty = bars + a.n_stage;                 // [n_stage]  in each CTA: multicast commit
+  uint64_t* tg_ready = bars + 2 * a.n_stage;          // [8]        used in the leader: 256 arrivals (both CTAs)
+  uint64_t* tin_full = tg_ready + kTmemGroups;        // [8]        in each CTA: its own T
+  uint64_t* acc_full = tin_full + kTmemGroups;        // [2]        in each CTA: multicast commit
+  uint64_t* acc_empty = acc_full + 2;                 // [2]        used in the leader: 512 arrivals
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int c0 = (int)((long long)seg * a.n_chunks / segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / segs);
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
+    for (int i = 0; i < kTmemGroups; ++i) { mbar_init(tg_ready + i, 256); mbar_init(tin_full + i, 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 512); }
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT); }
+  if (warp == 1) tmem_alloc_pair(tmem_slot, 512);
+  tc_fence_before();
+  cluster_sync_all();                                 // barriers of both CTAs exist before anything arrives on them
+  tc_fence_after();
+  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+  const uint32_t t_thi = tmem;                        // columns [0, A_pad): T_hi
+  // Two accumulator buffers of 128 points.  ONE accumulator per chunk takes all three products, the small ones first:
+  // the tensor core truncates when it adds into the fp32 accumulator, so T_hi D_lo + T_lo D_hi (2^-11 of the dose) are
+  // summed while the accumulator is still small and the 4 G adds of T_hi D_hi come last -- the same one-sided error as
+  // with k_dose_tc's separate correction accumulator, in half the columns, which is what lets the epilogue of chunk c
+  // overlap the MMAs of chunk c + 1.  The price is a second pass over the chunk's D_hi slabs (3 G ring entries per
+  // chunk instead of 2 G), affordable here because every CTA loads half slabs.
+  const uint32_t t_acc = tmem + G * 32;
+
+  if (warp == 0) {
+    if (c1 > c0) {
+      const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
+      if (elect_one()) {
+        for (int g = 0; g < G; ++g) {
+          mbar_expect_tx(tin_full + g, (uint32_t)kTloBox);
+          tma_load_3d(&tmT, tlo + (size_t)g * kTloBox, tin_full + g, 0, tile * 128, g, polT);
+        }
+      }
+      __syncwarp();
+      const uint32_t lfull0 = leader_addr(full);
+      int st = 0; uint32_t ph = 0;
+      for (int c = c0; c < c1; ++c) {
+        for (int g2 = 0; g2 < 3 * Gp; ++g2) {         // entries 2 p, 2 p + 1: D_lo, D_hi (corrections); 2 Gp + p: D_hi (main)
+          const int gp = g2 < 2 * Gp ? g2 >> 1 : g2 - 2 * Gp, lo = g2 < 2 * Gp ? (g2 & 1) ^ 1 : 0;
+          mbar_wait(empty + st, ph ^ 1);
+          if (elect_one()) {
+            if (leader) mbar_expect_tx(full + st, 2u * (uint32_t)kPairEntry);
+            tma_load_3d_pair(lo ? &tmD_lo : &tmD_hi, ring + (size_t)st * kPairEntry, lfull0 + 8u * (uint32_t)st, 0,
+                             c * kPC + rank * kHalfPC, 2 * gp, polD);
+          }
+          __syncwarp();
+          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (leader && c1 > c0) {
+      constexpr uint32_t idesc = instr_desc_pair(kPC);
+      constexpr uint32_t dhi = desc_hi(1024, kSwz128);
+      const int n_stage = a.n_stage;
+      const uint32_t ring_lo = desc_lo(smem_u32(ring), 16), ring_step = (uint32_t)kPairEntry >> 4;
+      const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
+      const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
+      constexpr uint32_t kG1 = (uint32_t)kHalfSlab >> 4;       // second dwell group of an entry
+      int st = 0; uint32_t ph = 0;
+      for (int c = c0; c < c1; ++c) {
+        const int b = (c - c0) & 1, use = (c - c0) >> 1;
+        mbar_wait_cluster(acc_empty + b, (use & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t acc = t_acc + (uint32_t)b * kPC;
+        uint32_t thi = t_thi, alo = tlo_lo0;
+        for (int gp = 0; gp < Gp; thi += 64, alo += 2 * (kTloBox >> 4), ++gp) {     // corrections first
+          const bool two = 2 * gp + 1 < G;
+          if (c == c0) {
+            mbar_wait_cluster(tg_ready + 2 * gp, 0);
+            if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
+            tc_fence_after();
+          }
+          mbar_wait_addr(full0 + 8 * st, ph);         // D_lo: T_hi D_lo
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+            mma_ts2_pair(acc, thi, bd, dhi, idesc, gp != 0);
+#pragma unroll
+            for (int j = 1; j < 4; ++j) mma_ts2_pair(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+            if (two) {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 32 + 8 * j, bd + kG1 + 2 * j, dhi, idesc, 1);
+            }
+            tc_commit_pair(empty0 + 8 * st);
+          }
+          __syncwarp();
+          if (++st == n_stage) { st = 0; ph ^= 1; }
+          mbar_wait_addr(full0 + 8 * st, ph);         // D_hi: T_lo D_hi
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) mma_ss2_pair(acc, alo + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
+            if (two) {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) mma_ss2_pair(acc, alo + (kTloBox >> 4) + 2 * j, dhi, bd + kG1 + 2 * j, dhi, idesc, 1);
+            }
+            tc_commit_pair(empty0 + 8 * st);
+          }
+          __syncwarp();
+          if (++st == n_stage) { st = 0; ph ^= 1; }
+        }
+        thi = t_thi;
+        for (int gp = 0; gp < Gp; thi += 64, ++gp) {  // then the large product: D_hi again: T_hi D_hi
+          const bool two = 2 * gp + 1 < G;
+          mbar_wait_addr(full0 + 8 * st, ph);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+            if (two) {
+#pragma unroll
+              for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 32 + 8 * j, bd + kG1 + 2 * j, dhi, idesc, 1);
+            }
+            tc_commit_pair(empty0 + 8 * st);
+            if (gp == Gp - 1) tc_commit_pair(smem_u32(acc_full + b));
+          }
+          __syncwarp();
+          if (++st == n_stage) { st = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else {
+    const int e = warp - 2;                           // 0..7
+    const int q = warp & 3;                           // TMEM lane quadrant this warp may access
+    const int h = e >> 2;                             // which 64 of the chunk's 128 points this warp evaluates
+    const int L = q * 32 + lane;                      // lane = plan inside the tile
+    const int plan = tile * 128 + L;
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    float f_lo = 0.f, f_hi = 0.f;
+    if (c1 > c0) {
+      const uint32_t l_tg = leader_addr(tg_ready), l_ae = leader_addr(acc_empty);
+      // prologue: split this CTA's T into tf32 hi (TMEM) and lo (in place), as in k_dose_tc<true>
+      const int row = q * 32 + lane;
+      for (int g = h; g < G; g += 2) {
+        uint8_t* base = tlo + (size_t)g * kTloBox + row * 128;
+        mbar_wait(tin_full + g, 0);
+        uint32_t v[32];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          float4* cell = reinterpret_cast<float4*>(base + ((k ^ (row & 7)) << 4));
+          const float4 t = *cell;
+          float4 hi, lo;
+          hi.x = tf32_rn(t.x); hi.y = tf32_rn(t.y); hi.z = tf32_rn(t.z); hi.w = tf32_rn(t.w);
+          lo.x = tf32_rn(t.x - hi.x); lo.y = tf32_rn(t.y - hi.y); lo.z = tf32_rn(t.z - hi.z); lo.w = tf32_rn(t.w - hi.w);
+          *cell = lo;
+          v[4 * k + 0] = __float_as_uint(hi.x); v[4 * k + 1] = __float_as_uint(hi.y);
+          v[4 * k + 2] = __float_as_uint(hi.z); v[4 * k + 3] = __float_as_uint(hi.w);
+        }
+        tmem_st32(t_thi + lane_base + g * 32, v);
+        tmem_st_wait();
+        tc_fence_before();
+        fence_proxy_async();                          // the lo stores above are read by the MMA (async proxy)
+        mbar_arrive_cluster(l_tg + 8u * (uint32_t)g);
+      }
+
+      int s_n = a.tile_struct[2 * c0 + h], nv_n = a.tile_valid[2 * c0 + h];
+      float wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n], whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
+      for (int c = c0; c < c1; ++c) {
+        const int s = s_n, nv = nv_n;
+        const float wlo = wlo_n, whi = whi_n;
+        if (c + 1 < c1) {
+          s_n = a.tile_struct[2 * (c + 1) + h]; nv_n = a.tile_valid[2 * (c + 1) + h];
+          wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n]; whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
+        }
+        const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
+        const int b = (c - c0) & 1, use = (c - c0) >> 1;
+        mbar_wait(acc_full + b, use & 1);
+        tc_fence_after();
+        uint32_t v[2][32];
+        const uint32_t t_main = t_acc + lane_base + (uint32_t)b * kPC + h * 64;
+        tmem_ld32(t_main, v[0]);
+        tmem_ld32(t_main + 32, v[1]);
+        tmem_ld_wait();
+        tc_fence_before();
+        mbar_arrive_cluster(l_ae + 8u * (uint32_t)b);
+#pragma unroll
+        for (int sub = 0; sub < 2; ++sub) {
+          const int nvh = nv - sub * 32;
+          const size_t p0 = (size_t)c * kPC + h * 64 + sub * 32;
+          float* rp = a.R + p0 * a.K_pad + plan;
+          if (nvh >= 32) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const float d = __uint_as_float(v[sub][j]);
+              rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, f_lo, f_hi);  // = dF/dd / 2
+            }
+          } else {                                                          // ragged tail of a structure
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const float d = __uint_as_float(v[sub][j]);
+              float t_lo = f_lo, t_hi = f_hi;
+              rp[(size_t)j * a.K_pad] = eq2_accumulate<float>(d, dlo, dhi, wlo, whi, t_lo, t_hi);  // padding rows: value unused
+              if (j < nvh) { f_lo = t_lo; f_hi = t_hi; }
+            }
+          }
+          if (a.dose_dbg && plan < a.K) {
+            for (int j = 0; j < 32; ++j) {
+              if (j < nvh) a.dose_dbg[(size_t)a.row_src[p0 + j] * a.K + plan] = __uint_as_float(v[sub][j]);
+            }
+          }
+        }
+      }
+    }
+    a.Fpart[(((size_t)tile * segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
+  }
+  tc_fence_before();
+  cluster_sync_all();                                 // neither CTA's shared memory, TMEM or barriers may go before both are done
+  if (warp == 1) { tc_fence_after(); tmem_dealloc_pair(tmem, 512); }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a5 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point slabs [seg n_slabs / segs, (seg + 1) n_slabs / segs) of PS points each.
 // Stage = [R | R_lo | D_hi | D_lo]: TMA brings R (fp32), D_hi, D_lo; warps 2-5 split R in place into its
@@ -773,6 +1103,8 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long cols,
 struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
+  CUtensorMap pair_D_hi, pair_D_lo;                // 64-point boxes of the CTA-pair dose kernel
+  int dose_pair = 0, pair_stages = 0, pair_smem = 0;
   int segs = 1, n_tiles = 0;
   int dose_stages = 0, dose_smem = 0, tlo_resident = 1;
   int grad_ps = 32, grad_stages = 0, grad_smem = 0;
@@ -832,6 +1164,27 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
             make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
+  // CTA-pair dose kernel: resident layout, an even number of plan tiles (GMCO_DOSE_PAIR=0 keeps the single-CTA kernel)
+  {
+    const char* env = getenv("GMCO_DOSE_PAIR");
+    t->dose_pair = t->tlo_resident && t->n_tiles % 2 == 0 && !(env && env[0] == '0');
+    if (t->dose_pair) {
+      const int fixedp = G * kTloBox + slack;
+      t->pair_stages = (kSmemMax - fixedp) / kPairEntry;
+      if (t->pair_stages > 12) t->pair_stages = 12;
+      t->pair_smem = fixedp + t->pair_stages * kPairEntry;
+      ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
+           make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
+      if (ok && cudaFuncSetAttribute(k_dose_tc_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem) != cudaSuccess) ok = false;
+      if (getenv("GMCO_DEBUG")) {
+        cudaLaunchConfig_t cfg = {}; cfg.gridDim = dim3(t->n_tiles, t->segs); cfg.blockDim = dim3(kDoseThreads); cfg.dynamicSmemBytes = t->pair_smem;
+        int nc = -1; cudaError_t o = cudaOccupancyMaxActiveClusters(&nc, k_dose_tc_pair, &cfg);
+        cudaFuncAttributes fa{}; cudaFuncGetAttributes(&fa, k_dose_tc_pair);
+        fprintf(stderr, "[gmco] pair kernel: grid (%d, %d) smem %d stages %d regs %d static smem %zu clusters %d (%s) ok %d\n", t->segs, t->n_tiles,
+                t->pair_smem, t->pair_stages, fa.numRegs, fa.sharedSizeBytes, nc, cudaGetErrorName(o), (int)ok);
+      }
+    }
+  }
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
   cudaError_t e = t->tlo_resident ? cudaFuncSetAttribute(k_dose_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem)
                                    : cudaFuncSetAttribute(k_dose_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
@@ -850,6 +1203,7 @@ void tc_plan_destroy(TcPlan* t) {
 }
 
 int tc_num_segments(const TcPlan* t) { return t->n_tiles * t->segs; }
+int tc_dose_pair(const TcPlan* t) { return t->dose_pair; }
 const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
 
 // at least the static split (a single tile keeps all its CTAs), at most 36 segments: k_step reads one gradient partial
@@ -867,9 +1221,12 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   da.segs = t->segs; da.n_stage = t->dose_stages; da.sep_corr = 1;                                // T_hi takes at most 256 TMEM columns: both accumulators always fit
   da.n_acc = 1;
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
-  if (t->tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+  if (t->dose_pair) {
+    da.n_stage = t->pair_stages;
+    k_dose_tc_pair<<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
+  } else if (t->tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
   else k_dose_tc<false><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
-  if (cudaGetLastError() != cudaSuccess) return -1;
+  if (cudaPeekAtLastError() != cudaSuccess) return -1;   // left for the caller's message
   GradArgs ga{};
   ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
   ga.n_stage = t->grad_stages; ga.compact_cap = da.compact_cap;
