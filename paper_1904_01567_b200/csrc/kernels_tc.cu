@@ -54,6 +54,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// no memory ordering (the accumulator hand-back: TMEM accesses are ordered by the tcgen05 waits and fences around it)
+__device__ __forceinline__ void mbar_arrive_relaxed(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
@@ -540,7 +544,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           tmem_ld_wait();
         }
         tc_fence_before();
-        mbar_arrive(acc_empty + b);
+        mbar_arrive_relaxed(acc_empty + b);
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
           const int nvh = nv - sub * 32;
@@ -603,6 +607,21 @@ __device__ __forceinline__ uint32_t leader_addr(const void* p) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// The accumulator hand-back orders TMEM accesses only (tcgen05.wait::ld before, tcgen05.fence after): a RELAXED arrive
+// and wait.  A release at cluster scope would first drain the epilogue's outstanding R stores (MEMBAR.ALL.GPU: measured
+// as the epilogue's top stall) and an acquire invalidates L1 on every pass.
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_bar) {
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster_relaxed(uint64_t* bar, uint32_t parity) {
+  uint32_t spins = 0, ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.relaxed.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (!ok && ++spins > kWatchdog) __trap();
+  } while (!ok);
+}
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {   // acquires remote arrivals
   uint32_t spins = 0, ok;
   do {
@@ -664,6 +683,7 @@ __device__ __forceinline__ bool compact_remap_pair(int n_running, int cap, int r
   return pt < tap;
 }
 
+template <int GP, int NS>   // GP > 0: ceil(A_pad / 64) and the ring size are compile-time (static issue schedule); 0: any shape
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kDoseThreads, 1)
 k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
                const __grid_constant__ CUtensorMap tmT, const DoseArgs a) {
@@ -751,68 +771,89 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
       const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
       const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
       constexpr uint32_t kG1 = (uint32_t)kHalfSlab >> 4;       // second dwell group of an entry
-      int st = 0; uint32_t ph = 0;
-      for (int c = c0; c < c1; ++c) {
-        const int b = (c - c0) & 1, use = (c - c0) >> 1;
-        mbar_wait_cluster(acc_empty + b, (use & 1) ^ 1);
+      // One ring entry: wait, 4 or 8 MMAs, commit.  kind 0: T_hi D_lo, 1: T_lo D_hi, 2: T_hi D_hi.
+      auto entry = [&](const int kind, const int gp, const int st, const uint32_t ph, const uint32_t acc, const bool two,
+                       const uint32_t acc_full_bar) {
+        mbar_wait_addr(full0 + 8 * st, ph);
         tc_fence_after();
-        const uint32_t acc = t_acc + (uint32_t)b * kPC;
-        uint32_t thi = t_thi, alo = tlo_lo0;
-        for (int gp = 0; gp < Gp; thi += 64, alo += 2 * (kTloBox >> 4), ++gp) {     // corrections first
-          const bool two = 2 * gp + 1 < G;
-          if (c == c0) {
-            mbar_wait_cluster(tg_ready + 2 * gp, 0);
-            if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
-            tc_fence_after();
-          }
-          mbar_wait_addr(full0 + 8 * st, ph);         // D_lo: T_hi D_lo
-          tc_fence_after();
-          if (elect_one()) {
-            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
-            mma_ts2_pair(acc, thi, bd, dhi, idesc, gp != 0);
-#pragma unroll
-            for (int j = 1; j < 4; ++j) mma_ts2_pair(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
-            if (two) {
-#pragma unroll
-              for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 32 + 8 * j, bd + kG1 + 2 * j, dhi, idesc, 1);
-            }
-            tc_commit_pair(empty0 + 8 * st);
-          }
-          __syncwarp();
-          if (++st == n_stage) { st = 0; ph ^= 1; }
-          mbar_wait_addr(full0 + 8 * st, ph);         // D_hi: T_lo D_hi
-          tc_fence_after();
-          if (elect_one()) {
-            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+        if (elect_one()) {
+          const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+          const uint32_t thi = t_thi + 64 * gp, alo = tlo_lo0 + 2 * (kTloBox >> 4) * gp;
+          if (kind == 1) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) mma_ss2_pair(acc, alo + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
             if (two) {
 #pragma unroll
               for (int j = 0; j < 4; ++j) mma_ss2_pair(acc, alo + (kTloBox >> 4) + 2 * j, dhi, bd + kG1 + 2 * j, dhi, idesc, 1);
             }
-            tc_commit_pair(empty0 + 8 * st);
-          }
-          __syncwarp();
-          if (++st == n_stage) { st = 0; ph ^= 1; }
-        }
-        thi = t_thi;
-        for (int gp = 0; gp < Gp; thi += 64, ++gp) {  // then the large product: D_hi again: T_hi D_hi
-          const bool two = 2 * gp + 1 < G;
-          mbar_wait_addr(full0 + 8 * st, ph);
-          tc_fence_after();
-          if (elect_one()) {
-            const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
+          } else {
+            mma_ts2_pair(acc, thi, bd, dhi, idesc, (kind == 0 && gp == 0) ? 0u : 1u);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
+            for (int j = 1; j < 4; ++j) mma_ts2_pair(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
             if (two) {
 #pragma unroll
               for (int j = 0; j < 4; ++j) mma_ts2_pair(acc, thi + 32 + 8 * j, bd + kG1 + 2 * j, dhi, idesc, 1);
             }
-            tc_commit_pair(empty0 + 8 * st);
-            if (gp == Gp - 1) tc_commit_pair(smem_u32(acc_full + b));
           }
-          __syncwarp();
-          if (++st == n_stage) { st = 0; ph ^= 1; }
+          tc_commit_pair(empty0 + 8 * st);
+          if (acc_full_bar) tc_commit_pair(acc_full_bar);
+        }
+        __syncwarp();
+      };
+      if constexpr (GP > 0) {
+        // Static schedule: 3 GP entries per chunk go round a ring of NS entries a whole number of times, so every
+        // entry's ring slot is a compile-time constant and its phase is one bit toggled per chunk.
+        constexpr int E = 3 * GP, REV = E / NS;
+        static_assert(E % NS == 0, "ring size must divide the entries of a chunk");
+        uint32_t chunk_par = 0;
+        const bool odd = (G & 1) != 0;
+        for (int c = c0; c < c1; ++c) {
+          const int b = (c - c0) & 1, use = (c - c0) >> 1;
+          mbar_wait_cluster_relaxed(acc_empty + b, (use & 1) ^ 1);
+          tc_fence_after();
+          const uint32_t acc = t_acc + (uint32_t)b * kPC;
+#pragma unroll
+          for (int gp = 0; gp < GP; ++gp) {
+            const bool two = gp < GP - 1 || !odd;
+            if (c == c0) {                            // the first chunk overlaps the prologue, group by group
+              mbar_wait_cluster(tg_ready + 2 * gp, 0);
+              if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
+              tc_fence_after();
+            }
+            entry(0, gp, (2 * gp) % NS, chunk_par ^ (((2 * gp) / NS) & 1), acc, two, 0u);
+            entry(1, gp, (2 * gp + 1) % NS, chunk_par ^ (((2 * gp + 1) / NS) & 1), acc, two, 0u);
+          }
+#pragma unroll
+          for (int gp = 0; gp < GP; ++gp) {
+            const bool two = gp < GP - 1 || !odd;
+            entry(2, gp, (2 * GP + gp) % NS, chunk_par ^ (((2 * GP + gp) / NS) & 1), acc, two,
+                  gp == GP - 1 ? smem_u32(acc_full + b) : 0u);
+          }
+          chunk_par ^= (uint32_t)(REV & 1);
+        }
+      } else {
+        int st = 0; uint32_t ph = 0;
+        for (int c = c0; c < c1; ++c) {
+          const int b = (c - c0) & 1, use = (c - c0) >> 1;
+          mbar_wait_cluster_relaxed(acc_empty + b, (use & 1) ^ 1);
+          tc_fence_after();
+          const uint32_t acc = t_acc + (uint32_t)b * kPC;
+          for (int gp = 0; gp < Gp; ++gp) {           // corrections first
+            const bool two = 2 * gp + 1 < G;
+            if (c == c0) {
+              mbar_wait_cluster(tg_ready + 2 * gp, 0);
+              if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
+              tc_fence_after();
+            }
+            entry(0, gp, st, ph, acc, two, 0u);
+            if (++st == n_stage) { st = 0; ph ^= 1; }
+            entry(1, gp, st, ph, acc, two, 0u);
+            if (++st == n_stage) { st = 0; ph ^= 1; }
+          }
+          for (int gp = 0; gp < Gp; ++gp) {           // then the large product: D_hi again
+            entry(2, gp, st, ph, acc, 2 * gp + 1 < G, gp == Gp - 1 ? smem_u32(acc_full + b) : 0u);
+            if (++st == n_stage) { st = 0; ph ^= 1; }
+          }
         }
       }
     }
@@ -869,7 +910,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         tmem_ld32(t_main + 32, v[1]);
         tmem_ld_wait();
         tc_fence_before();
-        mbar_arrive_cluster(l_ae + 8u * (uint32_t)b);
+        mbar_arrive_cluster_relaxed(l_ae + 8u * (uint32_t)b);
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
           const int nvh = nv - sub * 32;
@@ -1104,7 +1145,7 @@ struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
   CUtensorMap pair_D_hi, pair_D_lo;                // 64-point boxes of the CTA-pair dose kernel
-  int dose_pair = 0, pair_stages = 0, pair_smem = 0;
+  int dose_pair = 0, pair_static = 0, pair_stages = 0, pair_smem = 0;
   int segs = 1, n_tiles = 0;
   int dose_stages = 0, dose_smem = 0, tlo_resident = 1;
   int grad_ps = 32, grad_stages = 0, grad_smem = 0;
@@ -1175,11 +1216,15 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
       t->pair_smem = fixedp + t->pair_stages * kPairEntry;
       ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
            make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
-      if (ok && cudaFuncSetAttribute(k_dose_tc_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem) != cudaSuccess) ok = false;
+      // static issue schedule for the production shape (A_pad 193..256: 12 entries per chunk, ring of 6)
+      t->pair_static = (G + 1) / 2 == 4 && t->pair_stages >= 6;
+      if (t->pair_static) { t->pair_stages = 6; t->pair_smem = fixedp + 6 * kPairEntry; }
+      if (ok && (t->pair_static ? cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem)
+                                : cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem)) != cudaSuccess) ok = false;
       if (getenv("GMCO_DEBUG")) {
         cudaLaunchConfig_t cfg = {}; cfg.gridDim = dim3(t->n_tiles, t->segs); cfg.blockDim = dim3(kDoseThreads); cfg.dynamicSmemBytes = t->pair_smem;
-        int nc = -1; cudaError_t o = cudaOccupancyMaxActiveClusters(&nc, k_dose_tc_pair, &cfg);
-        cudaFuncAttributes fa{}; cudaFuncGetAttributes(&fa, k_dose_tc_pair);
+        int nc = -1; cudaError_t o = cudaOccupancyMaxActiveClusters(&nc, k_dose_tc_pair<0, 0>, &cfg);
+        cudaFuncAttributes fa{}; cudaFuncGetAttributes(&fa, k_dose_tc_pair<0, 0>);
         fprintf(stderr, "[gmco] pair kernel: grid (%d, %d) smem %d stages %d regs %d static smem %zu clusters %d (%s) ok %d\n", t->segs, t->n_tiles,
                 t->pair_smem, t->pair_stages, fa.numRegs, fa.sharedSizeBytes, nc, cudaGetErrorName(o), (int)ok);
       }
@@ -1223,7 +1268,8 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
   da.tlo_resident = t->tlo_resident; da.thr = t->thr;
   if (t->dose_pair) {
     da.n_stage = t->pair_stages;
-    k_dose_tc_pair<<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
+    if (t->pair_static) k_dose_tc_pair<4, 6><<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
+    else k_dose_tc_pair<0, 0><<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
   } else if (t->tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
   else k_dose_tc<false><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
   if (cudaPeekAtLastError() != cudaSuccess) return -1;   // left for the caller's message
