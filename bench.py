@@ -31,9 +31,9 @@ sys.path.insert(0, str(ROOT))
 import gmco_cases as gc  # noqa: E402
 
 METRIC, UNIT = "plans_per_s", "plans/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_dose_tc + one k_grad_tc launch, from the ncu --set full
-# capture summarised in profiles/r1_ncu_full_summary.md (a constant copied from that file, not measured here)
-NCU_TRAFFIC_BYTES = {"C3": int((26.053888 + 3.508736 + 74.339328 + 4.086272) * 1e6)}   # cold-cache capture: ncu flushes L2 per kernel
+# dram__bytes_read.sum + dram__bytes_write.sum of one dose launch (k_dose_tc_pair, profiles/r1_ncu_dose_pair.md) + one
+# k_grad_tc launch (profiles/r1_ncu_full_summary.md), from ncu --set full captures (constants copied from those files)
+NCU_TRAFFIC_BYTES = {"C3": int((26.057472 + 3.099904 + 74.339328 + 4.086272) * 1e6)}   # cold-cache capture: ncu flushes L2 per kernel
 
 
 def env_int(name, default):
@@ -414,7 +414,7 @@ def roofline(case, prec, g, prof, peaks):
     if prec == g.GMCO_PREC_TF32X3:
         peak = peaks["bf16_sustained"] * (1.1 / 2.25)
         issued = 3.0 * flops / (ms * 1e-3) / 1e12
-        return {"bound": "tensor", "kernel": "k_dose_tc + k_grad_tc (the two contractions of one round, timed as a pair)",
+        return {"bound": "tensor", "kernel": "dose + gradient contractions of one round (k_dose_tc_pair, or k_dose_tc where the pair kernel does not apply, + k_grad_tc), timed as a pair",
                 "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
                 "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["eval_launches"],
                 "plans_per_launch": plans_per_launch,
