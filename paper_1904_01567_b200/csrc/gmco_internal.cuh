@@ -139,7 +139,7 @@ struct SelectArgs {
 int launch_pareto(const float* obj, int K, int M, unsigned char* nondom, int* count, cudaStream_t st);
 int launch_select(const float* dvh, int K, int S, const SelectArgs& c, int* plan_class, int* out, cudaStream_t st);
 
-// tensor path (kernel_fused_tc.cu)
+// tensor path (kernels_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
                        char* err, int errlen);

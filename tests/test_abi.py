@@ -40,6 +40,7 @@ def test_version_and_default_options(built_lib):
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
+    assert o.compaction == 1 and list(o.reserved) == [0]
 
 
 def test_struct_layouts_match_the_header(built_lib):
@@ -61,6 +62,9 @@ def test_argument_errors_are_reported_without_a_gpu(built_lib):
     with pytest.raises(g.GmcoError) as e:
         g.gmco_create(c.D, c.structures, -1.0)
     assert e.value.code == -1
+    with pytest.raises(g.GmcoError) as e:
+        g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(compaction=2))
+    assert e.value.code == -1 and "options" in str(e.value)
     with pytest.raises(g.GmcoError) as e:
         g.gmco_create(np.zeros((8, 500), np.float32), [gc.Structure("s", 8, 1, 2, 1, 1, 0, 0)], 15.0)
     assert e.value.code == -2
