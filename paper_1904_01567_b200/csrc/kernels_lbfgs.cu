@@ -158,9 +158,28 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
   const int n_run = pp.n_running[parity];
   const int status0 = pp.status[k];
   const int cur = sp.compact_cap ? pp.slot[k] : -1;            // where this round's partials of the plan are
-  if (n_run == 0 || status0 != PLAN_RUNNING) return;
   const int npl = sp.A_pad >> 5;
   const long long row = (long long)k * sp.A_pad + lane;
+  // Every global read of the plan's state is issued here as well, before the status is known (all rows exist for
+  // k < K; a plan that has stopped just discards them): the whole kernel then pays about one memory round trip plus the
+  // batches of the gradient partials (it is latency-bound, not bandwidth-bound).  rho / gamma of the m history pairs
+  // live in lanes 0..m-1 and are broadcast by shuffle in the two-loop recursion: a global load per recursion step
+  // would put 2 m dependent L2 latencies on the critical path.
+  float G[NPL], xt[NPL], gt[NPL], x[NPL], g[NPL];
+#pragma unroll
+  for (int j = 0; j < NPL; ++j) {
+    xt[j] = j < npl ? pp.xt[row + 32 * j] : 0.f;
+    x[j] = j < npl ? pp.x[row + 32 * j] : 0.f;
+    g[j] = j < npl ? pp.g[row + 32 * j] : 0.f;
+  }
+  float rho_l = lane < sp.m ? pp.rho[(long long)lane * pp.K_pad + k] : 0.f;
+  float gam_l = lane < sp.m ? pp.gam[(long long)lane * pp.K_pad + k] : 0.f;
+  int tr = pp.trials[k];
+  float F = pp.F[k];
+  int it = pp.it_done[k];
+  int hc = pp.hcount[k], hh = pp.hhead[k];
+  const float alpha = pp.alpha[k], gp = pp.gp[k];
+  if (n_run == 0 || status0 != PLAN_RUNNING) return;
   const long long hstride = (long long)pp.K_pad * sp.A_pad;
   float* hS = s_hist + (size_t)warp * 2 * sp.m * sp.A_pad;     // [m][A_pad] s vectors, by ring slot
   float* hY = hS + (size_t)sp.m * sp.A_pad;                    // [m][A_pad] y vectors
@@ -190,24 +209,6 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     }
   };
 
-  // Every global read of the plan's state is issued here, before the partial sums, so that the whole kernel pays
-  // about one memory round trip plus the two batches of the gradient partials (it is latency-bound, not
-  // bandwidth-bound).  rho / gamma of the m history pairs live in lanes 0..m-1 and are broadcast by shuffle in the
-  // two-loop recursion: a global load per recursion step would put 2 m dependent L2 latencies on the critical path.
-  float G[NPL], xt[NPL], gt[NPL], x[NPL], g[NPL];
-#pragma unroll
-  for (int j = 0; j < NPL; ++j) {
-    xt[j] = j < npl ? pp.xt[row + 32 * j] : 0.f;
-    x[j] = j < npl ? pp.x[row + 32 * j] : 0.f;
-    g[j] = j < npl ? pp.g[row + 32 * j] : 0.f;
-  }
-  float rho_l = lane < sp.m ? pp.rho[(long long)lane * pp.K_pad + k] : 0.f;
-  float gam_l = lane < sp.m ? pp.gam[(long long)lane * pp.K_pad + k] : 0.f;
-  int tr = pp.trials[k];
-  float F = pp.F[k];
-  int it = pp.it_done[k];
-  int hc = pp.hcount[k], hh = pp.hhead[k];
-  const float alpha = pp.alpha[k], gp = pp.gp[k];
   const float Ft = reduce_partials<NPL>(sp, k, lane, npl, G, cur, n_run);
 #pragma unroll
   for (int j = 0; j < NPL; ++j) gt[j] = g_scale * xt[j] * G[j];   // Eq. 3 summed: g = 2 x o (D^T r)
