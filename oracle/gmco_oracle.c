@@ -19,6 +19,10 @@
  *                   least-squares solution, random starts -> same F.
  *   orc_dvh       : hand-built dose vectors incl. exact ties.
  *   orc_sa_chain  : incremental dose == D t recomputed; zero-temperature monotonicity.
+ *   orc_dose_rate : value at 1 cm, inverse-square law with g = 1, the r floor, role swap = transpose, axis
+ *                   relabelling, element independence, the generator's numpy recipe (independent code).
+ *   select_plan / pareto_front (oracle/__init__.py, written-out definitions): hand-built tables, a 2-D
+ *                   sorting sweep, exhaustive enumeration, invariants (tests/test_oracle_pool.py).
  *   Absolute values printed by the paper: none exist (figures only) -> parity with the
  *   paper's figures is UNPINNED.
  */
