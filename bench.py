@@ -120,7 +120,11 @@ def run_reference(args, case):
     rank = env_int("RANK", 0)
     if rank != 0:
         return
-    sample = args.ref_sample
+    # bounded: about 12 s per step at 256 plans on 16 cores; with many steps the per-step sample shrinks so that the
+    # whole --steps/--warmup run still ends within a few minutes (plans are independent: plans/s does not depend on it)
+    total = max(args.warmup + args.steps, 1)
+    sample = args.ref_sample if total <= 8 else max(16, args.ref_sample * 8 // total)
+    sample = min(sample, case.n_plans)
     vals = []
     for i in range(args.warmup + args.steps):
         v, dt, cores = oracle_leg(case, sample)
