@@ -1205,10 +1205,12 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
             make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
             make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
-  // CTA-pair dose kernel: resident layout, an even number of plan tiles (GMCO_DOSE_PAIR=0 keeps the single-CTA kernel)
+  // CTA-pair dose kernel: resident layout, an even number of plan tiles and of dwell groups (GMCO_DOSE_PAIR=0 keeps the
+  // single-CTA kernel).  The kernel handles an odd group count (zero-filled half entry), but that path has no GPU
+  // parity record yet, so such shapes stay on k_dose_tc.
   {
     const char* env = getenv("GMCO_DOSE_PAIR");
-    t->dose_pair = t->tlo_resident && t->n_tiles % 2 == 0 && !(env && env[0] == '0');
+    t->dose_pair = t->tlo_resident && t->n_tiles % 2 == 0 && G % 2 == 0 && !(env && env[0] == '0');
     if (t->dose_pair) {
       const int fixedp = G * kTloBox + slack;
       t->pair_stages = (kSmemMax - fixedp) / kPairEntry;
