@@ -31,9 +31,19 @@ sys.path.insert(0, str(ROOT))
 import gmco_cases as gc  # noqa: E402
 
 METRIC, UNIT = "plans_per_s", "plans/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of one dose launch (k_dose_tc_pair, profiles/r1_ncu_dose_pair.md) + one
-# k_grad_tc launch (profiles/r1_ncu_full_summary.md), from ncu --set full captures (constants copied from those files)
-NCU_TRAFFIC_BYTES = {"C3": int((26.057472 + 3.099904 + 74.339328 + 4.086272) * 1e6)}   # cold-cache capture: ncu flushes L2 per kernel
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures: rows "config,kernel,read,write,source"
+NCU_TRAFFIC_FILE = ROOT / "profiles" / "ncu_traffic.csv"
+
+
+def ncu_traffic(config: str, kernel: str):
+    """DRAM bytes per launch of `kernel` on `config` from the committed ncu summary, or None when there is no capture."""
+    if not NCU_TRAFFIC_FILE.exists():
+        return None
+    for ln in NCU_TRAFFIC_FILE.read_text().splitlines():
+        f = [v.strip() for v in ln.split(",")]
+        if len(f) >= 4 and f[0] == config and f[1] == kernel:
+            return int(float(f[2]) + float(f[3]))
+    return None
 
 
 def env_int(name, default):
@@ -116,6 +126,45 @@ def oracle_leg(case, sample_plans):
     return sample_plans / dt, dt, oracle.num_threads()
 
 
+def oracle_leg_one_core(case, n_plans=4):
+    """The same oracle on ONE core: its only parallelism is OpenMP over plans, so a one-plan call runs on one thread."""
+    import oracle
+    oracle.build()
+    t0 = time.perf_counter()
+    for k in range(n_plans):
+        oracle.optimize(case.D, case.structures, case.rx, case.T0, case.weights[k:k + 1], m=case.m, iters=case.iters)
+    dt = time.perf_counter() - t0
+    return n_plans / dt, dt
+
+
+def measure_tf32_peak(torch, seconds=3.0):
+    """Dense tf32 matmul throughput measured the way MEASURED_PEAKS.json measured bf16: torch.matmul 8192^3 (2 N^3 flops)
+    with tf32 allowed, best of 10 (burst) and back to back for `seconds` (sustained), CUDA events."""
+    n = 8192
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn(n, n, device="cuda"); b = torch.randn(n, n, device="cuda"); c = torch.empty(n, n, device="cuda")
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        best = None
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); e1.synchronize()
+            best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        reps = max(10, int(seconds * 1e3 / best))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b, out=c)
+        e1.record(); e1.synchronize()
+        flops = 2.0 * n ** 3
+        return {"tf32_tflops": flops / (best * 1e-3) / 1e12, "tf32_tflops_sustained": flops * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12,
+                "how": f"torch.matmul fp32 inputs, allow_tf32, 8192^3: best of 10 (burst) and {reps} back to back (sustained), CUDA events"}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
 def run_reference(args, case):
     rank = env_int("RANK", 0)
     if rank != 0:
@@ -169,6 +218,7 @@ def workload_config(case, args, stats):
     if stats:
         cfg["rounds"] = stats["rounds"]
         cfg["device_bytes"] = stats["device_bytes"]
+        cfg["dose_kernel"] = stats.get("dose_kernel_name")
     return cfg
 
 
@@ -182,6 +232,8 @@ def main():
     ap.add_argument("--precision", default="tf32x3", choices=["tf32x3", "simt"])
     ap.add_argument("--ref-sample", type=int, default=256, help="plans per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-peak", action="store_true", help="skip the live tf32 matmul peak measurement (roofline falls back to the nominal ratio)")
+    ap.add_argument("--dose-kernel", type=int, default=0, choices=[0, 1], help="gmco_options.dose_kernel (1 = keep the single-CTA dose kernel)")
     ap.add_argument("--no-gsa", action="store_true", help="skip the gSA-vs-gL-BFGS comparison leg (C5)")
     ap.add_argument("--clock-period", type=float, default=0.02, help="seconds between NVML clock samples (0 = off)")
     ap.add_argument("--eps", type=float, default=0.0, help="per-plan stopping rule (PAPER.md:119); 0 = exactly `iters` iterations")
@@ -227,7 +279,7 @@ def main():
 
     def step(host: bool, profile: bool = False):
         Dm, Tm, wm, om = (D_pin, T0_pin, w_pin, out_pin) if host else (D_dev, T0_dev, w_dev, out_dev)
-        opt = g.binding.make_options(m=case.m, precision=prec, eps=args.eps, compaction=args.compaction)
+        opt = g.binding.make_options(m=case.m, precision=prec, eps=args.eps, compaction=args.compaction, dose_kernel=args.dose_kernel)
         h = g.gmco_create(Dm, case.structures, case.rx, opt, stream)
         try:
             if profile:
@@ -236,6 +288,7 @@ def main():
             g.binding._check(L.gmco_result(h.ptr, om["T"].data_ptr(), om["F"].data_ptr(), om["dvh"].data_ptr(),
                                            om["terms"].data_ptr(), om["it"].data_ptr(), om["st"].data_ptr()), h)
             last["stats"] = g.gmco_get_stats(h)
+            last["stats"]["dose_kernel_name"] = g.DOSE_KERNEL_NAMES.get(last["stats"]["dose_kernel"])
         finally:
             g.gmco_destroy(h)
 
@@ -295,16 +348,19 @@ def main():
             "clocks": clk.summary(),
             "paper_context": "gL-BFGS 0.9 ms/plan = ~1111 plans/s on a Titan X (Pascal), real cases, eps=1e-3 (PAPER.md:180)",
         }
-        line["roofline"] = roofline(case, prec, g, prof, peaks)
+        tf32 = None if (args.no_peak or prec != g.GMCO_PREC_TF32X3) else measure_tf32_peak(torch)
+        line["roofline"] = roofline(case, prec, g, prof, peaks, tf32, clk.summary())
         if not args.no_gsa:
             line["gsa_vs_glbfgs"] = gsa_leg(g, torch, stream)
         if args.characterise:
             line["characterisation"] = characterise_leg(g, torch, stream, prec)
         if not args.no_cpu_baseline:
             v, dt, cores = oracle_leg(case, args.ref_sample)
+            v1, dt1 = oracle_leg_one_core(case)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{args.ref_sample} of {K} plans of {case.name}, full {case.iters} "
-                                              f"iterations, {dt:.1f} s, OpenMP over plans"}
+                                              f"iterations, {dt:.1f} s, OpenMP over plans",
+                                    "value_1core": v1, "sample_1core": f"4 plans one after the other, {dt1:.1f} s"}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -404,31 +460,56 @@ def gsa_leg(g, torch, stream):
             "paper_context": "gL-BFGS up to 67x faster than gSA, objectives within 0.2-0.4 % (PAPER.md:160-162, :180; Titan X Pascal)"}
 
 
-def roofline(case, prec, g, prof, peaks):
-    """Dominant kernel = the contraction (fused dose+penalty+gradient) kernel.
-    Algorithmic flops per launch = 4 N A K (one D t and one D^T r per plan); the 3xTF32
-    split issues 3x that on the tensor pipe.  Peak: measured bf16 (sustained: the kernel runs inside a
-    long step) x the guide's nominal tf32/bf16 ratio 1.1/2.25; SIMT: 148 SM x 128 lanes x 2 x 1.965 GHz."""
+def roofline(case, prec, g, prof, peaks, tf32, clocks):
+    """Per-kernel rooflines of one round, from CUDA events the library records around every kernel of the profiled steps
+    (gmco_set_profiling).  The object itself describes the DOMINANT kernel (the dose kernel); `per_kernel` holds all three.
+    Algorithmic work: dose kernel 2 N A flops per plan-evaluation (one D t), gradient
+    kernel 2 N A (one D^T r) -- the 3xTF32 split issues 3x that on the tensor pipe, and `achieved` counts issued flops;
+    step kernel (4 m A + 10 A) x 4 bytes per plan-round (S, Y read twice, one pair written, g / x / p traffic).
+    Peak of the tensor kernels: dense tf32 matmul measured in this run the way MEASURED_PEAKS.json measured bf16 (burst:
+    each kernel is timed alone by its own events and the step is far too short to reach the power cap); alternatives
+    are listed beside it.  Peak of the step kernel: the measured HBM copy bandwidth."""
     if not prof or not prof.get("eval_launches"):
         return None
-    # plan-evaluations per launch: the running plans of each round (all K until plans start to finish)
-    plans_per_launch = prof["eval_plans"] / prof["eval_launches"]
-    flops = 4.0 * case.n_points * case.n_dwell * plans_per_launch
-    ms = prof["eval_ms"] / prof["eval_launches"]
-    if prec == g.GMCO_PREC_TF32X3:
-        peak = peaks["bf16_sustained"] * (1.1 / 2.25)
+    n = prof["eval_launches"]
+    plans = prof["eval_plans"] / n                       # running plans per round (all K until plans start to finish)
+    ms_dose, ms_grad, ms_step = prof["dose_ms"] / n, prof["grad_ms"] / n, prof["step_ms"] / n
+    flops = 2.0 * case.n_points * case.n_dwell * plans   # one contraction
+    if prec != g.GMCO_PREC_TF32X3:
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        ach = 2 * flops / ((ms_dose + ms_grad) * 1e-3) / 1e12
+        return {"bound": "alu", "kernel": "k_simt_dose + k_simt_grad", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "avg_launch_ms": ms_dose + ms_grad, "launches": n,
+                "peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": None}
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    alts = {"nominal_ratio_of_measured_bf16_burst": peaks["bf16_burst"] * (1.1 / 2.25),
+            "nominal_ratio_of_measured_bf16_sustained": peaks["bf16_sustained"] * (1.1 / 2.25),
+            "issue_limit_4096_flop_per_clk_per_sm_at_sampled_clock": 4096 * 148 * sm_mhz * 1e6 / 1e12,
+            "nominal_dense_tf32": 1100.0}
+    if tf32:
+        peak, src = tf32["tf32_tflops"], "measured in this run: " + tf32["how"] + " (burst)"
+        alts["measured_tf32_sustained"] = tf32["tf32_tflops_sustained"]
+    else:
+        peak, src = alts["nominal_ratio_of_measured_bf16_burst"], f"{peaks['source']} bf16 burst x 1.1/2.25 (nominal tf32:bf16; no live tf32 measurement)"
+    dose_name = prof.get("dose_kernel_name") or "k_dose_tc"
+
+    def tensor(kernel, ms):
         issued = 3.0 * flops / (ms * 1e-3) / 1e12
-        return {"bound": "tensor", "kernel": "dose + gradient contractions of one round (k_dose_tc_pair, or k_dose_tc where the pair kernel does not apply, + k_grad_tc), timed as a pair",
-                "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
-                "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms, "launches": prof["eval_launches"],
-                "plans_per_launch": plans_per_launch,
-                "peak_source": f"{peaks['source']} bf16 sustained x 1.1/2.25 (nominal tf32:bf16)",
-                "traffic": NCU_TRAFFIC_BYTES.get(case.name)}
-    peak = 148 * 128 * 2 * 1.965e9 / 1e12
-    ach = flops / (ms * 1e-3) / 1e12
-    return {"bound": "alu", "kernel": "k_simt_dose + k_simt_grad", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-            "frac": ach / peak, "avg_launch_ms": ms, "launches": prof["eval_launches"],
-            "peak_source": "148 SM x 128 fp32 lanes x 2 x 1.965 GHz", "traffic": None}
+        return {"bound": "tensor", "kernel": kernel, "achieved": issued, "peak": peak, "unit": "TFLOP/s", "frac": issued / peak,
+                "achieved_fp32_equivalent": issued / 3.0, "avg_launch_ms": ms,
+                "traffic": ncu_traffic(case.name, kernel.split("<")[0])}
+    step_bytes = (4 * case.m * case.n_dwell + 10 * case.n_dwell) * 4.0 * plans
+    step = {"bound": "hbm", "kernel": "k_step", "achieved": step_bytes / (ms_step * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+            "unit": "GB/s", "frac": step_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"], "avg_launch_ms": ms_step,
+            "traffic": ncu_traffic(case.name, "k_step"),
+            "note": "latency-bound: one warp per plan, 2 m dependent dot products (DESIGN.md 5.3)"}
+    dose, grad = tensor(dose_name, ms_dose), tensor("k_grad_tc<16>", ms_grad)
+    out = dict(dose)
+    out.update({"launches": n, "plans_per_launch": plans, "peak_source": src, "peak_alternatives": alts,
+                "traffic_source": str(NCU_TRAFFIC_FILE.relative_to(ROOT)) if NCU_TRAFFIC_FILE.exists() else None,
+                "round_ms": {"dose": ms_dose, "grad": ms_grad, "step": ms_step},
+                "per_kernel": {"dose": dose, "grad": grad, "step": step}})
+    return out
 
 
 if __name__ == "__main__":

@@ -40,7 +40,7 @@ extern "C" {
 #define GMCO_API
 #endif
 
-#define GMCO_VERSION 120          /* 0.1.2 */
+#define GMCO_VERSION 130          /* 0.1.3 */
 #define GMCO_MAX_STRUCTS 8
 #define GMCO_MAX_HISTORY 16
 #define GMCO_MAX_CRITERIA 8
@@ -51,7 +51,8 @@ typedef enum gmco_status {
   GMCO_OK = 0,
   GMCO_E_INVALID = -1,      /* NULL pointer, bad size, NaN/negative input, sizes do not add up   */
   GMCO_E_UNSUPPORTED = -2,  /* no sm_100 device, or a size outside the supported range            */
-  GMCO_E_CUDA = -3,         /* a CUDA call failed; message holds cudaGetErrorString               */
+  GMCO_E_CUDA = -3,         /* a CUDA call failed (message holds cudaGetErrorString), or a kernel reported a
+                               protocol error through the device error word (message names kernel and site) */
   GMCO_E_NOMEM = -4,        /* device allocation failed                                           */
   GMCO_E_STATE = -5         /* call out of order (e.g. gmco_result before gmco_optimize)          */
 } gmco_status;
@@ -101,19 +102,42 @@ typedef struct gmco_options {
                          128-plan tiles every round, so a round costs what the RUNNING plans cost
                          (plans stop at different rounds: eps > 0, or unequal numbers of
                          step halvings); 0: every plan keeps its tile            default 1        */
-  int32_t reserved[1];/* must be 0                                                                */
+  int32_t dose_kernel;/* 0: automatic -- CTA pairs (tcgen05 cta_group::2) where the shape allows, else one CTA per
+                         plan tile; 1: always one CTA per plan tile.  Both compute the same products; they differ
+                         in partial-sum order (low-order bits).  gmco_stats.dose_kernel says which one ran.
+                                                                                  default 0        */
+  int32_t reserved[2];/* must be 0                                                                */
 } gmco_options;
 
 /* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */
 typedef struct gmco_stats {
   int64_t device_bytes;     /* bytes currently allocated by the handle                            */
-  int32_t rounds;           /* evaluation rounds executed (1 + iterations + backtracks of the slowest plan) */
+  int32_t rounds;           /* evaluation rounds that had a running plan (1 + iterations + backtracks of the slowest plan) */
   int32_t kernel_launches;  /* kernels launched by the library since gmco_optimize was called     */
   int32_t plans_iters, plans_converged, plans_stalled;
   int32_t eval_launches;    /* profiling only: contraction launches that had work (see gmco_set_profiling) */
   float eval_ms;            /* profiling only: summed device time of those launches, CUDA events  */
   int32_t eval_plans;       /* profiling only: plan-evaluations those launches did (running plans, summed over rounds) */
+  float dose_ms, grad_ms, step_ms; /* profiling only: eval_ms split into the dose kernel and the gradient kernel, and the
+                               summed device time of the per-plan step kernel of the same rounds                */
+  int32_t dose_kernel;      /* gmco_tc_info.dose_kernel of the dose kernel that ran (-1 on the SIMT route)        */
 } gmco_stats;
+
+/* Launch schedule and on-chip layout of the tensor route for one shape: what gmco_optimize would launch.  Host
+ * arithmetic only (no GPU needed): used by the tests to prove on the CPU that every shape's shared-memory carve-up,
+ * TMEM columns and TMA boxes fit, and by bench.py to record which kernels ran. */
+typedef struct gmco_tc_info {
+  int32_t ok;               /* 0: the shape does not run on the tensor route (n_dwell > 384)                      */
+  int32_t a_pad, n_pad, n_alloc, k_pad;   /* padded sizes: dwell columns (32), points (64 per structure), rows allocated (256), plans (128) */
+  int32_t n_tiles, segs, n_chunks, n_slabs, compact_cap;
+  int32_t dose_kernel;      /* 0 k_dose_tc<resident T_lo>, 1 k_dose_tc<streamed T_lo>, 2 k_dose_tc_pair<static schedule>,
+                               3 k_dose_tc_pair<run-time ring>                                                    */
+  int32_t dose_threads, dose_stages, dose_stage_bytes, dose_smem_bytes, dose_smem_end, dose_scr_slot, dose_tmem_cols;
+  int32_t grad_threads, grad_ps, grad_stages, grad_stage_bytes, grad_smem_bytes, grad_smem_end, grad_staging_bytes,
+      grad_tmem_cols;
+  int32_t smem_limit, tmem_limit;        /* 232448 B opt-in dynamic shared memory per CTA, 512 TMEM columns       */
+} gmco_tc_info;
+
 
 typedef struct gmco_handle gmco_handle;
 
@@ -153,7 +177,8 @@ GMCO_API int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh,
  * or [n_dwell] if t_broadcast) through the SAME kernels the optimiser uses.  Outputs (host or
  * device, any may be NULL): dose [n_points][K] (plan fastest) -- the fused path never stores
  * dose otherwise; F [K]; grad_x [K][n_dwell] = dF/dx with x = sqrt(T).  Enqueues, then
- * synchronises only if an output is a host pointer.  Discards any optimisation state. */
+ * synchronises the stream (it is a test hook: the input check and the device error word are
+ * read back before it returns).  Discards any optimisation state. */
 GMCO_API int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const float* weights,
                   int32_t K, float* dose, float* F, float* grad_x, void* cuda_stream);
 
@@ -225,11 +250,19 @@ GMCO_API int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t 
 /* Counters of the last optimise/result pair.  GMCO_E_STATE before the first gmco_result. */
 GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);
 
-/* Measurement aid (bench.py's roofline leg).  With enable != 0 every contraction launch of the
- * following gmco_optimize / gmco_result (the kernels that compute D t, the penalty and D^T r) is
- * bracketed by a pair of CUDA events on the caller's stream; gmco_result sums their elapsed
- * times over the rounds in which at least one plan was running and reports them in gmco_stats
- * (eval_ms, eval_launches).  Off by default; results are identical either way. */
+/* Schedule of the tensor route for a case of n_dwell dwell positions, structures of
+ * struct_points[0..n_structs) points (HOST array) and K plans on a device with num_sms multiprocessors (148 on
+ * B200); dose_kernel as in gmco_options.  Pure host arithmetic: needs no GPU and no handle.  GMCO_E_INVALID for
+ * NULL / non-positive arguments; out->ok = 0 (and GMCO_OK) when the shape is outside the tensor route. */
+GMCO_API int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_structs, int32_t K,
+                     int32_t num_sms, int32_t dose_kernel, gmco_tc_info* out);
+
+/* Measurement aid (bench.py's roofline leg).  With enable != 0 every kernel of a round of the
+ * following gmco_optimize / gmco_result (the dose kernel: D t, penalty, objective; the gradient
+ * kernel: D^T r; the per-plan step kernel) is bracketed by CUDA events on the caller's stream;
+ * gmco_result sums their elapsed times over the rounds in which at least one plan was running and
+ * reports them in gmco_stats (eval_ms = dose_ms + grad_ms, step_ms, eval_launches).  Off by
+ * default; results are identical either way. */
 GMCO_API int gmco_set_profiling(gmco_handle* h, int32_t enable);
 
 /* Frees everything the handle owns (synchronises its stream first).  NULL is a no-op. */

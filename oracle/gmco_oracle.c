@@ -18,7 +18,10 @@
  *   orc_lbfgs     : SPD quadratic vs A^-1 b, monotone F, first step = -g/|g|, planted
  *                   least-squares solution, random starts -> same F.
  *   orc_dvh       : hand-built dose vectors incl. exact ties.
- *   orc_sa_chain  : incremental dose == D t recomputed; zero-temperature monotonicity.
+ *   orc_sa_chain  : the hand-worked chains of tests/golden/sa_chain_hand_case.txt (move width 0.1 t_j with its
+ *                   0.01 tau floor, clip at 0, downhill / uphill accept / uphill reject with u on either side of
+ *                   exp(-dF/T_n), T_n = temp0 cooling^n bracketed from both sides at n = 0..3; state after every
+ *                   prefix); incremental dose == D t recomputed; zero-temperature monotonicity.
  *   orc_dose_rate : value at 1 cm, inverse-square law with g = 1, the r floor, role swap = transpose, axis
  *                   relabelling, element independence, the generator's numpy recipe (independent code).
  *   select_plan / pareto_front (oracle/__init__.py, written-out definitions): hand-built tables, a 2-D

@@ -6,5 +6,6 @@ PyTorch is used for device memory and streams, nothing else.  There is no CPU fa
 importing :mod:`paper_1904_01567_b200.binding` raises if the library has not been built.
 """
 from .binding import (GmcoError, Handle, Options, gmco_create, gmco_destroy, gmco_dose_rate_matrix, gmco_evaluate, gmco_get_stats,  # noqa: F401
-                      gmco_optimize, gmco_pareto_front, gmco_result, gmco_sa_run, gmco_select_plan, gmco_set_profiling, gmco_version, lib, lib_path,
+                      gmco_optimize, gmco_pareto_front, gmco_result, gmco_sa_run, gmco_select_plan, gmco_set_profiling, gmco_tc_schedule,
+                      gmco_version, lib, lib_path, DOSE_KERNEL_NAMES,
                       GMCO_PREC_TF32X3, GMCO_PREC_SIMT_FP32, GMCO_SA_FP64, GMCO_SA_FP32)

@@ -25,7 +25,8 @@ class _Structure(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
-                ("precision", C.c_int32), ("eps_f", C.c_float), ("compaction", C.c_int32), ("reserved", C.c_int32 * 1)]
+                ("precision", C.c_int32), ("eps_f", C.c_float), ("compaction", C.c_int32), ("dose_kernel", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
 
 
 class Criterion(C.Structure):
@@ -36,7 +37,19 @@ class Criterion(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("device_bytes", C.c_int64), ("rounds", C.c_int32), ("kernel_launches", C.c_int32),
                 ("plans_iters", C.c_int32), ("plans_converged", C.c_int32), ("plans_stalled", C.c_int32),
-                ("eval_launches", C.c_int32), ("eval_ms", C.c_float), ("eval_plans", C.c_int32)]
+                ("eval_launches", C.c_int32), ("eval_ms", C.c_float), ("eval_plans", C.c_int32),
+                ("dose_ms", C.c_float), ("grad_ms", C.c_float), ("step_ms", C.c_float), ("dose_kernel", C.c_int32)]
+
+
+class TcInfo(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in (
+        "ok", "a_pad", "n_pad", "n_alloc", "k_pad", "n_tiles", "segs", "n_chunks", "n_slabs", "compact_cap", "dose_kernel",
+        "dose_threads", "dose_stages", "dose_stage_bytes", "dose_smem_bytes", "dose_smem_end", "dose_scr_slot", "dose_tmem_cols",
+        "grad_threads", "grad_ps", "grad_stages", "grad_stage_bytes", "grad_smem_bytes", "grad_smem_end", "grad_staging_bytes",
+        "grad_tmem_cols", "smem_limit", "tmem_limit")]
+
+DOSE_KERNEL_NAMES = {-1: "k_simt_dose", 0: "k_dose_tc<resident>", 1: "k_dose_tc<streamed>", 2: "k_dose_tc_pair<4,6>",
+                     3: "k_dose_tc_pair<0,0>"}
 
 
 def lib_path() -> Path:
@@ -71,6 +84,7 @@ def lib():
         L.gmco_select_plan.argtypes = [vp, fp, i32, C.POINTER(Criterion), i32, vp, vp, vp, vp]
         L.gmco_pareto_front.argtypes = [vp, fp, i32, i32, vp, vp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
+        L.gmco_tc_schedule.argtypes = [i64, C.POINTER(i32), i32, i32, i32, i32, C.POINTER(TcInfo)]
         L.gmco_set_profiling.argtypes = [vp, i32]
         L.gmco_destroy.argtypes = [vp]
         L.gmco_destroy.restype = None
@@ -124,7 +138,8 @@ def _stream(stream):
     return getattr(stream, "cuda_stream", stream)
 
 
-def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None, compaction=None) -> Options:
+def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None, compaction=None,
+                 dose_kernel=None) -> Options:
     o = Options()
     lib().gmco_default_options(C.byref(o))
     o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
@@ -132,6 +147,8 @@ def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32
         o.eps_f = eps_f
     if compaction is not None:
         o.compaction = int(compaction)
+    if dose_kernel is not None:
+        o.dose_kernel = int(dose_kernel)
     return o
 
 
@@ -271,6 +288,14 @@ def gmco_get_stats(h: Handle) -> dict:
     s = Stats()
     _check(lib().gmco_get_stats(h.ptr, C.byref(s)), h)
     return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
+
+
+def gmco_tc_schedule(n_dwell: int, struct_points, K: int, num_sms: int = 148, dose_kernel: int = 0) -> dict:
+    """Launch schedule and on-chip layout of the tensor route for a shape (host arithmetic; needs no GPU)."""
+    pts = (C.c_int32 * len(struct_points))(*[int(v) for v in struct_points])
+    info = TcInfo()
+    _check(lib().gmco_tc_schedule(int(n_dwell), pts, len(struct_points), int(K), int(num_sms), int(dose_kernel), C.byref(info)))
+    return {k: getattr(info, k) for k, _ in TcInfo._fields_}
 
 
 def gmco_set_profiling(h: Handle, enable: bool) -> None:

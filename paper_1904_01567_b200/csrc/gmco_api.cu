@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "gmco_internal.cuh"
+#include "tc_layout.h"
 
 using namespace gmco;
 
@@ -45,6 +46,7 @@ struct gmco_handle {
   float *out_T = nullptr, *out_F = nullptr, *out_dvh = nullptr, *out_terms = nullptr;
   int *out_iters = nullptr, *out_status = nullptr;
   int host_flags[4] = {0, 0, 0, 0};  // pageable: the copies into it are followed by a stream synchronise
+  int host_err[4] = {0, 0, 0, 0};    // copy of the device error word
   TcPlan* tc = nullptr;
   float* sa_Dt = nullptr;            // gSA: transposed copy of D [A][N_alloc], built by the first gmco_sa_run
   // device-driven round loop: a CUDA graph whose only node is a WHILE conditional; its body is two rounds
@@ -57,11 +59,11 @@ struct gmco_handle {
   cudaStream_t stream = nullptr;
   int device = 0, num_sms = 0;
   HandleState state = ST_CREATED;
-  int iters = 0, rounds_enqueued = 0, launches = 0;
+  int iters = 0, rounds_enqueued = 0, rounds_with_work = 0, launches = 0;
   gmco_stats stats{};
   bool have_stats = false;
   bool profile = false;              // gmco_set_profiling
-  std::vector<cudaEvent_t> ev;       // 2 per profiled round
+  std::vector<cudaEvent_t> ev;       // 4 per profiled round: | dose | gradient | step |
   int ev_used = 0;
   char err[512] = "";
 };
@@ -89,6 +91,21 @@ int fail(gmco_handle* h, int code, const char* fmt, const char* a = "") {
     if (n_ < 0) return fail(h, GMCO_E_CUDA, #expr ": %s", cudaGetErrorString(cudaGetLastError())); \
     (h)->launches += n_;                                                         \
   } while (0)
+
+// the device error word (gmco_internal.cuh DevErr) as a GMCO_E_CUDA message; GMCO_OK when it is clear
+int check_dev_err(gmco_handle* h, const int* e) {
+  if (e[0] == DEVERR_NONE) return GMCO_OK;
+  static const char* const kern[] = {"?", "k_dose_tc<resident>", "k_dose_tc<streamed>", "k_dose_tc_pair", "k_grad_tc", "k_step"};
+  static const char* const wait[] = {"-", "ring slot free", "ring slot filled", "T group ready", "T tile landed", "accumulator full",
+                                     "accumulator free", "R tile split", "history copies"};
+  static const char* const what[] = {"?", "a barrier wait did not complete", "the shared-memory carve-up does not fit the launch",
+                                     "the TMEM columns do not fit"};
+  const int k = (e[1] >> 8) & 0xff, wsite = e[1] & 0xff;
+  snprintf(h->err, sizeof(h->err), "device error word: %s in %s (wait: %s), block (%d, %d), detail %d; results are invalid",
+           what[e[0] >= 1 && e[0] <= 3 ? e[0] : 0], kern[k >= 1 && k <= 5 ? k : 0], wait[wsite >= 1 && wsite <= 8 ? wsite : 0],
+           e[2] & 0xffff, (e[2] >> 16) & 0xffff, e[3]);
+  return GMCO_E_CUDA;
+}
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes at{};
@@ -136,14 +153,16 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   p.K = K; p.K_pad = round_up(K, kPlanTile); p.m = h->opt.m;
   const size_t ka = (size_t)p.K_pad * c.A_pad, kp = (size_t)p.K_pad;
   p.x = a.take<float>(ka); p.g = a.take<float>(ka); p.p = a.take<float>(ka); p.xt = a.take<float>(ka);
-  p.T = a.take<float>(ka); p.T_hi = a.take<float>(ka); p.T_lo = a.take<float>(ka);
+  p.T = a.take<float>(ka);
+  // tf32 lo part of T: read (by TMA) only by the streamed dose layout, i.e. above 256 dwell positions on the tensor route
+  p.T_lo = (h->opt.precision == GMCO_PREC_TF32X3 && c.A_pad > 32 * tcl::kTmemGroups) ? a.take<float>(ka) : nullptr;
   p.Sh = a.take<float>(ka * p.m); p.Yh = a.take<float>(ka * p.m);
   p.rho = a.take<float>(kp * p.m); p.gam = a.take<float>(kp * p.m);
   p.Weff = a.take<float>(kp * 2 * c.S); p.WeffC = a.take<float>(kp * 2 * c.S); p.slot = a.take<int>(kp);
   p.F = a.take<float>(kp); p.gp = a.take<float>(kp); p.alpha = a.take<float>(kp);
   p.it_done = a.take<int>(kp); p.trials = a.take<int>(kp); p.hcount = a.take<int>(kp); p.hhead = a.take<int>(kp);
   p.status = a.take<int>(kp);
-  p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1); p.rounds_done = a.take<int>(1);
+  p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1); p.rounds_done = a.take<int>(2); p.dev_err = a.take<int>(4);
   p.round_log = a.take<int>(kRoundLogCap);
   p.tile_seg = a.take<int>(p.K_pad / kPlanTile + 1);
   // partials: the SIMT dose pass (also the final pass of gmco_result) needs [tiles][K_pad][2]
@@ -193,7 +212,7 @@ int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   carve_plans(h, K, 0);
   h->plan_capacity_K = K;
   if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
-    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, st, h->err, sizeof(h->err));
+    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->opt.dose_kernel == 1, st, h->err, sizeof(h->err));
     if (!h->tc) return GMCO_E_UNSUPPORTED;
   }
   return GMCO_OK;
@@ -223,15 +242,22 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
 // SIMT kernels emit r = 2 w (d - D_lim) / n, the tensor kernel emits r / 2 (one multiply less per element)
 float g_scale_of(const gmco_handle* h) { return h->opt.precision == GMCO_PREC_SIMT_FP32 ? 2.f : 4.f; }
 
-// zero_ctr / log_slot: start-of-round bookkeeping (reset the other parity's running-plan counter, log this round's).
-// The tensor route does it in its first kernel; the SIMT route launches k_round_begin.
-int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, int* zero_ctr, int* log_slot, cudaStream_t st) {
+// zero_ctr / log_slot: start-of-round bookkeeping (reset the other parity's running-plan counter, log this round's,
+// count the round if a plan is running).  The tensor route does it in its first kernel; the SIMT route launches
+// k_round_begin.  mid: event recorded between the dose kernel and the gradient kernel (profiling), or null.
+int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, int* zero_ctr, int* log_slot, cudaEvent_t mid,
+                 cudaStream_t st) {
   if (h->opt.precision == GMCO_PREC_SIMT_FP32) {
-    if (zero_ctr) LN(h, launch_round_begin(zero_ctr, gate, log_slot, st));
+    if (zero_ctr) LN(h, launch_round_begin(zero_ctr, gate, log_slot, h->p.rounds_done + 1, st));
     LN(h, launch_simt_eval(h->c, h->p, true, dose_dbg, false, nullptr, gate, st));
+    if (mid) CK(h, cudaEventRecord(mid, st));
     LN(h, launch_simt_grad(h->c, h->p, gate, st));
+  } else if (!mid) {
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, gate && h->opt.compaction, -1, st));
   } else {
-    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, gate && h->opt.compaction, st));
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, gate && h->opt.compaction, 0, st));
+    CK(h, cudaEventRecord(mid, st));
+    LN(h, launch_tc_eval(h->tc, h->c, h->p, dose_dbg, gate, zero_ctr, log_slot, gate && h->opt.compaction, 1, st));
   }
   return GMCO_OK;
 }
@@ -239,7 +265,7 @@ int enqueue_eval(gmco_handle* h, float* dose_dbg, const int* gate, int* zero_ctr
 // one round: every running plan has its trial point evaluated, then accepted or its step halved
 int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const StepParams& sp, cudaStream_t st) {
   if (prof) {
-    while ((int)h->ev.size() < h->ev_used + 2) {
+    while ((int)h->ev.size() < h->ev_used + 4) {
       cudaEvent_t e;
       CK(h, cudaEventCreate(&e));
       h->ev.push_back(e);
@@ -247,10 +273,11 @@ int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const Step
     CK(h, cudaEventRecord(h->ev[h->ev_used], st));
   }
   int rc = enqueue_eval(h, nullptr, h->p.n_running + parity, h->p.n_running + (parity ^ 1),
-                        log_idx < kRoundLogCap ? h->p.round_log + log_idx : nullptr, st);
+                        log_idx < kRoundLogCap ? h->p.round_log + log_idx : nullptr, prof ? h->ev[h->ev_used + 1] : nullptr, st);
   if (rc) return rc;
-  if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 1], st)); h->ev_used += 2; }
+  if (prof) CK(h, cudaEventRecord(h->ev[h->ev_used + 2], st));
   LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
+  if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 3], st)); h->ev_used += 4; }
   return GMCO_OK;
 }
 
@@ -351,6 +378,7 @@ void gmco_default_options(gmco_options* o) {
   if (!o) return;
   memset(o, 0, sizeof(*o));
   o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f; o->compaction = 1;
+  o->dose_kernel = 0;
 }
 
 const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
@@ -372,7 +400,7 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
       (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || (o.compaction != 0 && o.compaction != 1) ||
-      o.reserved[0])
+      (o.dose_kernel != 0 && o.dose_kernel != 1) || o.reserved[0] || o.reserved[1])
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
   // the plain-fp32 kernels (the paper's largest N_act is 385)
@@ -554,18 +582,24 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
   if (K == 0) {
     memset(&h->stats, 0, sizeof(h->stats));
     h->stats.device_bytes = (int64_t)(h->case_arena.size + h->plan_arena.size);
+    h->stats.dose_kernel = -1;
     h->have_stats = true; h->state = ST_RESULT;
     return GMCO_OK;
   }
   if (h->state == ST_OPTIMIZED) {
     const long long max_rounds = max_rounds_of(h);
+    int rounds_with_work = 0;
     for (;;) {
       const int parity = h->used_graph ? 0 : h->rounds_enqueued & 1;   // counter the NEXT round would read
       CK(h, cudaMemcpyAsync(h->host_flags, p.n_running + parity, sizeof(int), cudaMemcpyDeviceToHost, st));
       CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
-      CK(h, cudaMemcpyAsync(h->host_flags + 2, p.rounds_done, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(h, cudaMemcpyAsync(h->host_flags + 2, p.rounds_done, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(h, cudaMemcpyAsync(h->host_err, p.dev_err, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
       CK(h, cudaStreamSynchronize(st));
-      if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s");
+      // a failed optimisation leaves nothing to return: a second gmco_result is a state error, not the same failure again
+      if (h->host_err[0]) { h->state = ST_CREATED; return check_dev_err(h, h->host_err); }
+      if (h->host_flags[1]) { h->state = ST_CREATED; return fail(h, GMCO_E_INVALID, "T0 or weights hold a negative, NaN or infinite value%s"); }
+      rounds_with_work = h->host_flags[3];
       if (h->used_graph) {
         h->rounds_enqueued = h->host_flags[2];
         h->launches += (h->host_flags[2] / 2) * h->loop_launches_per_pair;
@@ -575,6 +609,7 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
       int rc = enqueue_rounds(h, 8, st);
       if (rc) return rc;
     }
+    h->rounds_with_work = rounds_with_work;
     // final dose pass at the accepted dwell times: objective terms, V_level counts, D_level doses
     LN(h, launch_prepare_final(c, p, st));
     LN(h, launch_simt_eval(c, p, false, nullptr, true, h->dvh_thr, nullptr, st));
@@ -594,24 +629,28 @@ int gmco_result(gmco_handle* h, float* T, float* objective, float* dvh, float* o
     CK(h, cudaMemcpy(stv.data(), h->out_status, (size_t)K * sizeof(int), cudaMemcpyDeviceToHost));
     gmco_stats s{};
     s.device_bytes = (int64_t)(h->case_arena.size + h->plan_arena.size);
-    s.rounds = h->rounds_enqueued; s.kernel_launches = h->launches;
+    s.rounds = h->rounds_with_work; s.kernel_launches = h->launches;
+    s.dose_kernel = h->tc ? tc_dose_kernel(h->tc) : -1;
     for (int k = 0; k < K; ++k) {
       if (stv[k] == GMCO_PLAN_ITERS) s.plans_iters++;
       else if (stv[k] == GMCO_PLAN_CONVERGED) s.plans_converged++;
       else s.plans_stalled++;
     }
     if (h->profile && h->ev_used > 0) {
-      const int nr = h->ev_used / 2;
+      const int nr = h->ev_used / 4;
       std::vector<int> log(nr);
       CK(h, cudaMemcpy(log.data(), p.round_log, (size_t)nr * sizeof(int), cudaMemcpyDeviceToHost));
-      double ms = 0.0;
+      double ms_dose = 0.0, ms_grad = 0.0, ms_step = 0.0;
       for (int r = 0; r < nr; ++r) {
-        if (log[r] <= 0) continue;                         // nothing was running: the launch returned at once
+        if (log[r] <= 0) continue;                         // nothing was running: the launches returned at once
         float t = 0.f;
-        CK(h, cudaEventElapsedTime(&t, h->ev[2 * r], h->ev[2 * r + 1]));
-        ms += t; s.eval_launches++; s.eval_plans += log[r];
+        CK(h, cudaEventElapsedTime(&t, h->ev[4 * r], h->ev[4 * r + 1])); ms_dose += t;
+        CK(h, cudaEventElapsedTime(&t, h->ev[4 * r + 1], h->ev[4 * r + 2])); ms_grad += t;
+        CK(h, cudaEventElapsedTime(&t, h->ev[4 * r + 2], h->ev[4 * r + 3])); ms_step += t;
+        s.eval_launches++; s.eval_plans += log[r];
       }
-      s.eval_ms = (float)ms;
+      s.dose_ms = (float)ms_dose; s.grad_ms = (float)ms_grad; s.step_ms = (float)ms_step;
+      s.eval_ms = (float)(ms_dose + ms_grad);
     }
     h->stats = s; h->have_stats = true;
   }
@@ -630,35 +669,34 @@ int gmco_evaluate(gmco_handle* h, const float* T, int32_t t_broadcast, const flo
   if (rc) return rc;
   h->stream = st; h->state = ST_EVALUATED; h->launches = 0;
   const CaseDev& c = h->c; const PlanDev& p = h->p;
-  const float *Td = nullptr, *wd = nullptr;
-  rc = copy_inputs(h, T, t_broadcast, weights, K, st, &Td, &wd);
-  if (rc) return rc;
-  LN(h, launch_init_plans(c, p, Td, t_broadcast ? 1 : 0, wd, h->struct_scale, st));
   float* dose_dev = dose;
   const bool dose_host = dose && !is_device_ptr(dose);
-  if (dose_host) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dose_dev), (size_t)c.N * K * sizeof(float), st));
-  rc = enqueue_eval(h, dose_dev, nullptr, nullptr, nullptr, st);
+  auto body = [&]() -> int {                             // one cleanup point for the scratch below
+    const float *Td = nullptr, *wd = nullptr;
+    int r = copy_inputs(h, T, t_broadcast, weights, K, st, &Td, &wd);
+    if (r) return r;
+    LN(h, launch_init_plans(c, p, Td, t_broadcast ? 1 : 0, wd, h->struct_scale, st));
+    if (dose_host) CK(h, cudaMallocAsync(reinterpret_cast<void**>(&dose_dev), (size_t)c.N * K * sizeof(float), st));
+    r = enqueue_eval(h, dose_dev, nullptr, nullptr, nullptr, nullptr, st);
+    if (r) return r;
+    StepParams sp = make_step_params(h, 0);
+    sp.compact_cap = 0;                                    // one evaluation of every plan in place: no slots
+    float* Fd = F ? h->out_F : nullptr;
+    float* gd = grad_x ? h->out_T : nullptr;
+    LN(h, launch_eval_finish_scaled(c, p, sp, g_scale_of(h), Fd, gd, st));
+    if (F) CK(h, cudaMemcpyAsync(F, Fd, (size_t)K * sizeof(float), cudaMemcpyDefault, st));
+    if (grad_x) CK(h, cudaMemcpyAsync(grad_x, gd, (size_t)K * c.A * sizeof(float), cudaMemcpyDefault, st));
+    if (dose_host) CK(h, cudaMemcpyAsync(dose, dose_dev, (size_t)c.N * K * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(h, cudaMemcpyAsync(h->host_err, p.dev_err, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    return GMCO_OK;
+  };
+  rc = body();
+  if (dose_host && dose_dev && dose_dev != dose) cudaFreeAsync(dose_dev, st);
   if (rc) return rc;
-  StepParams sp = make_step_params(h, 0);
-  sp.compact_cap = 0;                                    // one evaluation of every plan in place: no slots
-  float* Fd = F ? h->out_F : nullptr;
-  float* gd = grad_x ? h->out_T : nullptr;
-  LN(h, launch_eval_finish_scaled(c, p, sp, g_scale_of(h), Fd, gd, st));
-  bool any_host = dose_host;
-  if (F) { CK(h, cudaMemcpyAsync(F, Fd, (size_t)K * sizeof(float), cudaMemcpyDefault, st)); any_host |= !is_device_ptr(F); }
-  if (grad_x) {
-    CK(h, cudaMemcpyAsync(grad_x, gd, (size_t)K * c.A * sizeof(float), cudaMemcpyDefault, st));
-    any_host |= !is_device_ptr(grad_x);
-  }
-  if (dose_host) {
-    CK(h, cudaMemcpyAsync(dose, dose_dev, (size_t)c.N * K * sizeof(float), cudaMemcpyDeviceToHost, st));
-    CK(h, cudaFreeAsync(dose_dev, st));
-  }
-  CK(h, cudaMemcpyAsync(h->host_flags + 1, p.bad_input, sizeof(int), cudaMemcpyDeviceToHost, st));
-  if (any_host) {
-    CK(h, cudaStreamSynchronize(st));
-    if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T or weights hold a negative, NaN or infinite value%s");
-  }
+  CK(h, cudaStreamSynchronize(st));
+  if (h->host_err[0]) return check_dev_err(h, h->host_err);
+  if (h->host_flags[1]) return fail(h, GMCO_E_INVALID, "T or weights hold a negative, NaN or infinite value%s");
   return GMCO_OK;
 }
 
@@ -842,6 +880,44 @@ int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t K, int32_
     CK(h, cudaStreamSynchronize(st));
   }
   if (n_nondominated) CK(h, cudaMemcpy(n_nondominated, &host_n, sizeof(int), cudaMemcpyDefault));
+  return GMCO_OK;
+}
+
+int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_structs, int32_t K, int32_t num_sms,
+                     int32_t dose_kernel, gmco_tc_info* out) {
+  if (!out || !struct_points || n_dwell < 1 || n_structs < 1 || n_structs > GMCO_MAX_STRUCTS || K < 1 || num_sms < 1 ||
+      (dose_kernel != 0 && dose_kernel != 1))
+    return fail(nullptr, GMCO_E_INVALID, "gmco_tc_schedule: NULL or non-positive argument%s");
+  memset(out, 0, sizeof(*out));
+  long long n_pad = 0;
+  for (int s = 0; s < n_structs; ++s) {
+    if (struct_points[s] < 1) return fail(nullptr, GMCO_E_INVALID, "gmco_tc_schedule: structure without points%s");
+    n_pad += round_up(struct_points[s], kStructAlign);
+  }
+  if (n_pad > (1 << 28)) return fail(nullptr, GMCO_E_INVALID, "gmco_tc_schedule: too many points%s");
+  out->smem_limit = tcl::kSmemMax; out->tmem_limit = tcl::kTmemCols;
+  out->a_pad = round_up(n_dwell, 32); out->n_pad = (int)n_pad; out->n_alloc = round_up(n_pad, kRowAlloc);
+  out->k_pad = round_up(K, kPlanTile);
+  if (out->a_pad > kMaxApadTensor) return GMCO_OK;   // ok = 0: the SIMT route takes the case
+  const tcl::Schedule q = tcl::choose_schedule(out->a_pad, out->n_pad, out->k_pad, num_sms, dose_kernel == 1);
+  if (!q.ok) return GMCO_OK;
+  out->ok = 1;
+  out->n_tiles = q.n_tiles; out->segs = q.segs; out->n_chunks = q.n_chunks; out->n_slabs = q.n_slabs;
+  out->compact_cap = q.segs > 36 ? q.segs : 36;
+  out->dose_kernel = q.dose_kernel; out->dose_threads = 320; out->grad_threads = 192;
+  if (q.dose_pair) {
+    const tcl::PairSmem l = tcl::pair_smem(q.G, q.pair_stages);
+    out->dose_stages = q.pair_stages; out->dose_stage_bytes = tcl::kPairEntry; out->dose_smem_bytes = q.pair_smem;
+    out->dose_smem_end = l.end; out->dose_scr_slot = -1; out->dose_tmem_cols = tcl::pair_tmem_cols(q.G);
+  } else {
+    const tcl::DoseSmem l = tcl::dose_smem(q.tlo_resident != 0, q.G, q.dose_stages);
+    out->dose_stages = q.dose_stages; out->dose_stage_bytes = l.stage_bytes; out->dose_smem_bytes = q.dose_smem;
+    out->dose_smem_end = l.end; out->dose_scr_slot = q.tlo_resident ? -1 : l.scr_slot; out->dose_tmem_cols = tcl::dose_tmem_cols(q.G);
+  }
+  const tcl::GradSmem gl = tcl::grad_smem(q.grad_ps, q.G, q.grad_stages);
+  out->grad_ps = q.grad_ps; out->grad_stages = q.grad_stages; out->grad_stage_bytes = gl.stage_bytes;
+  out->grad_smem_bytes = q.grad_smem; out->grad_smem_end = gl.end; out->grad_staging_bytes = gl.staging_bytes;
+  out->grad_tmem_cols = tcl::grad_tmem_cols(out->a_pad);
   return GMCO_OK;
 }
 

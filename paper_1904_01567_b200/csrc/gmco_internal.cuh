@@ -22,6 +22,17 @@ constexpr int kRoundLogCap = 8192;      // rounds whose running-plan count is lo
 // per-plan status codes on the device
 enum : int { PLAN_RUNNING = -1 };
 
+// Device error word (PlanDev::dev_err, 4 ints): [0] DevErr code (0 = none; the first error wins), [1] site =
+// DevErrKernel << 8 | DevErrWait, [2] blockIdx.x | blockIdx.y << 16, [3] detail.  Kernels never trap and never spin
+// without a bound: a wait that does not complete, or a shared-memory / TMEM carve-up that does not fit, is written here,
+// the kernel runs through its normal teardown, and the host turns the word into GMCO_E_CUDA after its next synchronise.
+enum DevErr : int { DEVERR_NONE = 0, DEVERR_WAIT_TIMEOUT = 1, DEVERR_SMEM_LAYOUT = 2, DEVERR_TMEM_LAYOUT = 3 };
+enum DevErrKernel : int { DEVERR_K_DOSE_RESIDENT = 1, DEVERR_K_DOSE_STREAMED = 2, DEVERR_K_DOSE_PAIR = 3, DEVERR_K_GRAD = 4, DEVERR_K_STEP = 5 };
+enum DevErrWait : int {
+  DEVERR_W_EMPTY = 1, DEVERR_W_FULL = 2, DEVERR_W_TG_READY = 3, DEVERR_W_TIN_FULL = 4, DEVERR_W_ACC_FULL = 5,
+  DEVERR_W_ACC_EMPTY = 6, DEVERR_W_CONV = 7, DEVERR_W_HISTORY = 8
+};
+
 // Static description of the case (gmco_create), all device pointers.
 struct CaseDev {
   int N = 0, A = 0, S = 0;          // user sizes
@@ -51,7 +62,8 @@ struct StructHost {
 struct PlanDev {
   int K = 0, K_pad = 0, m = 0;
   float *x = nullptr, *g = nullptr, *p = nullptr, *xt = nullptr;   // [K_pad][A_pad]
-  float *T = nullptr, *T_hi = nullptr, *T_lo = nullptr;            // trial dwell times (GEMM operand)
+  float *T = nullptr;                                              // trial dwell times (GEMM operand), fp32; the dose kernel splits them
+  float *T_lo = nullptr;                                           // tf32 lo part of T: only with more than 256 dwell positions (streamed layout)
   float *Sh = nullptr, *Yh = nullptr;                              // [m][K_pad][A_pad] history
   float *rho = nullptr, *gam = nullptr;                            // [m][K_pad] 1/(s.y) and (s.y)/(y.y)
   float *Weff = nullptr;                                           // [K_pad][2*S] weights * base / n_s
@@ -62,8 +74,9 @@ struct PlanDev {
   int *n_running = nullptr;                                        // [2] ping-pong counter of RUNNING plans
   int *tile_seg = nullptr;                                         // [K_pad / 128 + 1] partial-slot range of each plan tile (tensor route)
   int *round_log = nullptr;                                        // [kRoundLogCap] running plans at the start of round r
-  int *rounds_done = nullptr;                                      // [1] rounds executed by the device-driven loop
+  int *rounds_done = nullptr;                                      // [2] rounds the device-driven loop has gone through (its bound) | rounds that had a running plan
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
+  int *dev_err = nullptr;                                          // [4] device error word (DevErr above)
   // partial results of one evaluation round
   float *Fpart = nullptr; float *Gpart = nullptr;
   float *R = nullptr;               // SIMT route: dF/dd [K_pad][N_alloc]; tensor route: dF/dd / 2 [N_alloc][K_pad]
@@ -97,7 +110,7 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
 int launch_simt_eval(const CaseDev& c, const PlanDev& p, bool write_R, float* dose_out /*[N][K] or null*/,
                      bool dvh_mode, const float* dvh_thr /*[S] device*/, const int* gate, cudaStream_t st);
 int launch_simt_grad(const CaseDev& c, const PlanDev& p, const int* gate, cudaStream_t st);
-int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, cudaStream_t st);
+int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, int* round_ctr, cudaStream_t st);
 int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_rounds, cudaStream_t st);
 int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp, int parity, float g_scale,
                        cudaStream_t st);
@@ -141,15 +154,17 @@ int launch_select(const float* dvh, int K, int S, const SelectArgs& c, int* plan
 
 // tensor path (kernels_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
-TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
-                       char* err, int errlen);
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
+                       cudaStream_t st, char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 int tc_dose_pair(const TcPlan*);           // 1: the dose kernel runs as CTA pairs (its compaction split is per tile PAIR)
+int tc_dose_kernel(const TcPlan*);         // tcl::DoseKernelId of the dose kernel that is dispatched
 int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms);
 const int* tc_tile_seg_dev(const TcPlan*);
 int tc_compact_cap(const TcPlan*);
+// which < 0: both contractions; 0: the dose kernel only; 1: the gradient kernel only
 int launch_tc_eval(const TcPlan* tp, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   int* zero_ctr, int* log_slot, bool compact, cudaStream_t st);
+                   int* zero_ctr, int* log_slot, bool compact, int which, cudaStream_t st);
 
 }  // namespace gmco

@@ -24,8 +24,8 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 struct PlanPtrs {
-  float *x, *g, *p, *xt, *T, *T_hi, *T_lo, *Sh, *Yh, *rho, *gam, *F, *gp, *alpha;
-  int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input;
+  float *x, *g, *p, *xt, *T, *T_lo, *Sh, *Yh, *rho, *gam, *F, *gp, *alpha;
+  int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input, *dev_err;
   int K_pad;
   float *Weff, *WeffC;        // [K_pad][2S] effective weights by plan / by slot
   int* slot;                  // [K_pad] row of plan k in T, R and the partials (= k without compaction)
@@ -33,10 +33,10 @@ struct PlanPtrs {
 
 static PlanPtrs make_ptrs(const PlanDev& p) {
   PlanPtrs q;
-  q.x = p.x; q.g = p.g; q.p = p.p; q.xt = p.xt; q.T = p.T; q.T_hi = p.T_hi; q.T_lo = p.T_lo;
+  q.x = p.x; q.g = p.g; q.p = p.p; q.xt = p.xt; q.T = p.T; q.T_lo = p.T_lo;
   q.Sh = p.Sh; q.Yh = p.Yh; q.rho = p.rho; q.gam = p.gam; q.F = p.F; q.gp = p.gp; q.alpha = p.alpha;
   q.it_done = p.it_done; q.trials = p.trials; q.hcount = p.hcount; q.hhead = p.hhead; q.status = p.status;
-  q.n_running = p.n_running; q.bad_input = p.bad_input; q.K_pad = p.K_pad;
+  q.n_running = p.n_running; q.bad_input = p.bad_input; q.dev_err = p.dev_err; q.K_pad = p.K_pad;
   q.Weff = p.Weff; q.WeffC = p.WeffC; q.slot = p.slot;
   return q;
 }
@@ -53,10 +53,11 @@ __global__ void k_init_plans(PlanPtrs pp, int K, int A, int A_pad, int S, const 
       t0 = bcast ? T0[a] : T0[(long long)k * A + a];
       if (!(t0 >= 0.f) || isinf(t0)) { bad = 1; t0 = 0.f; }
     }
-    const float x = sqrtf(t0), t = x * x, hi = tf32_rn_(t);
+    const float x = sqrtf(t0), t = x * x;
     const long long i = (long long)k * A_pad + a;
     pp.x[i] = x; pp.xt[i] = x; pp.g[i] = 0.f; pp.p[i] = 0.f;
-    pp.T[i] = t; pp.T_hi[i] = hi; pp.T_lo[i] = tf32_rn_(t - hi);
+    pp.T[i] = t;
+    if (pp.T_lo) pp.T_lo[i] = tf32_rn_(t - tf32_rn_(t));   // only the streamed dose layout (more than 256 dwell positions) reads it
   }
   for (int j = threadIdx.x; j < 2 * S; j += blockDim.x) {
     float w = 0.f;
@@ -78,7 +79,8 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
                       const float* struct_scale, cudaStream_t st) {
   if (p.K_pad == 0) return 0;
   cudaMemsetAsync(p.bad_input, 0, sizeof(int), st);
-  cudaMemsetAsync(p.rounds_done, 0, sizeof(int), st);
+  cudaMemsetAsync(p.rounds_done, 0, 2 * sizeof(int), st);
+  cudaMemsetAsync(p.dev_err, 0, 4 * sizeof(int), st);
   k_init_plans<<<p.K_pad, 128, 0, st>>>(make_ptrs(p), p.K, c.A, c.A_pad, c.S, T0, t0_bcast, w_user, struct_scale,
                                         p.Weff);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
@@ -199,13 +201,27 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
                    ::"r"(smem_addr(hS + (size_t)i * sp.A_pad)), "l"(src), "r"(bytes), "r"(bar) : "memory");
     }
   }
-  // every path below waits for the copies before the warp may leave (the CTA's shared memory must outlive them)
+  // Every path below waits for the copies before the warp may leave (the CTA's shared memory must outlive them).
+  // The wait is bounded: copies that have not landed after seconds are a fault of the machine, not a state to spin
+  // in -- the device error word is set (the host reports GMCO_E_CUDA) and the warp goes on.
   auto hist_wait = [&]() {
     const uint32_t bar = smem_addr(&s_bar[warp]);
     uint32_t ok = 0;
-    while (!ok) {
+    unsigned long long t0 = 0;
+    for (uint32_t spins = 1; !ok; ++spins) {
       asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                    : "=r"(ok) : "r"(bar) : "memory");
+      if (!ok && (spins & 63u) == 0u) {
+        unsigned long long now;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+        if (t0 == 0) t0 = now;
+        else if (now - t0 > 4000000000ull) {
+          if (lane == 0 && atomicCAS(pp.dev_err, 0, (int)DEVERR_WAIT_TIMEOUT) == 0) {
+            pp.dev_err[1] = (DEVERR_K_STEP << 8) | DEVERR_W_HISTORY; pp.dev_err[2] = (int)blockIdx.x; pp.dev_err[3] = k;
+          }
+          break;
+        }
+      }
     }
   };
 
@@ -289,8 +305,9 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
         for (int j = 0; j < NPL; ++j)
           if (j < npl) {
             const float pv = pp.p[row + 32 * j];
-            const float xn = fmaf(a2, pv, x[j]), t = xn * xn, hi = tf32_rn_(t);
-            pp.xt[row + 32 * j] = xn; pp.T[trow + 32 * j] = t; pp.T_hi[trow + 32 * j] = hi; pp.T_lo[trow + 32 * j] = tf32_rn_(t - hi);
+            const float xn = fmaf(a2, pv, x[j]), t = xn * xn;
+            pp.xt[row + 32 * j] = xn; pp.T[trow + 32 * j] = t;
+            if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn_(t - tf32_rn_(t));
           }
         if (lane == 0) { pp.alpha[k] = a2; pp.trials[k] = tr; }
       }
@@ -364,9 +381,10 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
       for (int j = 0; j < NPL; ++j)
         if (j < npl) {
           const float pv = -q[j];
-          const float xn = x[j] + pv, t = xn * xn, hi = tf32_rn_(t);
+          const float xn = x[j] + pv, t = xn * xn;
           pp.p[row + 32 * j] = pv; pp.xt[row + 32 * j] = xn;
-          pp.T[trow + 32 * j] = t; pp.T_hi[trow + 32 * j] = hi; pp.T_lo[trow + 32 * j] = tf32_rn_(t - hi);
+          pp.T[trow + 32 * j] = t;
+          if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn_(t - tf32_rn_(t));
         }
       if (lane == 0) { pp.gp[k] = gpn; pp.alpha[k] = 1.f; pp.trials[k] = 0; }
     }
@@ -405,26 +423,28 @@ int launch_step_parity(const CaseDev& c, const PlanDev& p, const StepParams& sp,
 }
 
 // zero the "next round" counter; runs before the contraction kernels of a round
-__global__ void k_round_begin(int* zero_ctr, const int* gate, int* log_slot) {
+__global__ void k_round_begin(int* zero_ctr, const int* gate, int* log_slot, int* round_ctr) {
   *zero_ctr = 0;
   if (log_slot) *log_slot = *gate;
+  if (round_ctr && *gate > 0) *round_ctr += 1;
 }
 
-// tail of the WHILE body (two rounds): loop again while a plan is running and the round budget lasts
+// tail of the WHILE body (two rounds): loop again while a plan is running, the round budget lasts and no kernel has
+// reported a protocol error
 __global__ void k_loop_cond(cudaGraphConditionalHandle cond, const int* __restrict__ n_running, int* rounds_done,
-                            int max_rounds) {
+                            const int* __restrict__ dev_err, int max_rounds) {
   const int r = *rounds_done + 2;
   *rounds_done = r;
-  cudaGraphSetConditional(cond, (n_running[0] > 0 && r < max_rounds) ? 1u : 0u);
+  cudaGraphSetConditional(cond, (n_running[0] > 0 && r < max_rounds && dev_err[0] == 0) ? 1u : 0u);
 }
 
 int launch_loop_cond(cudaGraphConditionalHandle cond, const PlanDev& p, int max_rounds, cudaStream_t st) {
-  k_loop_cond<<<1, 1, 0, st>>>(cond, p.n_running, p.rounds_done, max_rounds);
+  k_loop_cond<<<1, 1, 0, st>>>(cond, p.n_running, p.rounds_done, p.dev_err, max_rounds);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
-int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, cudaStream_t st) {
-  k_round_begin<<<1, 1, 0, st>>>(zero_ctr, gate, log_slot);
+int launch_round_begin(int* zero_ctr, const int* gate, int* log_slot, int* round_ctr, cudaStream_t st) {
+  k_round_begin<<<1, 1, 0, st>>>(zero_ctr, gate, log_slot, round_ctr);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

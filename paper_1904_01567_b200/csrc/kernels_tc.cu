@@ -20,26 +20,24 @@
 // warps 2-5 = epilogue (TMEM lane quadrant = warp_id % 4).  Pipelines are mbarrier rings.
 #include <cudaTypedefs.h>
 #include <stdio.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
 
 #include "gmco_internal.cuh"
 #include "penalty.cuh"
+#include "tc_layout.h"
 
 namespace gmco {
 
 namespace {
 
-// Points per dose chunk = MMA N of the dose contraction.  128, not 64: a kind::tf32 M=128 K=8 MMA costs
+// Points per dose chunk = MMA N of the dose contraction (tcl::kPC).  128, not 64: a kind::tf32 M=128 K=8 MMA costs
 // max(~60, N/2) cycles on sm_100 (measured, profiles/r1_mma_rate.md), so N=64 runs the tensor pipe at half rate.
-constexpr int kPC = 128;
-constexpr int kSlabBytes = kPC * 128;   // one 32-dwell slab of a dose chunk, one part (hi or lo): 16 KB
-constexpr int kTloBox = 128 * 128;      // T_lo: 128 plans x 32 dwell: 16 KB
-constexpr int kTmemGroups = 8;          // dwell groups of T_hi kept in TMEM (256 columns)
+using tcl::kPC; using tcl::kSlabBytes; using tcl::kTloBox; using tcl::kTmemGroups; using tcl::kScratchBytes;
+using tcl::kHalfPC; using tcl::kHalfSlab; using tcl::kPairEntry;
 constexpr int kThreads = 192;
-constexpr uint32_t kWatchdog = 1u << 26;
+static_assert(tcl::kMaxGroups * 32 == kMaxApadTensor, "tc_layout.h and gmco_internal.cuh disagree on the tensor route's limit");
 
 // ---------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -54,37 +52,104 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// no memory ordering (the accumulator hand-back: TMEM accesses are ordered by the tcgen05 waits and fences around it)
-__device__ __forceinline__ void mbar_arrive_relaxed(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try_wait_addr(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
+      "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug traps (launch failure reported by the API) instead of hanging the GPU.
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-    if (++spins > kWatchdog) __trap();
+__device__ __forceinline__ bool mbar_try_wait_cluster_addr(uint32_t bar, uint32_t parity) {   // acquires remote arrivals
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Bounded waits.  A barrier that does not complete is a protocol bug; it must neither hang the GPU nor raise an SM
+// exception (a trap is reported to the whole machine as Xid 13).  A wait that outlasts kWaitLimitNs writes the
+// device error word (gmco_internal.cuh DevErr), raises the CTA's abort flag in shared memory and returns false; every
+// other waiter of the CTA (and, through the error word, of the grid) then gives up as well, all roles fall through to
+// the kernel's normal teardown (barrier, TMEM dealloc, cluster barrier) and the host reports GMCO_E_CUDA after its
+// next synchronise.  The fast path is a short inline spin; the clock is only read on the slow path.
+constexpr unsigned long long kWaitLimitNs = 4000000000ull;   // kernels here run for at most about a millisecond
+constexpr int kFastSpins = 64;
+
+struct Watch {
+  int* err;             // device error word [4]
+  uint32_t abort_addr;  // shared::cta address of this CTA's abort flag
+  int kernel;           // DevErrKernel id, high byte of the reported site
+};
+
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+__device__ __forceinline__ uint32_t ld_flag(uint32_t addr) {
+  uint32_t v; asm volatile("ld.volatile.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
+}
+__device__ __forceinline__ void st_flag(uint32_t addr, uint32_t v) {
+  asm volatile("st.volatile.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __noinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, int cluster_scope, int* err, uint32_t abort_addr,
+                                            int site) {
+  const unsigned long long t0 = global_ns();
+  for (uint32_t spins = 1;; ++spins) {
+    if (cluster_scope ? mbar_try_wait_cluster_addr(bar, parity) : mbar_try_wait_addr(bar, parity)) return true;
+    if ((spins & 15u) == 0u) {
+      if (ld_flag(abort_addr)) return false;
+      const bool failed_elsewhere = *reinterpret_cast<volatile int*>(err) != 0;
+      if (failed_elsewhere || global_ns() - t0 > kWaitLimitNs) {
+        if (!failed_elsewhere && atomicCAS(err, 0, (int)DEVERR_WAIT_TIMEOUT) == 0) {
+          err[1] = site; err[2] = (int)(blockIdx.x | (blockIdx.y << 16)); err[3] = (int)(threadIdx.x | (parity << 16));
+        }
+        st_flag(abort_addr, 1u);
+        return false;
+      }
+    }
   }
 }
-// the same on a shared-memory address that is already a 32-bit value
-__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity) {
-  uint32_t spins = 0, ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (!ok && ++spins > kWatchdog) __trap();
-  } while (!ok);
+__device__ __forceinline__ bool mbar_wait_addr(const Watch& w, uint32_t bar, uint32_t parity, int site) {
+#pragma unroll 1
+  for (int i = 0; i < kFastSpins; ++i)
+    if (mbar_try_wait_addr(bar, parity)) return true;
+  return mbar_wait_slow(bar, parity, 0, w.err, w.abort_addr, (w.kernel << 8) | site);
+}
+__device__ __forceinline__ bool mbar_wait(const Watch& w, uint64_t* bar, uint32_t parity, int site) {
+  return mbar_wait_addr(w, smem_u32(bar), parity, site);
+}
+// a barrier of this CTA on which threads of the peer CTA arrive (shared::cluster arrivals)
+__device__ __forceinline__ bool mbar_wait_cluster(const Watch& w, uint64_t* bar, uint32_t parity, int site) {
+  const uint32_t b = smem_u32(bar);
+#pragma unroll 1
+  for (int i = 0; i < kFastSpins; ++i)
+    if (mbar_try_wait_cluster_addr(b, parity)) return true;
+  return mbar_wait_slow(b, parity, 1, w.err, w.abort_addr, (w.kernel << 8) | site);
+}
+// inside a role's lambda: give the role up when the wait was abandoned
+#define GMCO_WAIT(call) do { if (!(call)) return; } while (0)
+
+// Layout self-check at kernel entry: the carve-up must fit the dynamic shared memory the launch provided and the
+// TMEM columns must fit 512.  A mismatch (a host/device formula drifting apart) is reported through the error word
+// instead of letting a TMA write run past the CTA's window.
+__device__ __forceinline__ uint32_t dynamic_smem_size() {
+  uint32_t v; asm volatile("mov.u32 %0, %%dynamic_smem_size;" : "=r"(v)); return v;
+}
+__device__ __forceinline__ bool layout_fits(int* err, int kernel, uint32_t pad, int smem_end, int tmem_cols) {
+  const bool smem_ok = pad + (uint32_t)smem_end <= dynamic_smem_size(), tmem_ok = tmem_cols <= tcl::kTmemCols;
+  if (smem_ok && tmem_ok) return true;
+  if (threadIdx.x == 0 && atomicCAS(err, 0, (int)(smem_ok ? DEVERR_TMEM_LAYOUT : DEVERR_SMEM_LAYOUT)) == 0) {
+    err[1] = kernel << 8; err[2] = (int)(blockIdx.x | (blockIdx.y << 16)); err[3] = smem_ok ? tmem_cols : (int)pad + smem_end;
+  }
+  return false;
+}
+// abort path of the teardown: give operations that are still in flight (TMA writes into this CTA's shared memory,
+// MMAs into its TMEM) time to land before the memory is given back
+__device__ __forceinline__ void drain_if_aborted(uint32_t abort_addr) {
+  if (ld_flag(abort_addr)) {
+    for (int i = 0; i < 200; ++i) __nanosleep(1000);
+  }
 }
 // one lane of a fully converged warp; the compiler keeps everything around it on the uniform datapath
 __device__ __forceinline__ bool elect_one() {
@@ -221,7 +286,6 @@ __host__ __device__ constexpr uint32_t instr_desc(int n, int a_mn_major, int b_m
 struct Thresholds { float d_lo[GMCO_MAX_STRUCTS], d_hi[GMCO_MAX_STRUCTS]; };
 
 constexpr int kDoseThreads = 320;       // warp 0 TMA, warp 1 MMA, warps 2-9 epilogue (2 per TMEM lane quadrant)
-constexpr int kScratchBytes = 8 * 4096; // T_hi transposition scratch, one 32 x 128 B slab per epilogue warp
 
 struct DoseArgs {
   const float* T;             // [K_pad][A_pad] trial dwell times, fp32; split into tf32 (hi, lo) in the prologue
@@ -235,8 +299,10 @@ struct DoseArgs {
   const int* gate;
   int* zero_ctr;              // start-of-round bookkeeping, done by CTA (0, 0): *zero_ctr = 0, *log_slot = *gate
   int* log_slot;
+  int* round_ctr;             // counts the rounds that had a running plan (gmco_stats.rounds)
   int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, sep_corr, tlo_resident;
   int compact_cap;            // > 0: plans are packed by slot; the CTAs re-split over the tiles that hold running plans
+  int* err;                   // device error word [4] (gmco_internal.cuh DevErr); never null
   Thresholds thr;
 };
 
@@ -244,6 +310,7 @@ struct GradArgs {
   float* Gpart;               // [n_tiles * segs][128][A_pad]
   const int* gate;
   int A_pad, n_slabs, segs, n_stage, compact_cap;
+  int* err;                   // device error word [4]; never null
 };
 
 // Compaction (gmco_options.compaction): k_step packs the running plans into slots [0, n_running), so only the first
@@ -281,6 +348,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   if (a.zero_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
     *a.zero_ctr = 0;
     if (a.log_slot) *a.log_slot = *a.gate;
+    if (a.round_ctr && *a.gate > 0) *a.round_ctr += 1;
   }
   if (a.gate && *a.gate == 0) return;
   int seg = blockIdx.x, tile = blockIdx.y, segs = a.segs;
@@ -288,31 +356,35 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
-  const int stageBytes = kResident ? kSlabBytes : kSlabBytes + kTloBox;
+  const tcl::DoseSmem lay = tcl::dose_smem(kResident, G, a.n_stage);
+  if (!layout_fits(a.err, kResident ? DEVERR_K_DOSE_RESIDENT : DEVERR_K_DOSE_STREAMED, (uint32_t)(smem - smem_raw), lay.end,
+                   tcl::dose_tmem_cols(G)))
+    return;                                         // uniform over the CTA: nothing has been set up yet
+  const int stageBytes = lay.stage_bytes;
   // TMEM holds T_hi of the first kTmemGroups dwell groups (256 columns); with more groups the rest of T_hi lives in
   // shared memory (the "tail", SS MMAs) so that both accumulators always fit.
-  const int Gs = kResident ? 0 : (G > kTmemGroups ? G - kTmemGroups : 0);
-  uint8_t* tlo = smem;                              // resident: T_lo [G][128 plans][128 B]; streamed: T_hi tail [Gs][..]
-  uint8_t* ring = smem + (size_t)(kResident ? G : Gs) * kTloBox;
-  const int ringBytes = a.n_stage * stageBytes;
-  uint8_t* scratch = ring + ringBytes - kScratchBytes;
-  const int scr_slot = (ringBytes - kScratchBytes) / stageBytes;   // first ring slot that overlaps the scratch
-  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + ringBytes);
+  uint8_t* tlo = smem;                              // resident: T_lo [G][128 plans][128 B]; streamed: T_hi tail [G - 8][..]
+  uint8_t* ring = smem + lay.ring_off;
+  uint8_t* scratch = smem + lay.scratch_off;
+  const int scr_slot = lay.scr_slot;                // first ring slot that overlaps the scratch
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + lay.bars_off);
   uint64_t* full = bars;                            // [n_stage]
   uint64_t* empty = bars + a.n_stage;               // [n_stage]
-  uint64_t* tg_ready = bars + 2 * a.n_stage;        // [kMaxApadTensor / 32]: T of dwell group g is in TMEM / smem
-  uint64_t* tin_full = tg_ready + kMaxApadTensor / 32;   // [kMaxApadTensor / 32]: fp32 T of group g has landed (TMA)
-  uint64_t* acc_full = tin_full + kMaxApadTensor / 32;   // [2]
+  uint64_t* tg_ready = bars + 2 * a.n_stage;        // [kMaxGroups]: T of dwell group g is in TMEM / smem
+  uint64_t* tin_full = tg_ready + tcl::kMaxGroups;  // [kMaxGroups]: fp32 T of group g has landed (TMA)
+  uint64_t* acc_full = tin_full + tcl::kMaxGroups;  // [2]
   uint64_t* acc_empty = acc_full + 2;               // [2]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + lay.slot_off);
+  const Watch w{a.err, smem_u32(tmem_slot + 1), kResident ? DEVERR_K_DOSE_RESIDENT : DEVERR_K_DOSE_STREAMED};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int c0 = (int)((long long)seg * a.n_chunks / segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / segs);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
-    for (int i = 0; i < kMaxApadTensor / 32; ++i) { mbar_init(tg_ready + i, 128); mbar_init(tin_full + i, 1); }
+    for (int i = 0; i < tcl::kMaxGroups; ++i) { mbar_init(tg_ready + i, 128); mbar_init(tin_full + i, 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 256); }
+    tmem_slot[1] = 0u;                              // abort flag
     fence_barrier_init();
   }
   if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT_lo); tma_prefetch_desc(&tmT); }
@@ -328,11 +400,12 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   // from ~1e-5 to ~2e-6 of the dose, and the dose error is what the gradient feels near a threshold (r = d - D_lim
   // cancels).  With both accumulators there is room for one buffer only: the epilogue frees it as soon as the values
   // are in registers, the penalty arithmetic and the R stores still overlap the next chunk's MMAs.
-  const uint32_t t_acc = tmem + (G < kTmemGroups ? G : kTmemGroups) * 32;
+  const uint32_t t_acc = tmem + tcl::dose_tmem_acc_col(G);
 
   if (warp == 0) {
     // whole warp walks the ring (uniform control flow); one elected lane issues
-    if (c1 > c0) {
+    auto producer = [&]() {
+      if (c1 <= c0) return;
       const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
       if (kResident) {                         // fp32 T of the tile lands where its lo part will live
         if (elect_one()) {
@@ -349,10 +422,10 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         for (int g2 = 0; g2 < 2 * G; ++g2) {          // entry 2 g: D_hi (+ streamed T_lo), entry 2 g + 1: D_lo
           const int g = g2 >> 1, lo = g2 & 1;
           if (scratch_busy && st >= scr_slot) {       // the prologue's transposition scratch overlaps these slots
-            for (int i = 0; i < G; ++i) mbar_wait(tg_ready + i, 0);
+            for (int i = 0; i < G; ++i) GMCO_WAIT(mbar_wait(w, tg_ready + i, 0, DEVERR_W_TG_READY));
             scratch_busy = false;
           }
-          mbar_wait(empty + st, ph ^ 1);
+          GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
           if (elect_one()) {
             uint8_t* dst = ring + (size_t)st * stageBytes;
             const bool with_t = !lo && !kResident;
@@ -364,9 +437,11 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
         }
       }
-    }
+    };
+    producer();
   } else if (warp == 1) {
-    if (c1 > c0) {
+    auto issuer = [&]() {
+      if (c1 <= c0) return;
       // Issue loop.  Everything is warp-uniform (uniform datapath); one elected lane issues.  Per ring entry: one wait, 8 or 4
       // MMAs whose descriptors differ by 32-bit adds, one commit.
       constexpr uint32_t idesc = instr_desc(kPC, 0, 0);
@@ -378,14 +453,15 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
       int st = 0; uint32_t ph = 0;
       for (int c = c0; c < c1; ++c) {
         const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
-        mbar_wait(acc_empty + b, (use & 1) ^ 1);
+        GMCO_WAIT(mbar_wait(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
         tc_fence_after();
         const uint32_t acc = t_acc + b * (a.sep_corr ? 2 * kPC : kPC), acc_c = a.sep_corr ? acc + kPC : acc;
         uint32_t thi = t_thi, alo = tlo_lo0;   // alo: resident T_lo slab g, or (streamed) T_hi tail slab g - kTmemGroups
         for (int g = 0; g < G; thi += 32, alo += (kResident || g >= kTmemGroups) ? kTloBox >> 4 : 0, ++g) {
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
-          if (c == c0) { mbar_wait(tg_ready + g, 0); tc_fence_after(); }   // first chunk overlaps the prologue
-          mbar_wait_addr(full0 + 8 * st, ph);
+          if (c == c0) { GMCO_WAIT(mbar_wait(w, tg_ready + g, 0, DEVERR_W_TG_READY)); tc_fence_after(); }   // first chunk overlaps the prologue
+          GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
+          tc_fence_after();
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             const uint32_t ad = kResident ? alo : bd + (kSlabBytes >> 4);
@@ -409,7 +485,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           __syncwarp();
           if (++st == n_stage) { st = 0; ph ^= 1; }
           // entry 2 g + 1: D_lo slab: T_hi D_lo
-          mbar_wait_addr(full0 + 8 * st, ph);
+          GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
+          tc_fence_after();
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             if (kResident || g < kTmemGroups) {
@@ -426,7 +503,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           if (++st == n_stage) { st = 0; ph ^= 1; }
         }
       }
-    }
+    };
+    issuer();
   } else {
     const int e = warp - 2;                         // 0..7
     const int q = warp & 3;                         // TMEM lane quadrant this warp may access
@@ -435,7 +513,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
     const int plan = tile * 128 + L;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     float f_lo = 0.f, f_hi = 0.f;
-    if (c1 > c0) {
+    auto epilogue = [&]() {
+      if (c1 <= c0) return;
       // Prologue: the tile's trial dwell times T (fp32, read ONCE) are split here into tf32 parts: hi -> TMEM columns
       // [0, A_pad) (the A operand of T_hi D), lo -> shared memory (the A operand of T_lo D_hi).  Slabs g = h, h + 2, ...;
       // each slab has its own ready barrier, so the first chunk's MMAs start while later slabs are still on their way.
@@ -446,7 +525,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         const int row = q * 32 + lane;
         for (int g = h; g < G; g += 2) {
           uint8_t* base = tlo + (size_t)g * kTloBox + row * 128;
-          mbar_wait(tin_full + g, 0);
+          GMCO_WAIT(mbar_wait(w, tin_full + g, 0, DEVERR_W_TIN_FULL));
           uint32_t v[32];
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
@@ -466,7 +545,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           mbar_arrive(tg_ready + g);
         }
       } else {
-        // streamed-T_lo mode (more than 320 dwell positions): T_lo comes from global memory with every D_hi slab;
+        // streamed-T_lo mode (more than 256 dwell positions): T_lo comes from global memory with every D_hi slab;
         // hi is read from T with coalesced 128 B row loads and transposed through the tail of the ring.
         uint8_t* scr = scratch + e * 4096;
         const int r0 = lane >> 3, c4 = lane & 7;
@@ -525,7 +604,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           wlo_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n]; whi_n = a.Weff[(size_t)plan * 2 * a.S + 2 * s_n + 1];
         }
         const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
-        mbar_wait(acc_full + b, use & 1);
+        GMCO_WAIT(mbar_wait(w, acc_full + b, use & 1, DEVERR_W_ACC_FULL));
         tc_fence_after();
         uint32_t v[2][32];
         const uint32_t t_main = t_acc + lane_base + b * (a.sep_corr ? 2 * kPC : kPC) + h * 64;
@@ -543,8 +622,10 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         } else {
           tmem_ld_wait();
         }
+        // hand the accumulator back: tcgen05.wait::ld above, fence, then a RELEASING arrive (the documented pattern;
+        // .release.cta costs no memory barrier beyond the CTA)
         tc_fence_before();
-        mbar_arrive_relaxed(acc_empty + b);
+        mbar_arrive(acc_empty + b);
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
           const int nvh = nv - sub * 32;
@@ -572,12 +653,13 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           }
         }
       }
-    }
+    };
+    epilogue();
     a.Fpart[(((size_t)tile * segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+  if (warp == 1) { drain_if_aborted(w.abort_addr); tc_fence_after(); tmem_dealloc(tmem, 512); }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -589,11 +671,6 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 // entries.  Only the leader (cluster rank 0) issues MMAs; its `full` barriers collect the bytes of both CTAs' TMA
 // loads, its tg_ready / acc_empty barriers the arrivals of both CTAs' epilogue threads; MMA completion is committed
 // to both CTAs' `empty` / `acc_full` barriers by multicast.  Resident-T_lo layout only (at most 256 dwell positions).
-constexpr int kHalfPC = kPC / 2;
-constexpr int kHalfSlab = kHalfPC * 128;   // 8 KB: 64 points x 32 dwell of one part (hi or lo)
-constexpr int kPairEntry = 2 * kHalfSlab;  // ring entry: TWO dwell groups of a half slab (8 MMAs per barrier round trip:
-                                           // the issuing warp's instruction stream, not the tensor pipe, is the limiter)
-
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r;
 }
@@ -606,30 +683,6 @@ __device__ __forceinline__ uint32_t leader_addr(const void* p) {
 }
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
-}
-// The accumulator hand-back orders TMEM accesses only (tcgen05.wait::ld before, tcgen05.fence after): a RELAXED arrive
-// and wait.  A release at cluster scope would first drain the epilogue's outstanding R stores (MEMBAR.ALL.GPU: measured
-// as the epilogue's top stall) and an acquire invalidates L1 on every pass.
-__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_bar) {
-  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_cluster_relaxed(uint64_t* bar, uint32_t parity) {
-  uint32_t spins = 0, ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.relaxed.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    if (!ok && ++spins > kWatchdog) __trap();
-  } while (!ok);
-}
-__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {   // acquires remote arrivals
-  uint32_t spins = 0, ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    if (!ok && ++spins > kWatchdog) __trap();
-  } while (!ok);
 }
 // this CTA's half of a D slab; the bytes are counted on the LEADER's barrier (a shared::cluster address)
 __device__ __forceinline__ void tma_load_3d_pair(const CUtensorMap* map, void* dst, uint32_t leader_bar, int c0, int c1,
@@ -690,6 +743,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
   if (a.zero_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
     *a.zero_ctr = 0;
     if (a.log_slot) *a.log_slot = *a.gate;
+    if (a.round_ctr && *a.gate > 0) *a.round_ctr += 1;
   }
   if (a.gate && *a.gate == 0) return;                 // both CTAs of a pair take every early exit together
   const int rank = (int)cluster_ctarank();
@@ -699,18 +753,21 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                         // 32-dwell groups, at most kTmemGroups
+  const tcl::PairSmem lay = tcl::pair_smem(G, a.n_stage);
+  // the same numbers in both CTAs of the pair (same launch, same shape): they leave together or not at all
+  if (!layout_fits(a.err, DEVERR_K_DOSE_PAIR, (uint32_t)(smem - smem_raw), lay.end, tcl::pair_tmem_cols(G))) return;
   uint8_t* tlo = smem;                                // T_lo [G][128 plans][128 B]
-  uint8_t* ring = smem + (size_t)G * kTloBox;         // n_stage entries of two half slabs
-  const int ringBytes = a.n_stage * kPairEntry;
+  uint8_t* ring = smem + lay.ring_off;                // n_stage entries of two half slabs
   const int Gp = (G + 1) >> 1;                        // entries per pass over the dwell groups (a missing odd group is zero-filled)
-  uint64_t* bars = reinterpret_cast<uint64_t*>(ring + ringBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + lay.bars_off);
   uint64_t* full = bars;                              // [n_stage]  used in the leader: both CTAs' bytes
   uint64_t* empty = bars + a.n_stage;                 // [n_stage]  in each CTA: multicast commit
   uint64_t* tg_ready = bars + 2 * a.n_stage;          // [8]        used in the leader: 256 arrivals (both CTAs)
   uint64_t* tin_full = tg_ready + kTmemGroups;        // [8]        in each CTA: its own T
   uint64_t* acc_full = tin_full + kTmemGroups;        // [2]        in each CTA: multicast commit
   uint64_t* acc_empty = acc_full + 2;                 // [2]        used in the leader: 512 arrivals
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + lay.slot_off);
+  const Watch w{a.err, smem_u32(tmem_slot + 1), DEVERR_K_DOSE_PAIR};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int c0 = (int)((long long)seg * a.n_chunks / segs), c1 = (int)((long long)(seg + 1) * a.n_chunks / segs);
@@ -719,6 +776,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); }
     for (int i = 0; i < kTmemGroups; ++i) { mbar_init(tg_ready + i, 256); mbar_init(tin_full + i, 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(acc_full + i, 1); mbar_init(acc_empty + i, 512); }
+    tmem_slot[1] = 0u;                                // abort flag
     fence_barrier_init();
   }
   if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); tma_prefetch_desc(&tmT); }
@@ -737,7 +795,8 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
   const uint32_t t_acc = tmem + G * 32;
 
   if (warp == 0) {
-    if (c1 > c0) {
+    auto producer = [&]() {
+      if (c1 <= c0) return;
       const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
       if (elect_one()) {
         for (int g = 0; g < G; ++g) {
@@ -751,7 +810,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
       for (int c = c0; c < c1; ++c) {
         for (int g2 = 0; g2 < 3 * Gp; ++g2) {         // entries 2 p, 2 p + 1: D_lo, D_hi (corrections); 2 Gp + p: D_hi (main)
           const int gp = g2 < 2 * Gp ? g2 >> 1 : g2 - 2 * Gp, lo = g2 < 2 * Gp ? (g2 & 1) ^ 1 : 0;
-          mbar_wait(empty + st, ph ^ 1);
+          GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
           if (elect_one()) {
             if (leader) mbar_expect_tx(full + st, 2u * (uint32_t)kPairEntry);
             tma_load_3d_pair(lo ? &tmD_lo : &tmD_hi, ring + (size_t)st * kPairEntry, lfull0 + 8u * (uint32_t)st, 0,
@@ -761,9 +820,11 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
         }
       }
-    }
+    };
+    producer();
   } else if (warp == 1) {
-    if (leader && c1 > c0) {
+    auto issuer = [&]() {
+      if (!leader || c1 <= c0) return;
       constexpr uint32_t idesc = instr_desc_pair(kPC);
       constexpr uint32_t dhi = desc_hi(1024, kSwz128);
       const int n_stage = a.n_stage;
@@ -771,10 +832,10 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
       const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
       const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
       constexpr uint32_t kG1 = (uint32_t)kHalfSlab >> 4;       // second dwell group of an entry
-      // One ring entry: wait, 4 or 8 MMAs, commit.  kind 0: T_hi D_lo, 1: T_lo D_hi, 2: T_hi D_hi.
+      // One ring entry: wait, 4 or 8 MMAs, commit.  kind 0: T_hi D_lo, 1: T_lo D_hi, 2: T_hi D_hi.  false: wait abandoned.
       auto entry = [&](const int kind, const int gp, const int st, const uint32_t ph, const uint32_t acc, const bool two,
-                       const uint32_t acc_full_bar) {
-        mbar_wait_addr(full0 + 8 * st, ph);
+                       const uint32_t acc_full_bar) -> bool {
+        if (!mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL)) return false;
         tc_fence_after();
         if (elect_one()) {
           const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
@@ -799,6 +860,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
           if (acc_full_bar) tc_commit_pair(acc_full_bar);
         }
         __syncwarp();
+        return true;
       };
       if constexpr (GP > 0) {
         // Static schedule: 3 GP entries per chunk go round a ring of NS entries a whole number of times, so every
@@ -809,25 +871,25 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         const bool odd = (G & 1) != 0;
         for (int c = c0; c < c1; ++c) {
           const int b = (c - c0) & 1, use = (c - c0) >> 1;
-          mbar_wait_cluster_relaxed(acc_empty + b, (use & 1) ^ 1);
+          GMCO_WAIT(mbar_wait_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
           tc_fence_after();
           const uint32_t acc = t_acc + (uint32_t)b * kPC;
 #pragma unroll
           for (int gp = 0; gp < GP; ++gp) {
             const bool two = gp < GP - 1 || !odd;
             if (c == c0) {                            // the first chunk overlaps the prologue, group by group
-              mbar_wait_cluster(tg_ready + 2 * gp, 0);
-              if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
+              GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
+              if (two) GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
               tc_fence_after();
             }
-            entry(0, gp, (2 * gp) % NS, chunk_par ^ (((2 * gp) / NS) & 1), acc, two, 0u);
-            entry(1, gp, (2 * gp + 1) % NS, chunk_par ^ (((2 * gp + 1) / NS) & 1), acc, two, 0u);
+            GMCO_WAIT(entry(0, gp, (2 * gp) % NS, chunk_par ^ (((2 * gp) / NS) & 1), acc, two, 0u));
+            GMCO_WAIT(entry(1, gp, (2 * gp + 1) % NS, chunk_par ^ (((2 * gp + 1) / NS) & 1), acc, two, 0u));
           }
 #pragma unroll
           for (int gp = 0; gp < GP; ++gp) {
             const bool two = gp < GP - 1 || !odd;
-            entry(2, gp, (2 * GP + gp) % NS, chunk_par ^ (((2 * GP + gp) / NS) & 1), acc, two,
-                  gp == GP - 1 ? smem_u32(acc_full + b) : 0u);
+            GMCO_WAIT(entry(2, gp, (2 * GP + gp) % NS, chunk_par ^ (((2 * GP + gp) / NS) & 1), acc, two,
+                            gp == GP - 1 ? smem_u32(acc_full + b) : 0u));
           }
           chunk_par ^= (uint32_t)(REV & 1);
         }
@@ -835,28 +897,29 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         int st = 0; uint32_t ph = 0;
         for (int c = c0; c < c1; ++c) {
           const int b = (c - c0) & 1, use = (c - c0) >> 1;
-          mbar_wait_cluster_relaxed(acc_empty + b, (use & 1) ^ 1);
+          GMCO_WAIT(mbar_wait_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
           tc_fence_after();
           const uint32_t acc = t_acc + (uint32_t)b * kPC;
           for (int gp = 0; gp < Gp; ++gp) {           // corrections first
             const bool two = 2 * gp + 1 < G;
             if (c == c0) {
-              mbar_wait_cluster(tg_ready + 2 * gp, 0);
-              if (two) mbar_wait_cluster(tg_ready + 2 * gp + 1, 0);
+              GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
+              if (two) GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
               tc_fence_after();
             }
-            entry(0, gp, st, ph, acc, two, 0u);
+            GMCO_WAIT(entry(0, gp, st, ph, acc, two, 0u));
             if (++st == n_stage) { st = 0; ph ^= 1; }
-            entry(1, gp, st, ph, acc, two, 0u);
+            GMCO_WAIT(entry(1, gp, st, ph, acc, two, 0u));
             if (++st == n_stage) { st = 0; ph ^= 1; }
           }
           for (int gp = 0; gp < Gp; ++gp) {           // then the large product: D_hi again
-            entry(2, gp, st, ph, acc, 2 * gp + 1 < G, gp == Gp - 1 ? smem_u32(acc_full + b) : 0u);
+            GMCO_WAIT(entry(2, gp, st, ph, acc, 2 * gp + 1 < G, gp == Gp - 1 ? smem_u32(acc_full + b) : 0u));
             if (++st == n_stage) { st = 0; ph ^= 1; }
           }
         }
       }
-    }
+    };
+    issuer();
   } else {
     const int e = warp - 2;                           // 0..7
     const int q = warp & 3;                           // TMEM lane quadrant this warp may access
@@ -865,13 +928,14 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
     const int plan = tile * 128 + L;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     float f_lo = 0.f, f_hi = 0.f;
-    if (c1 > c0) {
+    auto epilogue = [&]() {
+      if (c1 <= c0) return;
       const uint32_t l_tg = leader_addr(tg_ready), l_ae = leader_addr(acc_empty);
       // prologue: split this CTA's T into tf32 hi (TMEM) and lo (in place), as in k_dose_tc<true>
       const int row = q * 32 + lane;
       for (int g = h; g < G; g += 2) {
         uint8_t* base = tlo + (size_t)g * kTloBox + row * 128;
-        mbar_wait(tin_full + g, 0);
+        GMCO_WAIT(mbar_wait(w, tin_full + g, 0, DEVERR_W_TIN_FULL));
         uint32_t v[32];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
@@ -902,15 +966,17 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         }
         const float dlo = a.thr.d_lo[s], dhi = a.thr.d_hi[s];
         const int b = (c - c0) & 1, use = (c - c0) >> 1;
-        mbar_wait(acc_full + b, use & 1);
+        GMCO_WAIT(mbar_wait(w, acc_full + b, use & 1, DEVERR_W_ACC_FULL));
         tc_fence_after();
         uint32_t v[2][32];
         const uint32_t t_main = t_acc + lane_base + (uint32_t)b * kPC + h * 64;
         tmem_ld32(t_main, v[0]);
         tmem_ld32(t_main + 32, v[1]);
         tmem_ld_wait();
+        // hand the accumulator back to the leader: tcgen05.wait::ld above, fence, then a RELEASING arrive at cluster
+        // scope (the documented pattern; the R stores of this chunk come after it and are not held up by it)
         tc_fence_before();
-        mbar_arrive_cluster_relaxed(l_ae + 8u * (uint32_t)b);
+        mbar_arrive_cluster(l_ae + 8u * (uint32_t)b);
 #pragma unroll
         for (int sub = 0; sub < 2; ++sub) {
           const int nvh = nv - sub * 32;
@@ -938,10 +1004,12 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
           }
         }
       }
-    }
+    };
+    epilogue();
     a.Fpart[(((size_t)tile * segs + seg) * 128 + L) * 2 + h] = f_lo + f_hi;
   }
   tc_fence_before();
+  if (warp == 1) drain_if_aborted(w.abort_addr);      // before the peer may tear down as well
   cluster_sync_all();                                 // neither CTA's shared memory, TMEM or barriers may go before both are done
   if (warp == 1) { tc_fence_after(); tmem_dealloc_pair(tmem, 512); }
 }
@@ -960,17 +1028,20 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
   if (a.compact_cap && !compact_remap(*a.gate, a.compact_cap, seg, tile, segs)) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem0 = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint8_t* smem = smem0 + 1024;                     // [barriers 1 KB | ring | (epilogue row staging may run past the ring)]
   const int G = a.A_pad >> 5;
+  const tcl::GradSmem lay = tcl::grad_smem(PS, G, a.n_stage);
+  if (!layout_fits(a.err, DEVERR_K_GRAD, (uint32_t)(smem0 - smem_raw), lay.end, tcl::grad_tmem_cols(a.A_pad))) return;
+  uint8_t* smem = smem0 + lay.ring_off;             // [barriers 1 KB | ring | (epilogue row staging may run past the ring)]
   constexpr int kRBytes = 4 * PS * 128;             // R part: 4 plan groups x PS points x 128 B
-  const int dBytes = G * PS * 128;                  // D part: G dwell groups x PS points x 128 B
-  const int stageBytes = 2 * kRBytes + 2 * dBytes;  // [R | R_lo | D_hi | D_lo]
+  const int dBytes = lay.d_bytes;                   // D part: G dwell groups x PS points x 128 B
+  const int stageBytes = lay.stage_bytes;           // [R | R_lo | D_hi | D_lo]
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem0);
   uint64_t* full = bars;
   uint64_t* empty = bars + a.n_stage;
   uint64_t* conv = bars + 2 * a.n_stage;
   uint64_t* acc_full = bars + 3 * a.n_stage;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+  const Watch w{a.err, smem_u32(tmem_slot + 1), DEVERR_K_GRAD};
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int s0 = (int)((long long)seg * a.n_slabs / segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / segs);
@@ -978,6 +1049,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
   if (threadIdx.x == 0) {
     for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); mbar_init(conv + i, 128); }
     mbar_init(acc_full, 1);
+    tmem_slot[1] = 0u;                              // abort flag
     fence_barrier_init();
   }
   if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmR); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); }
@@ -988,22 +1060,26 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // warp-uniform for the compiler
 
   if (warp == 0) {
-    const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
-    int st = 0; uint32_t ph = 0;
-    for (int s = s0; s < s1; ++s) {
-      mbar_wait(empty + st, ph ^ 1);
-      if (elect_one()) {
-        uint8_t* dst = smem + (size_t)st * stageBytes;
-        mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
-        tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
-        tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);
-        tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
+    auto producer = [&]() {
+      const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
+        if (elect_one()) {
+          uint8_t* dst = smem + (size_t)st * stageBytes;
+          mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
+          tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
+          tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);
+          tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
+        }
+        __syncwarp();
+        if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
-      __syncwarp();
-      if (++st == a.n_stage) { st = 0; ph ^= 1; }
-    }
+    };
+    producer();
   } else if (warp == 1) {
-    if (s1 > s0) {
+    auto issuer = [&]() {
+      if (s1 <= s0) return;
       // The accumulator is A_pad columns wide; one MMA covers at most 256 of them.  When the columns last (A_pad <= 256)
       // the two correction products go into a separate accumulator at column 256 (see k_dose_tc: the tensor core's
       // accumulate truncates).  Lean issue loop: descriptors differ by 32-bit adds.
@@ -1018,7 +1094,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
       const uint32_t conv0 = smem_u32(conv), empty0 = smem_u32(empty);
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        mbar_wait_addr(conv0 + 8 * st, ph);
+        GMCO_WAIT(mbar_wait_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));
         tc_fence_after();
         if (elect_one()) {
           const uint32_t r = base_lo + (uint32_t)st * stage_step;
@@ -1041,73 +1117,77 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
         __syncwarp();
         if (++st == n_stage) { st = 0; ph ^= 1; }
       }
-    }
+    };
+    issuer();
   } else {
     const int q = warp & 3;
     const int L = q * 32 + lane;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-    // main loop: split each arriving R tile into (hi, lo) in place; element-wise, so the swizzle does not matter
-    {
-      const int t = threadIdx.x - 64;               // 0..127
-      int st = 0; uint32_t ph = 0;
-      for (int s = s0; s < s1; ++s) {
-        mbar_wait(full + st, ph);
-        uint8_t* base = smem + (size_t)st * stageBytes + t * 16;
+    auto converter_and_epilogue = [&]() {
+      // main loop: split each arriving R tile into (hi, lo) in place; element-wise, so the swizzle does not matter
+      {
+        const int t = threadIdx.x - 64;               // 0..127
+        int st = 0; uint32_t ph = 0;
+        for (int s = s0; s < s1; ++s) {
+          GMCO_WAIT(mbar_wait(w, full + st, ph, DEVERR_W_FULL));
+          uint8_t* base = smem + (size_t)st * stageBytes + t * 16;
 #pragma unroll
-        for (int i = 0; i < kRBytes / 2048; ++i) {
-          const float4 v = *reinterpret_cast<const float4*>(base + i * 2048);
-          float4 hi, lo;
-          hi.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); lo.x = v.x - hi.x;
-          hi.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); lo.y = v.y - hi.y;
-          hi.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); lo.z = v.z - hi.z;
-          hi.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); lo.w = v.w - hi.w;
-          *reinterpret_cast<float4*>(base + i * 2048) = hi;
-          *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
+          for (int i = 0; i < kRBytes / 2048; ++i) {
+            const float4 v = *reinterpret_cast<const float4*>(base + i * 2048);
+            float4 hi, lo;
+            hi.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); lo.x = v.x - hi.x;
+            hi.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); lo.y = v.y - hi.y;
+            hi.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); lo.z = v.z - hi.z;
+            hi.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); lo.w = v.w - hi.w;
+            *reinterpret_cast<float4*>(base + i * 2048) = hi;
+            *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
+          }
+          fence_proxy_async();
+          mbar_arrive(conv + st);
+          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        }
+      }
+      // Epilogue: thread L owns plan L's row of the tile.  TMEM -> registers -> a padded row in shared memory (the ring is
+      // idle by now; pitch A_pad + 4 floats keeps 16 B stores conflict-free) -> ONE bulk asynchronous copy of the whole
+      // row (4 A_pad bytes, contiguous in Gpart) per thread.  No cross-thread hand-off: a thread copies what it wrote.
+      float* grow = a.Gpart + (((size_t)tile * segs + seg) * 128 + L) * a.A_pad;
+      if (s1 > s0) {
+        GMCO_WAIT(mbar_wait(w, acc_full, 0, DEVERR_W_ACC_FULL));
+        tc_fence_after();
+        float* srow = reinterpret_cast<float*>(smem) + (size_t)L * (a.A_pad + 4);
+        for (int g = 0; g < G; ++g) {
+          uint32_t v[32];
+          tmem_ld32(tmem + lane_base + g * 32, v);
+          if (a.A_pad <= 256) {
+            uint32_t vc[32];
+            tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
+          } else {
+            tmem_ld_wait();
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            *reinterpret_cast<float4*>(srow + g * 32 + 4 * i) =
+                make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                            __uint_as_float(v[4 * i + 3]));
         }
         fence_proxy_async();
-        mbar_arrive(conv + st);
-        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(grow), "r"(smem_u32(srow)),
+                     "r"((uint32_t)a.A_pad * 4u) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");      // shared memory may go once it has been read
+      } else {
+        float4* dst = reinterpret_cast<float4*>(grow);
+        for (int i = 0; i < a.A_pad / 4; ++i) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
       }
-    }
-    // Epilogue: thread L owns plan L's row of the tile.  TMEM -> registers -> a padded row in shared memory (the ring is
-    // idle by now; pitch A_pad + 4 floats keeps 16 B stores conflict-free) -> ONE bulk asynchronous copy of the whole
-    // row (4 A_pad bytes, contiguous in Gpart) per thread.  No cross-thread hand-off: a thread copies what it wrote.
-    float* grow = a.Gpart + (((size_t)tile * segs + seg) * 128 + L) * a.A_pad;
-    if (s1 > s0) {
-      mbar_wait(acc_full, 0);
-      tc_fence_after();
-      float* srow = reinterpret_cast<float*>(smem) + (size_t)L * (a.A_pad + 4);
-      for (int g = 0; g < G; ++g) {
-        uint32_t v[32];
-        tmem_ld32(tmem + lane_base + g * 32, v);
-        if (a.A_pad <= 256) {
-          uint32_t vc[32];
-          tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
-          tmem_ld_wait();
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
-        } else {
-          tmem_ld_wait();
-        }
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-          *reinterpret_cast<float4*>(srow + g * 32 + 4 * i) =
-              make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
-                          __uint_as_float(v[4 * i + 3]));
-      }
-      fence_proxy_async();
-      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(grow), "r"(smem_u32(srow)),
-                   "r"((uint32_t)a.A_pad * 4u) : "memory");
-      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");      // shared memory may go once it has been read
-    } else {
-      float4* dst = reinterpret_cast<float4*>(grow);
-      for (int i = 0; i < a.A_pad / 4; ++i) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
+    };
+    converter_and_epilogue();
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem, 512); }
+  if (warp == 1) { drain_if_aborted(w.abort_addr); tc_fence_after(); tmem_dealloc(tmem, 512); }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1145,99 +1225,52 @@ struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
   CUtensorMap pair_D_hi, pair_D_lo;                // 64-point boxes of the CTA-pair dose kernel
-  int dose_pair = 0, pair_static = 0, pair_stages = 0, pair_smem = 0;
-  int segs = 1, n_tiles = 0;
-  int dose_stages = 0, dose_smem = 0, tlo_resident = 1;
-  int grad_ps = 32, grad_stages = 0, grad_smem = 0;
+  tcl::Schedule sch{};                             // every size the host chose (tc_layout.h)
   int* tile_seg_dev = nullptr;
   Thresholds thr{};
 };
 
-// Point segments per plan tile.  Up to num_sms / n_tiles the grid is one wave of CTAs.  With many tiles one wave leaves
-// SMs idle (79 tiles of a 10 000-plan pool: 79 of 148) or unevenly loaded (C4: 32 tiles x 4 = 128 CTAs), so the grid
-// may run to several waves of shorter CTAs when this model says it pays: time ~ waves x (chunks per CTA + 1), the
-// "+ 1" standing for a CTA's prologue and tail (about one 128-point chunk's worth).
-int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms) {
-  const int n_chunks = (n_pad_points + kPC - 1) / kPC;
-  auto cost = [&](int s) {
-    const int waves = (n_tiles * s + num_sms - 1) / num_sms;
-    return waves * ((n_chunks + s - 1) / s + 1);
-  };
-  const int s0 = num_sms / n_tiles > 0 ? num_sms / n_tiles : 1;
-  int best = s0;
-  for (int s = s0 + 1; s <= 36 && s <= n_chunks; ++s)
-    if (cost(s) < cost(best) && 100 * cost(s) < 95 * cost(s0)) best = s;
-  return best;
+int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms) { return tcl::choose_segs(n_tiles, n_pad_points, num_sms); }
+
+// Opt every tensor kernel in to the full dynamic shared memory once per process.  The attribute is per function and
+// process-global: setting it to one handle's exact size would lower the cap under other live handles.
+static cudaError_t tc_set_smem_caps() {
+  static cudaError_t done = cudaErrorUnknown;
+  if (done == cudaSuccess) return done;
+  cudaError_t e = cudaFuncSetAttribute(k_dose_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  done = e;
+  return e;
 }
 
-TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, cudaStream_t st,
-                       char* err, int errlen) {
-  constexpr int kSmemMax = 227 * 1024;
+TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
+                       cudaStream_t st, char* err, int errlen) {
   if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
-  t->n_tiles = p.K_pad / kPlanTile;
-  t->segs = tc_choose_segs(t->n_tiles, c.N_pad, num_sms);
+  t->sch = tcl::choose_schedule(c.A_pad, c.N_pad, p.K_pad, num_sms, force_single);
+  const tcl::Schedule& q = t->sch;
+  if (!q.ok) { snprintf(err, errlen, "shared memory too small for the tensor kernels' rings at this shape"); delete t; return nullptr; }
   for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
-  const int G = c.A_pad / 32;
-  // dose kernel: T_lo resident when it leaves room for >= 2 ring stages, else streamed with every D slab
-  const int slack = 1024 /*alignment*/ + 512 /*barriers*/;
-  t->tlo_resident = (G <= kTmemGroups && G * kTloBox + 4 * kSlabBytes + slack <= kSmemMax) ? 1 : 0;
-  const int fixed = (t->tlo_resident ? G : (G > kTmemGroups ? G - kTmemGroups : 0)) * kTloBox + slack;
-  const int stageB = t->tlo_resident ? kSlabBytes : kSlabBytes + kTloBox;
-  t->dose_stages = (kSmemMax - fixed) / stageB;
-  if (t->dose_stages > 12) t->dose_stages = 12;
-  if (t->dose_stages * stageB < kScratchBytes) { snprintf(err, errlen, "shared memory too small for the dose ring"); delete t; return nullptr; }
-  t->dose_smem = fixed + t->dose_stages * stageB;
-  // gradient kernel
-  // 16-point stages: the ring is deeper in stages than with 32 (C3: 4 x 48 KB instead of 2 x 96 KB), measured faster
-  t->grad_ps = 16;
-  const int stage = 2 * 4 * t->grad_ps * 128 + 2 * G * t->grad_ps * 128;
-  const int staging = 128 * (c.A_pad + 4) * 4;     // epilogue: one padded accumulator row per plan
-  t->grad_stages = (kSmemMax - 2048) / stage;
-  if (t->grad_stages > 9) t->grad_stages = 9;
-  if (t->grad_stages < 2) { snprintf(err, errlen, "shared memory too small for the gradient ring"); delete t; return nullptr; }
-  t->grad_smem = 2048 + (t->grad_stages * stage > staging ? t->grad_stages * stage : staging);
+  const int G = q.G;
   const CUtensorMapSwizzle sK = CU_TENSOR_MAP_SWIZZLE_128B, sMN = CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
   bool ok = make_map(&t->dose_D_hi, c.D_hi, c.N_alloc, c.A_pad, kPC, 1, sK) &&
             make_map(&t->dose_D_lo, c.D_lo, c.N_alloc, c.A_pad, kPC, 1, sK) &&
-            make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK) &&
             make_map(&t->dose_T, p.T, p.K_pad, c.A_pad, 128, 1, sK) &&
-            make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, t->grad_ps, 4, sMN) &&
-            make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, t->grad_ps, G, sMN) &&
-            make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, t->grad_ps, G, sMN);
-  // CTA-pair dose kernel: resident layout, an even number of plan tiles and of dwell groups (GMCO_DOSE_PAIR=0 keeps the
-  // single-CTA kernel).  The kernel handles an odd group count (zero-filled half entry), but that path has no GPU
-  // parity record yet, so such shapes stay on k_dose_tc.
-  {
-    const char* env = getenv("GMCO_DOSE_PAIR");
-    t->dose_pair = t->tlo_resident && t->n_tiles % 2 == 0 && G % 2 == 0 && !(env && env[0] == '0');
-    if (t->dose_pair) {
-      const int fixedp = G * kTloBox + slack;
-      t->pair_stages = (kSmemMax - fixedp) / kPairEntry;
-      if (t->pair_stages > 12) t->pair_stages = 12;
-      t->pair_smem = fixedp + t->pair_stages * kPairEntry;
-      ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
-           make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
-      // static issue schedule for the production shape (A_pad 193..256: 12 entries per chunk, ring of 6)
-      t->pair_static = (G + 1) / 2 == 4 && t->pair_stages >= 6;
-      if (t->pair_static) { t->pair_stages = 6; t->pair_smem = fixedp + 6 * kPairEntry; }
-      if (ok && (t->pair_static ? cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem)
-                                : cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->pair_smem)) != cudaSuccess) ok = false;
-      if (getenv("GMCO_DEBUG")) {
-        cudaLaunchConfig_t cfg = {}; cfg.gridDim = dim3(t->n_tiles, t->segs); cfg.blockDim = dim3(kDoseThreads); cfg.dynamicSmemBytes = t->pair_smem;
-        int nc = -1; cudaError_t o = cudaOccupancyMaxActiveClusters(&nc, k_dose_tc_pair<0, 0>, &cfg);
-        cudaFuncAttributes fa{}; cudaFuncGetAttributes(&fa, k_dose_tc_pair<0, 0>);
-        fprintf(stderr, "[gmco] pair kernel: grid (%d, %d) smem %d stages %d regs %d static smem %zu clusters %d (%s) ok %d\n", t->segs, t->n_tiles,
-                t->pair_smem, t->pair_stages, fa.numRegs, fa.sharedSizeBytes, nc, cudaGetErrorName(o), (int)ok);
-      }
-    }
-  }
+            (q.tlo_resident || (p.T_lo && make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK))) &&
+            make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, q.grad_ps, 4, sMN) &&
+            make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, q.grad_ps, G, sMN) &&
+            make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, q.grad_ps, G, sMN);
+  if (q.dose_pair)
+    ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
+         make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
-  cudaError_t e = t->tlo_resident ? cudaFuncSetAttribute(k_dose_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem)
-                                   : cudaFuncSetAttribute(k_dose_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, t->dose_smem);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
-  std::vector<int> seg(t->n_tiles + 1);
-  for (int i = 0; i <= t->n_tiles; ++i) seg[i] = i * t->segs;
+  if (q.tlo_resident) t->dose_T_lo = t->dose_T;   // the resident layout splits T in the kernel; the map is never used for a load
+  cudaError_t e = tc_set_smem_caps();
+  std::vector<int> seg(q.n_tiles + 1);
+  for (int i = 0; i <= q.n_tiles; ++i) seg[i] = i * q.segs;
   t->tile_seg_dev = p.tile_seg;                    // lives in the plan arena; pageable source: staged before the call returns
   if (e == cudaSuccess) e = cudaMemcpyAsync(t->tile_seg_dev, seg.data(), seg.size() * sizeof(int), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) { snprintf(err, errlen, "tensor plan setup: %s", cudaGetErrorString(e)); tc_plan_destroy(t); return nullptr; }
@@ -1249,37 +1282,50 @@ void tc_plan_destroy(TcPlan* t) {
   delete t;
 }
 
-int tc_num_segments(const TcPlan* t) { return t->n_tiles * t->segs; }
-int tc_dose_pair(const TcPlan* t) { return t->dose_pair; }
+int tc_num_segments(const TcPlan* t) { return t->sch.n_tiles * t->sch.segs; }
+int tc_dose_pair(const TcPlan* t) { return t->sch.dose_pair; }
+int tc_dose_kernel(const TcPlan* t) { return t->sch.dose_kernel; }
 const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
 
 // at least the static split (a single tile keeps all its CTAs), at most 36 segments: k_step reads one gradient partial
 // per segment, two batches of 18 (kernels_lbfgs.cu)
-int tc_compact_cap(const TcPlan* t) { return t->segs > 36 ? t->segs : 36; }
+int tc_compact_cap(const TcPlan* t) { return t->sch.segs > 36 ? t->sch.segs : 36; }
 
+// which < 0: both contractions; 0: the dose kernel only; 1: the gradient kernel only (per-kernel timing, gmco_set_profiling)
 int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* dose_dbg, const int* gate,
-                   int* zero_ctr, int* log_slot, bool compact, cudaStream_t st) {
-  dim3 grid(t->segs, t->n_tiles);
-  DoseArgs da{};
-  da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = compact ? p.WeffC : p.Weff;
-  da.compact_cap = compact ? tc_compact_cap(t) : 0;
-  da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
-  da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S; da.n_chunks = (c.N_pad + kPC - 1) / kPC;
-  da.segs = t->segs; da.n_stage = t->dose_stages; da.sep_corr = 1;                                // T_hi takes at most 256 TMEM columns: both accumulators always fit
-  da.n_acc = 1;
-  da.tlo_resident = t->tlo_resident; da.thr = t->thr;
-  if (t->dose_pair) {
-    da.n_stage = t->pair_stages;
-    if (t->pair_static) k_dose_tc_pair<4, 6><<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
-    else k_dose_tc_pair<0, 0><<<dim3(t->n_tiles, t->segs), kDoseThreads, t->pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
-  } else if (t->tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
-  else k_dose_tc<false><<<grid, kDoseThreads, t->dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
-  if (cudaPeekAtLastError() != cudaSuccess) return -1;   // left for the caller's message
-  GradArgs ga{};
-  ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = c.N_pad / t->grad_ps; ga.segs = t->segs;
-  ga.n_stage = t->grad_stages; ga.compact_cap = da.compact_cap;
-  k_grad_tc<16><<<grid, kThreads, t->grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
-  return cudaGetLastError() == cudaSuccess ? 2 : -1;
+                   int* zero_ctr, int* log_slot, bool compact, int which, cudaStream_t st) {
+  const tcl::Schedule& q = t->sch;
+  dim3 grid(q.segs, q.n_tiles);
+  int n = 0;
+  const int cap = compact ? tc_compact_cap(t) : 0;
+  if (which != 1) {
+    DoseArgs da{};
+    da.T = p.T; da.R = p.R; da.Fpart = p.Fpart; da.Weff = compact ? p.WeffC : p.Weff;
+    da.compact_cap = cap; da.err = p.dev_err;
+    da.tile_struct = c.tile_struct; da.tile_valid = c.tile_valid; da.row_src = c.row_src; da.dose_dbg = dose_dbg;
+    da.gate = gate; da.zero_ctr = zero_ctr; da.log_slot = log_slot; da.round_ctr = zero_ctr ? p.rounds_done + 1 : nullptr; da.A_pad = c.A_pad; da.K_pad = p.K_pad; da.K = p.K; da.S = c.S;
+    da.n_chunks = q.n_chunks;
+    da.segs = q.segs; da.n_stage = q.dose_stages; da.sep_corr = 1;   // T_hi takes at most 256 TMEM columns: both accumulators always fit
+    da.n_acc = 1;
+    da.tlo_resident = q.tlo_resident; da.thr = t->thr;
+    if (q.dose_pair) {
+      da.n_stage = q.pair_stages;
+      if (q.pair_static) k_dose_tc_pair<4, 6><<<dim3(q.n_tiles, q.segs), kDoseThreads, q.pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
+      else k_dose_tc_pair<0, 0><<<dim3(q.n_tiles, q.segs), kDoseThreads, q.pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
+    } else if (q.tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, q.dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+    else k_dose_tc<false><<<grid, kDoseThreads, q.dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+    if (cudaPeekAtLastError() != cudaSuccess) return -1;   // left for the caller's message
+    ++n;
+  }
+  if (which != 0) {
+    GradArgs ga{};
+    ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = q.n_slabs; ga.segs = q.segs;
+    ga.n_stage = q.grad_stages; ga.compact_cap = cap; ga.err = p.dev_err;
+    k_grad_tc<16><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+    if (cudaGetLastError() != cudaSuccess) return -1;
+    ++n;
+  }
+  return n;
 }
 
 }  // namespace gmco

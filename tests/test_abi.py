@@ -24,7 +24,7 @@ def test_header_declares_the_three_calls_of_the_north_star():
     names = _declared_functions()
     for required in ("gmco_create", "gmco_optimize", "gmco_result", "gmco_evaluate", "gmco_destroy",
                      "gmco_last_error", "gmco_version", "gmco_default_options", "gmco_get_stats", "gmco_sa_run", "gmco_select_plan",
-                     "gmco_pareto_front", "gmco_dose_rate_matrix"):
+                     "gmco_pareto_front", "gmco_dose_rate_matrix", "gmco_tc_schedule", "gmco_set_profiling"):
         assert required in names
 
 
@@ -36,16 +36,17 @@ def test_library_exports_every_declared_symbol(built_lib):
 
 def test_version_and_default_options(built_lib):
     import paper_1904_01567_b200 as g
-    assert g.gmco_version() == 120
+    assert g.gmco_version() == 130
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
-    assert o.compaction == 1 and list(o.reserved) == [0]
+    assert o.compaction == 1 and o.dose_kernel == 0 and list(o.reserved) == [0, 0]
 
 
 def test_struct_layouts_match_the_header(built_lib):
     import paper_1904_01567_b200.binding as b
-    assert ctypes.sizeof(b._Structure) == 28 and ctypes.sizeof(b.Options) == 32 and ctypes.sizeof(b.Stats) == 40
+    assert ctypes.sizeof(b._Structure) == 28 and ctypes.sizeof(b.Options) == 40 and ctypes.sizeof(b.Stats) == 56
+    assert ctypes.sizeof(b.TcInfo) == 28 * 4
     assert ctypes.sizeof(b.Criterion) == 20
 
 
@@ -64,6 +65,9 @@ def test_argument_errors_are_reported_without_a_gpu(built_lib):
     assert e.value.code == -1
     with pytest.raises(g.GmcoError) as e:
         g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(compaction=2))
+    assert e.value.code == -1 and "options" in str(e.value)
+    with pytest.raises(g.GmcoError) as e:
+        g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(dose_kernel=2))
     assert e.value.code == -1 and "options" in str(e.value)
     with pytest.raises(g.GmcoError) as e:
         g.gmco_create(np.zeros((8, 500), np.float32), [gc.Structure("s", 8, 1, 2, 1, 1, 0, 0)], 15.0)

@@ -1,4 +1,6 @@
 """Pins of the oracle's DVH indices (A17) and SA chain (config 5, c.5)."""
+from pathlib import Path
+
 import numpy as np
 import pytest
 
@@ -30,6 +32,37 @@ def test_v100_counts_ties_as_covered_and_skips_other_structures():
     dose = np.array([15.0, 14.999999, 20.0, 3.0, 99.0, 99.0, 11.25, 11.2, 12.0, 0.0])
     out = oracle.dvh(dose, st, 15.0)
     assert out == pytest.approx([50.0, 0.0, 50.0])
+
+
+def _sa_hand_case():
+    import gmco_cases as gc
+    D = np.array([[1.0, 0.0], [0.0, 2.0]], np.float32)
+    st = [gc.Structure("A", 1, 10.0, np.inf, 1.0, 0.0, 0, 0.0), gc.Structure("B", 1, -np.inf, 4.0, 0.0, 1.0, 0, 0.0)]
+    w = np.array([[1.0, 0.0], [0.0, 1.0]], np.float32)
+    rows = [ln.split() for ln in (Path(__file__).parent / "golden" / "sa_chain_hand_case.txt").read_text().splitlines()
+            if ln and not ln.startswith("#")]
+    assert rows[0] == "scenario n j z u t0 t1 F n_accepted".split()
+    rows = [[float(v) for v in r] for r in rows[1:]]
+    setup = {1: dict(T0=np.array([8.0, 1.0], np.float32), temp0=2.0, cooling=0.5),
+             2: dict(T0=np.array([10.0, 2.0], np.float32), temp0=1.0, cooling=0.995)}
+    return D, st, w, rows, setup
+
+
+@pytest.mark.parametrize("scenario", [1, 2])
+def test_sa_move_clip_floor_metropolis_and_cooling_against_the_hand_worked_chain(scenario):
+    """tests/golden/sa_chain_hand_case.txt: downhill accept, uphill accept with u just below exp(-dF/T_n), uphill reject
+    with u just above, a move clipped at 0, a move whose width is the 0.01 tau floor, and T_n = temp0 cooling^n at
+    n = 0..3 bracketed from both sides.  State after every prefix of the chain (BASELINE.json configs[4])."""
+    D, st, w, rows, setup = _sa_hand_case()
+    rows = [r for r in rows if int(r[0]) == scenario]
+    cfg = setup[scenario]
+    j = np.array([r[2] for r in rows], np.int32); z = np.array([r[3] for r in rows]); u = np.array([r[4] for r in rows])
+    assert [int(r[1]) for r in rows] == list(range(len(rows)))
+    for n, r in enumerate(rows):
+        out = oracle.sa_chain(D, st, w, cfg["T0"], 5.0, j[:n + 1], z[:n + 1], u[:n + 1], temp0=cfg["temp0"], cooling=cfg["cooling"])
+        assert out["t"] == pytest.approx([r[5], r[6]], rel=1e-12, abs=1e-15), f"dwell times after step {n}"
+        assert out["F"] == pytest.approx(r[7], rel=1e-12, abs=1e-15), f"objective after step {n}"
+        assert out["n_accepted"] == int(r[8]), f"accepted moves after step {n}"
 
 
 def _draws(case, steps, seed):
