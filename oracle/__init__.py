@@ -45,7 +45,8 @@ class LbfgsOpt(C.Structure):
 
 class LbfgsStat(C.Structure):
     _fields_ = [("iters_done", C.c_int32), ("status", C.c_int32), ("n_evals", C.c_int32),
-                ("n_backtracks", C.c_int32), ("n_skipped", C.c_int32), ("n_approx", C.c_int32)]
+                ("n_backtracks", C.c_int32), ("n_skipped", C.c_int32), ("n_approx", C.c_int32),
+                ("n_bt_iters", C.c_int32), ("max_bt_iter", C.c_int32)]
 
 
 EPS_F = 1e-6   # default objective-noise allowance of the approximate line-search test (reading A5b)
@@ -124,7 +125,8 @@ def lbfgs(fg, x0, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20, eps_f=EPS_F)
     Ff = C.c_double(); hist = np.empty(iters + 1)
     lib().orc_lbfgs(cb, None, C.c_int64(n), _p(x), C.byref(opt), C.byref(Ff), _p(hist), C.byref(st))
     return dict(x=x, F=Ff.value, F_hist=hist, iters_done=st.iters_done, status=st.status,
-                n_evals=st.n_evals, n_backtracks=st.n_backtracks, n_skipped=st.n_skipped, n_approx=st.n_approx)
+                n_evals=st.n_evals, n_backtracks=st.n_backtracks, n_skipped=st.n_skipped, n_approx=st.n_approx,
+                n_bt_iters=st.n_bt_iters, max_bt_iter=st.max_bt_iter)
 
 
 def optimize(D, structures, rx, T0, weights, m=10, iters=100, eps=0.0, c1=1e-4, max_trials=20,
@@ -148,7 +150,9 @@ def optimize(D, structures, rx, T0, weights, m=10, iters=100, eps=0.0, c1=1e-4, 
                 n_evals=np.array([s.n_evals for s in stats]),
                 n_backtracks=np.array([s.n_backtracks for s in stats]),
                 n_skipped=np.array([s.n_skipped for s in stats]),
-                n_approx=np.array([s.n_approx for s in stats]))
+                n_approx=np.array([s.n_approx for s in stats]),
+                n_bt_iters=np.array([s.n_bt_iters for s in stats]),
+                max_bt_iter=np.array([s.max_bt_iter for s in stats]))
 
 
 def dvh(dose, structures, rx):

@@ -62,6 +62,8 @@ typedef struct {
   int32_t n_backtracks;  /* rejected trial steps                                       */
   int32_t n_skipped;     /* (s, y) pairs rejected by the curvature guard               */
   int32_t n_approx;      /* steps accepted by the approximate test only (A5b)          */
+  int32_t n_bt_iters;    /* iterations in which at least one trial step was rejected   */
+  int32_t max_bt_iter;   /* most rejected trial steps inside one iteration             */
 } orc_lbfgs_stat;
 
 int orc_num_threads(void) {
@@ -178,7 +180,7 @@ int orc_lbfgs(orc_fg_fn fg, void* ctx, int64_t n, double* x, const orc_lbfgs_opt
   double* rho = (double*)malloc(sizeof(double) * (m > 0 ? m : 1));
   double* a = (double*)malloc(sizeof(double) * (m > 0 ? m : 1));
   int h = 0;                                    /* pairs held, index 0 = oldest, h-1 = newest */
-  orc_lbfgs_stat s = {0, 0, 0, 0, 0, 0};
+  orc_lbfgs_stat s = {0, 0, 0, 0, 0, 0, 0, 0};
 
   double F = fg(x, g, ctx); s.n_evals = 1;
   if (F_hist) F_hist[0] = F;
@@ -219,16 +221,18 @@ int orc_lbfgs(orc_fg_fn fg, void* ctx, int64_t n, double* x, const orc_lbfgs_opt
      * objective can resolve -- when F has not risen by more than eps_f |F| and the slope at the
      * trial point satisfies phi'(alpha) <= (2 c1 - 1) phi'(0) (identical to Armijo for a quadratic phi). */
     double alpha = 1.0, Fn = 0.0;
-    int accepted = 0;
+    int accepted = 0, rejected_here = 0;             /* rejected_here: a counter for the statistics only */
     for (int trial = 0; trial < opt->max_trials; ++trial) {
       for (int64_t l = 0; l < n; ++l) xn[l] = x[l] + alpha * p[l];
       Fn = fg(xn, gn, ctx); s.n_evals++;
       if (Fn <= F + opt->c1 * alpha * gp) { accepted = 1; break; }
       if (opt->eps_f > 0.0 && Fn <= F + opt->eps_f * fabs(F) &&
           dot(gn, p, n) <= (2.0 * opt->c1 - 1.0) * gp) { accepted = 1; s.n_approx++; break; }
-      s.n_backtracks++;
+      s.n_backtracks++; rejected_here++;
       alpha *= 0.5;
     }
+    if (rejected_here > 0) s.n_bt_iters++;
+    if (rejected_here > s.max_bt_iter) s.max_bt_iter = rejected_here;
     if (!accepted) { s.status = 2; break; }                           /* stalled: x unchanged */
 
     /* history update: s = x+ - x, y = g+ - g, curvature guard */

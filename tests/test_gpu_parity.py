@@ -84,24 +84,43 @@ def test_evaluation_parity_max_dwell_count(g, prec):
     _check_eval(g, c, prec, np.repeat(c.T0[None], 5, axis=0))
 
 
+WIDE = [(18, 16), (22, 16), (24, 16)]
+
+
+def _wide_case(n_cath, n_pos):
+    c = gc.make_case("C1", n_cath=n_cath, n_pos=n_pos, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
+    assert c.n_dwell == n_cath * n_pos
+    return c
+
+
 @pytest.mark.parametrize("prec", PRECISIONS)
 def test_evaluation_parity_more_than_256_dwell_positions(g, prec):
     """288, 352 and 384 dwell positions (C4's count).  Above 256 the T_lo operand is streamed with every D_hi slab and
     the T_hi groups beyond TMEM's 256 columns are read from a shared-memory tail, so that the separate correction
     accumulator still fits.  K = 130 gives two plan tiles, the point counts give ragged 64-row tiles and a ragged last
-    128-point chunk.  Points: random starts, and the WORST case for the gradient -- uniform dwell times scaled so that
-    the mean prostate dose sits on the 15 Gy threshold, where r = d - D_lim cancels and a dose error of 5e-6 shows
-    up 20-fold in the gradient.  Dose and objective are held to the north_star's 1e-4; the gradient of these
-    threshold-sitting plans to 2e-4 on the tensor route (measured 1.4e-4: the dot products are 1.5 times longer than
-    at 256 positions), to 1e-4 on the fp32 route."""
-    for n_cath, n_pos in ((18, 16), (22, 16), (24, 16)):
-        c = gc.make_case("C1", n_cath=n_cath, n_pos=n_pos, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
-        assert c.n_dwell == n_cath * n_pos
-        tol = TOL_EVAL if prec == 1 else 2e-4
+    128-point chunk.  Random starts: north_star's 1e-4 on dose, objective and gradient, both routes."""
+    for n_cath, n_pos in WIDE:
+        c = _wide_case(n_cath, n_pos)
         for T in _eval_points(c, n_random=2)[1:3]:
-            _check_eval(g, c, prec, T, tol_grad=tol)
-        worst = np.repeat(c.T0[None], 130, axis=0) * np.linspace(0.6, 1.4, 130)[:, None].astype(np.float32)
-        _check_eval(g, c, prec, worst, tol_grad=tol)
+            _check_eval(g, c, prec, T)
+
+
+@pytest.mark.parametrize("n_cath,n_pos", WIDE)
+@pytest.mark.parametrize("prec", PRECISIONS)
+def test_evaluation_parity_more_than_256_dwell_positions_threshold_sitting_plans(g, prec, n_cath, n_pos):
+    """The WORST case for the gradient: uniform dwell times scaled so that the mean prostate dose sits on the 15 Gy
+    threshold, where r = d - D_lim cancels and a dose error of 5e-6 shows up 20-fold in the gradient.  The bar is
+    north_star's 1e-4 on every quantity.  KNOWN SHORTFALL: on the tensor route the gradient of these
+    plans measured 1.0-1.4e-4 in round 1 (48 truncating adds into one TMEM accumulator); the test reports that as XFAIL,
+    not as a pass, and fails outright above 2e-4 or on dose / objective.  The plain-fp32 route must meet 1e-4."""
+    c = _wide_case(n_cath, n_pos)
+    worst = np.repeat(c.T0[None], 130, axis=0) * np.linspace(0.6, 1.4, 130)[:, None].astype(np.float32)
+    if prec == 1:
+        _check_eval(g, c, prec, worst)
+        return
+    _, _, e_g = _check_eval(g, c, prec, worst, tol_grad=2e-4)        # dose and F are held to 1e-4 inside
+    if e_g >= TOL_EVAL:
+        pytest.xfail(f"gradient of threshold-sitting plans at {c.n_dwell} dwell positions: {e_g:.2e} >= 1e-4 (known, DESIGN.md 5.6)")
 
 
 @pytest.mark.parametrize("prec", PRECISIONS)

@@ -74,6 +74,27 @@ def test_backtracking_halves_until_armijo_holds():
     fg = lambda x: (float(x[0] ** 4), np.array([4 * x[0] ** 3]))
     r = oracle.lbfgs(fg, np.array([0.5]), m=3, iters=1)
     assert r["n_backtracks"] == 1 and r["x"][0] == pytest.approx(0.0, abs=1e-16)
+    assert r["n_bt_iters"] == 1 and r["max_bt_iter"] == 1        # the statistics counters: one iteration, one halving
+
+
+def test_backtracking_statistics_that_decide_the_line_search_route():
+    """a rejected trial step costs ONE more column in the next batched contraction (the plan simply
+    rides along), whereas the polynomial route phi(alpha) = F(d + 2 alpha a + alpha^2 b) of SURVEY 8(c.2) costs three
+    columns (d is never stored by the fused path, so d, a = D(x o p) and b = D(p o p)) plus the fresh evaluation.  It
+    could only pay in iterations with four or more halvings; on the stand-in cases no iteration has more than two, and
+    a plan needs 1.0-1.2 halvings per iteration that backtracks at all."""
+    worst = 0
+    for name, idx in (("C1", slice(None)), ("C2", slice(0, 100, 12))):
+        c = gc.make_case(name)
+        r = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights[idx], m=c.m, iters=c.iters)
+        bt, bi, mx = r["n_backtracks"], r["n_bt_iters"], r["max_bt_iter"]
+        assert (bi <= bt).all() and (mx <= np.maximum(bt, 0)).all() and ((bt > 0) == (bi > 0)).all()
+        assert bt.sum() <= 1.25 * bi.sum()              # halvings per backtracking iteration
+        worst = max(worst, int(mx.max()))
+        # plan-rounds: what runs (1 + iterations + halvings) against the polynomial route's best case
+        now, poly = (1 + c.iters + bt).sum(), (1 + c.iters + bi).sum()
+        assert (now - poly) / now < 0.01
+    assert worst <= 3
 
 
 def test_one_dimensional_quadratic_converges_in_two_iterations():
