@@ -461,7 +461,6 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
           if (c == c0) { GMCO_WAIT(mbar_wait(w, tg_ready + g, 0, DEVERR_W_TG_READY)); tc_fence_after(); }   // first chunk overlaps the prologue
           GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
-          tc_fence_after();
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             const uint32_t ad = kResident ? alo : bd + (kSlabBytes >> 4);
@@ -486,7 +485,6 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           if (++st == n_stage) { st = 0; ph ^= 1; }
           // entry 2 g + 1: D_lo slab: T_hi D_lo
           GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
-          tc_fence_after();
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             if (kResident || g < kTmemGroups) {
