@@ -106,7 +106,12 @@ typedef struct gmco_options {
                          plan tile; 1: always one CTA per plan tile.  Both compute the same products; they differ
                          in partial-sum order (low-order bits).  gmco_stats.dose_kernel says which one ran.
                                                                                   default 0        */
-  int32_t reserved[2];/* must be 0                                                                */
+  int32_t wide_accum; /* above 256 dwell positions (streamed T_lo layout) only.  1: the main product T_hi D_hi is
+                         accumulated in TWO TMEM accumulators (first / second half of the dwell groups) that the
+                         epilogue sums in fp32, which halves the tensor core's truncation error at
+                         the price of a shallower operand ring (4 instead of 8 dwell groups of T_hi stay in TMEM);
+                         0: one main accumulator.  Not yet validated on hardware.        default 0        */
+  int32_t reserved[1];/* must be 0                                                                */
 } gmco_options;
 
 /* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */
@@ -133,6 +138,7 @@ typedef struct gmco_tc_info {
   int32_t dose_kernel;      /* 0 k_dose_tc<resident T_lo>, 1 k_dose_tc<streamed T_lo>, 2 k_dose_tc_pair<static schedule>,
                                3 k_dose_tc_pair<run-time ring>                                                    */
   int32_t dose_threads, dose_stages, dose_stage_bytes, dose_smem_bytes, dose_smem_end, dose_scr_slot, dose_tmem_cols;
+  int32_t dose_tmem_groups, dose_n_main; /* dwell groups of T_hi kept in TMEM; main accumulators (2 with wide_accum) */
   int32_t grad_threads, grad_ps, grad_stages, grad_stage_bytes, grad_smem_bytes, grad_smem_end, grad_staging_bytes,
       grad_tmem_cols;
   int32_t smem_limit, tmem_limit;        /* 232448 B opt-in dynamic shared memory per CTA, 512 TMEM columns       */
@@ -252,10 +258,11 @@ GMCO_API int gmco_get_stats(const gmco_handle* h, gmco_stats* out);
 
 /* Schedule of the tensor route for a case of n_dwell dwell positions, structures of
  * struct_points[0..n_structs) points (HOST array) and K plans on a device with num_sms multiprocessors (148 on
- * B200); dose_kernel as in gmco_options.  Pure host arithmetic: needs no GPU and no handle.  GMCO_E_INVALID for
- * NULL / non-positive arguments; out->ok = 0 (and GMCO_OK) when the shape is outside the tensor route. */
+ * B200); dose_kernel and wide_accum as in gmco_options.  Pure host arithmetic: needs no GPU and no handle.
+ * GMCO_E_INVALID for NULL / non-positive arguments; out->ok = 0 (and GMCO_OK) when the shape is outside the tensor
+ * route. */
 GMCO_API int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_structs, int32_t K,
-                     int32_t num_sms, int32_t dose_kernel, gmco_tc_info* out);
+                     int32_t num_sms, int32_t dose_kernel, int32_t wide_accum, gmco_tc_info* out);
 
 /* Measurement aid (bench.py's roofline leg).  With enable != 0 every kernel of a round of the
  * following gmco_optimize / gmco_result (the dose kernel: D t, penalty, objective; the gradient

@@ -26,7 +26,7 @@ class _Structure(C.Structure):
 class Options(C.Structure):
     _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
                 ("precision", C.c_int32), ("eps_f", C.c_float), ("compaction", C.c_int32), ("dose_kernel", C.c_int32),
-                ("reserved", C.c_int32 * 2)]
+                ("wide_accum", C.c_int32), ("reserved", C.c_int32 * 1)]
 
 
 class Criterion(C.Structure):
@@ -45,6 +45,7 @@ class TcInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "ok", "a_pad", "n_pad", "n_alloc", "k_pad", "n_tiles", "segs", "n_chunks", "n_slabs", "compact_cap", "dose_kernel",
         "dose_threads", "dose_stages", "dose_stage_bytes", "dose_smem_bytes", "dose_smem_end", "dose_scr_slot", "dose_tmem_cols",
+        "dose_tmem_groups", "dose_n_main",
         "grad_threads", "grad_ps", "grad_stages", "grad_stage_bytes", "grad_smem_bytes", "grad_smem_end", "grad_staging_bytes",
         "grad_tmem_cols", "smem_limit", "tmem_limit")]
 
@@ -84,7 +85,7 @@ def lib():
         L.gmco_select_plan.argtypes = [vp, fp, i32, C.POINTER(Criterion), i32, vp, vp, vp, vp]
         L.gmco_pareto_front.argtypes = [vp, fp, i32, i32, vp, vp, vp]
         L.gmco_get_stats.argtypes = [vp, C.POINTER(Stats)]
-        L.gmco_tc_schedule.argtypes = [i64, C.POINTER(i32), i32, i32, i32, i32, C.POINTER(TcInfo)]
+        L.gmco_tc_schedule.argtypes = [i64, C.POINTER(i32), i32, i32, i32, i32, i32, C.POINTER(TcInfo)]
         L.gmco_set_profiling.argtypes = [vp, i32]
         L.gmco_destroy.argtypes = [vp]
         L.gmco_destroy.restype = None
@@ -139,7 +140,7 @@ def _stream(stream):
 
 
 def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None, compaction=None,
-                 dose_kernel=None) -> Options:
+                 dose_kernel=None, wide_accum=None) -> Options:
     o = Options()
     lib().gmco_default_options(C.byref(o))
     o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
@@ -149,6 +150,8 @@ def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32
         o.compaction = int(compaction)
     if dose_kernel is not None:
         o.dose_kernel = int(dose_kernel)
+    if wide_accum is not None:
+        o.wide_accum = int(wide_accum)
     return o
 
 
@@ -290,11 +293,12 @@ def gmco_get_stats(h: Handle) -> dict:
     return {k: getattr(s, k) for k, _ in Stats._fields_ if k != "reserved"}
 
 
-def gmco_tc_schedule(n_dwell: int, struct_points, K: int, num_sms: int = 148, dose_kernel: int = 0) -> dict:
+def gmco_tc_schedule(n_dwell: int, struct_points, K: int, num_sms: int = 148, dose_kernel: int = 0, wide_accum: int = 0) -> dict:
     """Launch schedule and on-chip layout of the tensor route for a shape (host arithmetic; needs no GPU)."""
     pts = (C.c_int32 * len(struct_points))(*[int(v) for v in struct_points])
     info = TcInfo()
-    _check(lib().gmco_tc_schedule(int(n_dwell), pts, len(struct_points), int(K), int(num_sms), int(dose_kernel), C.byref(info)))
+    _check(lib().gmco_tc_schedule(int(n_dwell), pts, len(struct_points), int(K), int(num_sms), int(dose_kernel), int(wide_accum),
+                                  C.byref(info)))
     return {k: getattr(info, k) for k, _ in TcInfo._fields_}
 
 

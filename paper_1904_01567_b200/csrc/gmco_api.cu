@@ -212,7 +212,8 @@ int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   carve_plans(h, K, 0);
   h->plan_capacity_K = K;
   if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
-    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->opt.dose_kernel == 1, st, h->err, sizeof(h->err));
+    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->opt.dose_kernel == 1, h->opt.wide_accum == 1, st, h->err,
+                           sizeof(h->err));
     if (!h->tc) return GMCO_E_UNSUPPORTED;
   }
   return GMCO_OK;
@@ -378,7 +379,7 @@ void gmco_default_options(gmco_options* o) {
   if (!o) return;
   memset(o, 0, sizeof(*o));
   o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f; o->compaction = 1;
-  o->dose_kernel = 0;
+  o->dose_kernel = 0; o->wide_accum = 0;
 }
 
 const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
@@ -400,7 +401,7 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
       (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || (o.compaction != 0 && o.compaction != 1) ||
-      (o.dose_kernel != 0 && o.dose_kernel != 1) || o.reserved[0] || o.reserved[1])
+      (o.dose_kernel != 0 && o.dose_kernel != 1) || (o.wide_accum != 0 && o.wide_accum != 1) || o.reserved[0])
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
   // the plain-fp32 kernels (the paper's largest N_act is 385)
@@ -884,9 +885,9 @@ int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t K, int32_
 }
 
 int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_structs, int32_t K, int32_t num_sms,
-                     int32_t dose_kernel, gmco_tc_info* out) {
+                     int32_t dose_kernel, int32_t wide_accum, gmco_tc_info* out) {
   if (!out || !struct_points || n_dwell < 1 || n_structs < 1 || n_structs > GMCO_MAX_STRUCTS || K < 1 || num_sms < 1 ||
-      (dose_kernel != 0 && dose_kernel != 1))
+      (dose_kernel != 0 && dose_kernel != 1) || (wide_accum != 0 && wide_accum != 1))
     return fail(nullptr, GMCO_E_INVALID, "gmco_tc_schedule: NULL or non-positive argument%s");
   memset(out, 0, sizeof(*out));
   long long n_pad = 0;
@@ -899,7 +900,7 @@ int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_st
   out->a_pad = round_up(n_dwell, 32); out->n_pad = (int)n_pad; out->n_alloc = round_up(n_pad, kRowAlloc);
   out->k_pad = round_up(K, kPlanTile);
   if (out->a_pad > kMaxApadTensor) return GMCO_OK;   // ok = 0: the SIMT route takes the case
-  const tcl::Schedule q = tcl::choose_schedule(out->a_pad, out->n_pad, out->k_pad, num_sms, dose_kernel == 1);
+  const tcl::Schedule q = tcl::choose_schedule(out->a_pad, out->n_pad, out->k_pad, num_sms, dose_kernel == 1, wide_accum == 1);
   if (!q.ok) return GMCO_OK;
   out->ok = 1;
   out->n_tiles = q.n_tiles; out->segs = q.segs; out->n_chunks = q.n_chunks; out->n_slabs = q.n_slabs;
@@ -910,10 +911,12 @@ int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_st
     out->dose_stages = q.pair_stages; out->dose_stage_bytes = tcl::kPairEntry; out->dose_smem_bytes = q.pair_smem;
     out->dose_smem_end = l.end; out->dose_scr_slot = -1; out->dose_tmem_cols = tcl::pair_tmem_cols(q.G);
   } else {
-    const tcl::DoseSmem l = tcl::dose_smem(q.tlo_resident != 0, q.G, q.dose_stages);
+    const tcl::DoseSmem l = tcl::dose_smem(q.tlo_resident != 0, q.G, q.dose_stages, q.dose_tmem_groups);
     out->dose_stages = q.dose_stages; out->dose_stage_bytes = l.stage_bytes; out->dose_smem_bytes = q.dose_smem;
-    out->dose_smem_end = l.end; out->dose_scr_slot = q.tlo_resident ? -1 : l.scr_slot; out->dose_tmem_cols = tcl::dose_tmem_cols(q.G);
+    out->dose_smem_end = l.end; out->dose_scr_slot = q.tlo_resident ? -1 : l.scr_slot;
+    out->dose_tmem_cols = tcl::dose_tmem_cols(q.G, q.dose_tmem_groups, q.dose_n_main);
   }
+  out->dose_tmem_groups = q.dose_pair ? tcl::kTmemGroups : q.dose_tmem_groups; out->dose_n_main = q.dose_pair ? 1 : q.dose_n_main;
   const tcl::GradSmem gl = tcl::grad_smem(q.grad_ps, q.G, q.grad_stages);
   out->grad_ps = q.grad_ps; out->grad_stages = q.grad_stages; out->grad_stage_bytes = gl.stage_bytes;
   out->grad_smem_bytes = q.grad_smem; out->grad_smem_end = gl.end; out->grad_staging_bytes = gl.staging_bytes;

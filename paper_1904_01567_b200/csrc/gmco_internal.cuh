@@ -155,7 +155,7 @@ int launch_select(const float* dvh, int K, int S, const SelectArgs& c, int* plan
 // tensor path (kernels_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
-                       cudaStream_t st, char* err, int errlen);
+                       int wide_accum, cudaStream_t st, char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 int tc_dose_pair(const TcPlan*);           // 1: the dose kernel runs as CTA pairs (its compaction split is per tile PAIR)

@@ -301,6 +301,7 @@ struct DoseArgs {
   int* log_slot;
   int* round_ctr;             // counts the rounds that had a running plan (gmco_stats.rounds)
   int A_pad, K_pad, K, S, n_chunks, segs, n_stage, n_acc, sep_corr, tlo_resident;
+  int tmem_groups, n_main;    // streamed layout: dwell groups of T_hi in TMEM (8, or 4 with n_main = 2 main accumulators)
   int compact_cap;            // > 0: plans are packed by slot; the CTAs re-split over the tiles that hold running plans
   int* err;                   // device error word [4] (gmco_internal.cuh DevErr); never null
   Thresholds thr;
@@ -341,7 +342,8 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // the D_hi slab and the D_lo slab of one (chunk, 32-dwell group): 16 KB each, so the ring is deep in entries although
 // a chunk is 128 points wide; when T_lo is streamed, its 16 KB slab rides behind the D_hi slab of its group.
 // The last kScratchBytes of the ring double as the T_hi transposition scratch of the prologue.
-template <bool kResident>   // T_lo resident in shared memory (at most 256 dwell positions) or streamed with D_hi
+// kSplit (streamed layout only, gmco_options.wide_accum): two main accumulators and 4 instead of 8 dwell groups of T_hi in TMEM
+template <bool kResident, bool kSplit = false>   // T_lo resident in shared memory (at most 256 dwell positions) or streamed with D_hi
 __global__ void __launch_bounds__(kDoseThreads, 1)
 k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CUtensorMap tmD_lo,
           const __grid_constant__ CUtensorMap tmT_lo, const __grid_constant__ CUtensorMap tmT, const DoseArgs a) {
@@ -356,9 +358,12 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int G = a.A_pad >> 5;                       // 32-dwell slabs
-  const tcl::DoseSmem lay = tcl::dose_smem(kResident, G, a.n_stage);
+  // T_hi groups kept in TMEM and main accumulators: 8 / 1, or (streamed layout with gmco_options.wide_accum) 4 / 2
+  static_assert(!(kResident && kSplit), "the split main accumulator belongs to the streamed layout");
+  constexpr int kTg = kSplit ? tcl::kTmemGroupsSplit : kTmemGroups, n_main = kSplit ? 2 : 1;
+  const tcl::DoseSmem lay = tcl::dose_smem(kResident, G, a.n_stage, kTg);
   if (!layout_fits(a.err, kResident ? DEVERR_K_DOSE_RESIDENT : DEVERR_K_DOSE_STREAMED, (uint32_t)(smem - smem_raw), lay.end,
-                   tcl::dose_tmem_cols(G)))
+                   tcl::dose_tmem_cols(G, kTg, n_main)))
     return;                                         // uniform over the CTA: nothing has been set up yet
   const int stageBytes = lay.stage_bytes;
   // TMEM holds T_hi of the first kTmemGroups dwell groups (256 columns); with more groups the rest of T_hi lives in
@@ -400,7 +405,12 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   // from ~1e-5 to ~2e-6 of the dose, and the dose error is what the gradient feels near a threshold (r = d - D_lim
   // cancels).  With both accumulators there is room for one buffer only: the epilogue frees it as soon as the values
   // are in registers, the penalty arithmetic and the R stores still overlap the next chunk's MMAs.
-  const uint32_t t_acc = tmem + tcl::dose_tmem_acc_col(G);
+  // Split main (n_main = 2): the adds of T_hi D_hi go to accumulator A for the dwell groups below
+  // g_half and to accumulator B from g_half on, so that each takes half as many truncating adds at half the
+  // magnitude; the epilogue sums A + B + corrections in fp32 registers.  Columns: [main A | main B | corrections].
+  const uint32_t t_acc = tmem + tcl::dose_tmem_acc_col(G, kTg);
+  const int g_half = kSplit ? (G + 1) >> 1 : G;               // first dwell group of main accumulator B (none when G)
+  constexpr uint32_t corr_off = (uint32_t)n_main * kPC;        // column offset of the correction accumulator
 
   if (warp == 0) {
     // whole warp walks the ring (uniform control flow); one elected lane issues
@@ -455,17 +465,19 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
         GMCO_WAIT(mbar_wait(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
         tc_fence_after();
-        const uint32_t acc = t_acc + b * (a.sep_corr ? 2 * kPC : kPC), acc_c = a.sep_corr ? acc + kPC : acc;
-        uint32_t thi = t_thi, alo = tlo_lo0;   // alo: resident T_lo slab g, or (streamed) T_hi tail slab g - kTmemGroups
-        for (int g = 0; g < G; thi += 32, alo += (kResident || g >= kTmemGroups) ? kTloBox >> 4 : 0, ++g) {
+        const uint32_t acc0 = t_acc + b * (a.sep_corr ? (uint32_t)(n_main + 1) * kPC : kPC), acc_c = a.sep_corr ? acc0 + corr_off : acc0;
+        uint32_t thi = t_thi, alo = tlo_lo0;   // alo: resident T_lo slab g, or (streamed) T_hi tail slab g - kTg
+        for (int g = 0; g < G; thi += 32, alo += (kResident || g >= kTg) ? kTloBox >> 4 : 0, ++g) {
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
           if (c == c0) { GMCO_WAIT(mbar_wait(w, tg_ready + g, 0, DEVERR_W_TG_READY)); tc_fence_after(); }   // first chunk overlaps the prologue
           GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             const uint32_t ad = kResident ? alo : bd + (kSlabBytes >> 4);
-            if (kResident || g < kTmemGroups) {
-              mma_ts2(acc, thi, bd, dhi, idesc, g != 0);
+            const uint32_t acc = g < g_half ? acc0 : acc0 + kPC;                 // main accumulator A or B
+            const uint32_t first = (g != 0 && g != g_half) ? 1u : 0u;           // the first add into A / into B overwrites
+            if (kResident || g < kTg) {
+              mma_ts2(acc, thi, bd, dhi, idesc, first);
               mma_ss2(acc_c, ad, dhi, bd, dhi, idesc, (a.sep_corr && g == 0) ? 0u : 1u);
 #pragma unroll
               for (int j = 1; j < 4; ++j) {         // K-steps of 8 dwell positions: +32 B inside the swizzled row
@@ -473,8 +485,10 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
                 mma_ss2(acc_c, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
               }
             } else {                                // T_hi of this group is in the shared-memory tail
+              mma_ss2(acc, alo, dhi, bd, dhi, idesc, first);
+              mma_ss2(acc_c, ad, dhi, bd, dhi, idesc, 1);
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
+              for (int j = 1; j < 4; ++j) {
                 mma_ss2(acc, alo + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
                 mma_ss2(acc_c, ad + 2 * j, dhi, bd + 2 * j, dhi, idesc, 1);
               }
@@ -487,7 +501,7 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
           GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
           if (elect_one()) {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
-            if (kResident || g < kTmemGroups) {
+            if (kResident || g < kTg) {
 #pragma unroll
               for (int j = 0; j < 4; ++j) mma_ts2(acc_c, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);
             } else {
@@ -553,8 +567,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
 #pragma unroll
           for (int i = 0; i < 8; ++i)
             t[i] = *reinterpret_cast<const float4*>(src + (size_t)(i * 4 + r0) * a.A_pad + g * 32 + c4 * 4);
-          if (g >= kTmemGroups) {                    // tail group: hi goes to shared memory in the operand layout
-            uint8_t* dstg = tlo + (size_t)(g - kTmemGroups) * kTloBox + q * 4096;
+          if (g >= kTg) {                            // tail group: hi goes to shared memory in the operand layout
+            uint8_t* dstg = tlo + (size_t)(g - kTg) * kTloBox + q * 4096;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               const int r = i * 4 + r0;
@@ -605,17 +619,20 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         GMCO_WAIT(mbar_wait(w, acc_full + b, use & 1, DEVERR_W_ACC_FULL));
         tc_fence_after();
         uint32_t v[2][32];
-        const uint32_t t_main = t_acc + lane_base + b * (a.sep_corr ? 2 * kPC : kPC) + h * 64;
+        const uint32_t t_main = t_acc + lane_base + b * (a.sep_corr ? (uint32_t)(n_main + 1) * kPC : kPC) + h * 64;
         tmem_ld32(t_main, v[0]);
         tmem_ld32(t_main + 32, v[1]);
         if (a.sep_corr) {
 #pragma unroll
-          for (int sub = 0; sub < 2; ++sub) {
-            uint32_t vc[32];
-            tmem_ld32(t_main + kPC + sub * 32, vc);
-            tmem_ld_wait();
+          for (int part = 1; part <= n_main; ++part) {       // main accumulator B (split main), then the corrections
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[sub][j] = __float_as_uint(__uint_as_float(v[sub][j]) + __uint_as_float(vc[j]));
+            for (int sub = 0; sub < 2; ++sub) {
+              uint32_t vc[32];
+              tmem_ld32(t_main + (uint32_t)part * kPC + sub * 32, vc);
+              tmem_ld_wait();
+#pragma unroll
+              for (int j = 0; j < 32; ++j) v[sub][j] = __float_as_uint(__uint_as_float(v[sub][j]) + __uint_as_float(vc[j]));
+            }
           }
         } else {
           tmem_ld_wait();
@@ -1237,6 +1254,7 @@ static cudaError_t tc_set_smem_caps() {
   if (done == cudaSuccess) return done;
   cudaError_t e = cudaFuncSetAttribute(k_dose_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
@@ -1245,10 +1263,10 @@ static cudaError_t tc_set_smem_caps() {
 }
 
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
-                       cudaStream_t st, char* err, int errlen) {
+                       int wide_accum, cudaStream_t st, char* err, int errlen) {
   if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
-  t->sch = tcl::choose_schedule(c.A_pad, c.N_pad, p.K_pad, num_sms, force_single);
+  t->sch = tcl::choose_schedule(c.A_pad, c.N_pad, p.K_pad, num_sms, force_single, wide_accum);
   const tcl::Schedule& q = t->sch;
   if (!q.ok) { snprintf(err, errlen, "shared memory too small for the tensor kernels' rings at this shape"); delete t; return nullptr; }
   for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
@@ -1305,12 +1323,13 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
     da.n_chunks = q.n_chunks;
     da.segs = q.segs; da.n_stage = q.dose_stages; da.sep_corr = 1;   // T_hi takes at most 256 TMEM columns: both accumulators always fit
     da.n_acc = 1;
-    da.tlo_resident = q.tlo_resident; da.thr = t->thr;
+    da.tlo_resident = q.tlo_resident; da.thr = t->thr; da.tmem_groups = q.dose_tmem_groups; da.n_main = q.dose_n_main;
     if (q.dose_pair) {
       da.n_stage = q.pair_stages;
       if (q.pair_static) k_dose_tc_pair<4, 6><<<dim3(q.n_tiles, q.segs), kDoseThreads, q.pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
       else k_dose_tc_pair<0, 0><<<dim3(q.n_tiles, q.segs), kDoseThreads, q.pair_smem, st>>>(t->pair_D_hi, t->pair_D_lo, t->dose_T, da);
     } else if (q.tlo_resident) k_dose_tc<true><<<grid, kDoseThreads, q.dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
+    else if (q.dose_n_main == 2) k_dose_tc<false, true><<<grid, kDoseThreads, q.dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
     else k_dose_tc<false><<<grid, kDoseThreads, q.dose_smem, st>>>(t->dose_D_hi, t->dose_D_lo, t->dose_T_lo, t->dose_T, da);
     if (cudaPeekAtLastError() != cudaSuccess) return -1;   // left for the caller's message
     ++n;

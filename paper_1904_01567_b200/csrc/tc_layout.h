@@ -22,6 +22,7 @@ constexpr int kPC = 128;                   // points per dose chunk = MMA N of t
 constexpr int kSlabBytes = kPC * 128;      // one 32-dwell slab of a dose chunk, one part (hi or lo): 16 KB
 constexpr int kTloBox = 128 * 128;         // T_lo: 128 plans x 32 dwell: 16 KB
 constexpr int kTmemGroups = 8;             // dwell groups of T_hi kept in TMEM (256 columns)
+constexpr int kTmemGroupsSplit = 4;        // the same with the split main accumulator of the streamed layout (128 columns)
 constexpr int kTmemCols = 512;             // TMEM columns of one SM
 constexpr int kScratchBytes = 8 * 4096;    // T_hi transposition scratch (streamed layout), one 4 KB slab per epilogue warp
 constexpr int kHalfPC = kPC / 2;
@@ -46,9 +47,10 @@ struct DoseSmem {
   int slot_off;       // uint32 TMEM base address, uint32 abort flag
   int end;            // bytes used from the aligned base
 };
-GMCO_HD DoseSmem dose_smem(bool resident, int G, int n_stage) {
+// tmem_groups: dwell groups of T_hi that live in TMEM (kTmemGroups, or kTmemGroupsSplit for the split-main layout)
+GMCO_HD DoseSmem dose_smem(bool resident, int G, int n_stage, int tmem_groups = kTmemGroups) {
   DoseSmem s;
-  const int Gs = resident ? 0 : (G > kTmemGroups ? G - kTmemGroups : 0);
+  const int Gs = resident ? 0 : (G > tmem_groups ? G - tmem_groups : 0);
   s.tlo_bytes = (resident ? G : Gs) * kTloBox;
   s.stage_bytes = resident ? kSlabBytes : kSlabBytes + kTloBox;
   s.ring_off = s.tlo_bytes;
@@ -61,9 +63,12 @@ GMCO_HD DoseSmem dose_smem(bool resident, int G, int n_stage) {
   s.end = s.slot_off + 8;
   return s;
 }
-// TMEM columns: T_hi of min(G, kTmemGroups) groups, then one accumulator buffer (main + separate correction)
-GMCO_HD int dose_tmem_acc_col(int G) { return (G < kTmemGroups ? G : kTmemGroups) * 32; }
-GMCO_HD int dose_tmem_cols(int G) { return dose_tmem_acc_col(G) + 2 * kPC; }
+// TMEM columns: T_hi of min(G, tmem_groups) groups, then one accumulator buffer: n_main main accumulators (the main
+// product's adds split by dwell-group block) + the separate correction accumulator, 128 points each
+GMCO_HD int dose_tmem_acc_col(int G, int tmem_groups = kTmemGroups) { return (G < tmem_groups ? G : tmem_groups) * 32; }
+GMCO_HD int dose_tmem_cols(int G, int tmem_groups = kTmemGroups, int n_main = 1) {
+  return dose_tmem_acc_col(G, tmem_groups) + (n_main + 1) * kPC;
+}
 
 // ---- k_dose_tc_pair ---------------------------------------------------------------------------------------------------
 struct PairSmem {
@@ -128,14 +133,16 @@ struct Schedule {
   int ok;                  // 0: the shape does not fit the tensor route
   int G, n_tiles, segs, n_chunks;
   int tlo_resident, dose_stages, dose_smem;
+  int dose_tmem_groups, dose_n_main;   // streamed layout only: 4 groups of T_hi in TMEM and two main accumulators when wide_accum is on
   int dose_pair, pair_static, pair_stages, pair_smem;
   int grad_ps, grad_stages, grad_smem, n_slabs;
   int dose_kernel;         // DoseKernelId of the kernel that launch_tc_eval dispatches
 };
 
 // Every size the host chooses for a case of A_pad dwell columns, N_pad padded points and K_pad padded plans.
-// force_single != 0 keeps the single-CTA dose kernel where the CTA-pair kernel would be eligible.
-inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, int force_single) {
+// force_single != 0 keeps the single-CTA dose kernel where the CTA-pair kernel would be eligible.  wide_accum != 0
+// selects the split-main layout for the streamed dose kernel (more than 256 dwell positions).
+inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, int force_single, int wide_accum = 0) {
   Schedule t{};
   t.G = A_pad / 32;
   t.n_tiles = K_pad / 128;
@@ -146,8 +153,10 @@ inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, in
   const int slack = kAlign + kBarBytes;
   // dose kernel: T_lo resident when it leaves room for >= 4 ring stages, else streamed with every D_hi slab
   t.tlo_resident = (G <= kTmemGroups && G * kTloBox + 4 * kSlabBytes + slack <= kSmemMax) ? 1 : 0;
+  t.dose_tmem_groups = (!t.tlo_resident && wide_accum) ? kTmemGroupsSplit : kTmemGroups;
+  t.dose_n_main = (!t.tlo_resident && wide_accum) ? 2 : 1;
   {
-    const DoseSmem probe = dose_smem(t.tlo_resident != 0, G, 0);
+    const DoseSmem probe = dose_smem(t.tlo_resident != 0, G, 0, t.dose_tmem_groups);
     const int fixed = probe.tlo_bytes + slack;
     t.dose_stages = (kSmemMax - fixed) / probe.stage_bytes;
     if (t.dose_stages > kDoseMaxStages) t.dose_stages = kDoseMaxStages;

@@ -40,13 +40,13 @@ def test_version_and_default_options(built_lib):
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
-    assert o.compaction == 1 and o.dose_kernel == 0 and list(o.reserved) == [0, 0]
+    assert o.compaction == 1 and o.dose_kernel == 0 and o.wide_accum == 0 and list(o.reserved) == [0]
 
 
 def test_struct_layouts_match_the_header(built_lib):
     import paper_1904_01567_b200.binding as b
     assert ctypes.sizeof(b._Structure) == 28 and ctypes.sizeof(b.Options) == 40 and ctypes.sizeof(b.Stats) == 56
-    assert ctypes.sizeof(b.TcInfo) == 28 * 4
+    assert ctypes.sizeof(b.TcInfo) == 30 * 4
     assert ctypes.sizeof(b.Criterion) == 20
 
 

@@ -97,6 +97,7 @@ scenario("pair_ring", pair, b.make_options(m=pair.m))
 scenario("pair_forced_single", pair, b.make_options(m=pair.m, dose_kernel=1))
 wide = gc.make_case("C1", n_cath=24, n_pos=16, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
 scenario("wide_streamed", wide, b.make_options(m=wide.m, eps=1e-3, compaction=0))
+scenario("wide_split_main", wide, b.make_options(m=wide.m, wide_accum=1))
 c3 = gc.make_case("C3")
 scenario("c3_pair_static", c3, b.make_options(m=c3.m), iters=200)
 widest = gc.make_case("C1", n_cath=35, n_pos=11, counts=(300, 64, 100, 100), n_plans=5, seed_points=5)   # 385 dwell positions: SIMT route
@@ -184,14 +185,16 @@ def test_shapes_and_statistics_of_every_route(report):
 def test_every_launch_is_the_one_the_schedule_announces(report):
     import gmco_cases as gc
     import paper_1904_01567_b200 as g
-    cases = {"c1_tf32": (gc.make_case("C1"), 0), "pair_ring": (gc.make_case("C1", n_plans=256), 0),
-             "pair_forced_single": (gc.make_case("C1", n_plans=256), 1),
-             "wide_streamed": (gc.make_case("C1", n_cath=24, n_pos=16, counts=(700, 130, 250, 190), n_plans=130, seed_points=9), 0),
-             "c3_pair_static": (gc.make_case("C3"), 0)}
-    names = {0: "k_dose_tcILb1", 1: "k_dose_tcILb0", 2: "k_dose_tc_pairILi4ELi6", 3: "k_dose_tc_pairILi0ELi0"}
-    for tag, (c, dk) in cases.items():
-        q = g.gmco_tc_schedule(c.n_dwell, [s.n_points for s in c.structures], c.n_plans, 148, dk)
+    wide = gc.make_case("C1", n_cath=24, n_pos=16, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
+    cases = {"c1_tf32": (gc.make_case("C1"), 0, 0), "pair_ring": (gc.make_case("C1", n_plans=256), 0, 0),
+             "pair_forced_single": (gc.make_case("C1", n_plans=256), 1, 0),
+             "wide_streamed": (wide, 0, 0), "wide_split_main": (wide, 0, 1),
+             "c3_pair_static": (gc.make_case("C3"), 0, 0)}
+    names = {0: "k_dose_tcILb1ELb0", 1: "k_dose_tcILb0ELb0", 2: "k_dose_tc_pairILi4ELi6", 3: "k_dose_tc_pairILi0ELi0"}
+    for tag, (c, dk, wa) in cases.items():
+        q = g.gmco_tc_schedule(c.n_dwell, [s.n_points for s in c.structures], c.n_plans, 148, dk, wa)
         rep = report[tag]
+        names[1] = "k_dose_tcILb0ELb1" if wa else "k_dose_tcILb0ELb0"
         dose = _one(rep, names[q["dose_kernel"]])
         grid = [q["n_tiles"], q["segs"], 1] if q["dose_kernel"] >= 2 else [q["segs"], q["n_tiles"], 1]
         assert dose["grid"] == grid and dose["block"] == [320, 1, 1] and dose["smem"] == q["dose_smem_bytes"], tag

@@ -28,12 +28,12 @@ def _shapes():
             yield a, tiles
 
 
-@pytest.mark.parametrize("dose_kernel", [0, 1])
-def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel):
+@pytest.mark.parametrize("dose_kernel,wide_accum", [(0, 0), (1, 0), (0, 1)])
+def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel, wide_accum):
     n = 0
     for a, tiles in _shapes():
         for pts in ((64,), (100, 30), STRUCTS, (24000, 4000, 6000, 6000), (40000,)):
-            q = g.gmco_tc_schedule(a, pts, 128 * tiles, 148, dose_kernel)
+            q = g.gmco_tc_schedule(a, pts, 128 * tiles, 148, dose_kernel, wide_accum)
             assert q["ok"] == 1, (a, tiles, pts)
             G = q["a_pad"] // 32
             assert q["a_pad"] == 32 * ((a + 31) // 32) and q["k_pad"] == 128 * tiles and q["n_tiles"] == tiles
@@ -58,6 +58,11 @@ def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel):
             else:
                 assert G > 8 and q["dose_stage_bytes"] == K_SLAB + K_TLO
                 assert q["dose_scr_slot"] == q["dose_stages"] - 1                     # the scratch is exactly the last entry
+                # T_hi: 8 dwell groups in TMEM + main + corrections, or (wide_accum) 4 groups + two mains + corrections
+                assert (q["dose_tmem_groups"], q["dose_n_main"]) == ((4, 2) if wide_accum else (8, 1))
+                assert q["dose_tmem_cols"] == 32 * q["dose_tmem_groups"] + 128 * (q["dose_n_main"] + 1) == 512
+            if q["dose_kernel"] != 1:
+                assert (q["dose_tmem_groups"], q["dose_n_main"]) == (8, 1)            # wide_accum touches the streamed layout only
             assert q["dose_stage_bytes"] % 1024 == 0 and q["grad_stage_bytes"] % 1024 == 0
             assert q["grad_stage_bytes"] == 2 * 4 * q["grad_ps"] * 128 + 2 * G * q["grad_ps"] * 128
             # TMA boxes stay inside the global allocations (rows of D / R: n_alloc; rows of T: k_pad)
@@ -75,6 +80,29 @@ def test_shapes_outside_the_tensor_route_are_flagged_not_scheduled():
         g.gmco_tc_schedule(0, STRUCTS, 1000)
     with pytest.raises(g.GmcoError):
         g.gmco_tc_schedule(100, STRUCTS, 0)
+
+
+def test_split_main_accumulator_flags():
+    """gmco_options.wide_accum (k_dose_tc<streamed, split>): a restatement of the issuer's accumulator choice and
+    overwrite flags -- per chunk every accumulator is overwritten exactly once, by the first MMA that targets it, the
+    overwriting MMA of main accumulator B sits in the shared-memory-tail branch, and the adds split evenly."""
+    for G in (9, 10, 11, 12):
+        k_tg, g_half = 4, (G + 1) // 2
+        log = []                                     # (accumulator, overwrite?, branch) in issue order
+        for gq in range(G):
+            acc = "A" if gq < g_half else "B"
+            first = 0 if gq in (0, g_half) else 1
+            branch = "tmem" if gq < k_tg else "tail"
+            for j in range(4):
+                log.append((acc, (first if j == 0 else 1) == 0, branch))
+                log.append(("C", gq == 0 and j == 0, branch))                 # T_lo D_hi
+            log += [("C", False, branch)] * 4                                  # T_hi D_lo
+        for name in "ABC":
+            mine = [x for x in log if x[0] == name]
+            assert mine[0][1] and not any(x[1] for x in mine[1:])
+        assert [x for x in log if x[0] == "B"][0][2] == "tail"
+        nA, nB = sum(x[0] == "A" for x in log), sum(x[0] == "B" for x in log)
+        assert nA + nB == 4 * G and abs(nA - nB) <= 4
 
 
 def test_bench_shapes_take_the_documented_kernels():
@@ -377,13 +405,16 @@ def model_grad(sim, n_stage, n_slabs):
 
 
 def test_protocol_model_dose_single_cta_terminates_for_every_host_choice():
-    for a_pad in range(32, 385, 32):
-        q = g.gmco_tc_schedule(a_pad, STRUCTS, 128, 148, 1)
-        assert q["dose_kernel"] in (0, 1)
-        G, resident = a_pad // 32, q["dose_kernel"] == 0
-        for n_chunks in (1, 2, 3, 5, 6, 7):
-            for seed in range(3):
-                model_dose_single(Sim(seed), G, q["dose_stages"], n_chunks, resident, q["dose_scr_slot"])
+    for wide_accum in (0, 1):
+        for a_pad in range(32, 385, 32):
+            q = g.gmco_tc_schedule(a_pad, STRUCTS, 128, 148, 1, wide_accum)
+            assert q["dose_kernel"] in (0, 1)
+            G, resident = a_pad // 32, q["dose_kernel"] == 0
+            if wide_accum and resident:
+                continue
+            for n_chunks in (1, 2, 3, 5, 6, 7):
+                for seed in range(3):
+                    model_dose_single(Sim(seed), G, q["dose_stages"], n_chunks, resident, q["dose_scr_slot"])
     # smaller rings than the host would choose must still be sound (the arithmetic does not depend on a lucky size)
     for G, n_stage in ((8, 2), (8, 3), (5, 4), (1, 2), (3, 7)):
         model_dose_single(Sim(7), G, n_stage, 4, True, -1)
