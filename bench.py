@@ -235,6 +235,7 @@ def main():
     ap.add_argument("--no-peak", action="store_true", help="skip the live tf32 matmul peak measurement (roofline falls back to the nominal ratio)")
     ap.add_argument("--dose-kernel", type=int, default=0, choices=[0, 1], help="gmco_options.dose_kernel (1 = keep the single-CTA dose kernel)")
     ap.add_argument("--no-gsa", action="store_true", help="skip the gSA-vs-gL-BFGS comparison leg (C5)")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the C1 / C2 / C4 legs (SURVEY 8(d): 'plus the same for C1, C2, C4')")
     ap.add_argument("--clock-period", type=float, default=0.02, help="seconds between NVML clock samples (0 = off)")
     ap.add_argument("--eps", type=float, default=0.0, help="per-plan stopping rule (PAPER.md:119); 0 = exactly `iters` iterations")
     ap.add_argument("--compaction", type=int, default=1, choices=[0, 1], help="gmco_options.compaction")
@@ -348,19 +349,35 @@ def main():
             "clocks": clk.summary(),
             "paper_context": "gL-BFGS 0.9 ms/plan = ~1111 plans/s on a Titan X (Pascal), real cases, eps=1e-3 (PAPER.md:180)",
         }
-        tf32 = None if (args.no_peak or prec != g.GMCO_PREC_TF32X3) else measure_tf32_peak(torch)
-        line["roofline"] = roofline(case, prec, g, prof, peaks, tf32, clk.summary())
+        # Every leg below is auxiliary to the headline numbers above: a failure in one of them is recorded in the line
+        # instead of costing the run its record.
+        def leg(name, fn):
+            try:
+                return fn()
+            except Exception as e:                              # noqa: BLE001 -- reported, not swallowed
+                return {"error": f"{name}: {type(e).__name__}: {e}"}
+
+        tf32 = None
+        if not (args.no_peak or prec != g.GMCO_PREC_TF32X3):
+            tf32 = leg("tf32 peak", lambda: measure_tf32_peak(torch))
+            if "error" in tf32:
+                line["tf32_peak_error"], tf32 = tf32["error"], None
+        line["roofline"] = leg("roofline", lambda: roofline(case, prec, g, prof, peaks, tf32, clk.summary()))
         if not args.no_gsa:
-            line["gsa_vs_glbfgs"] = gsa_leg(g, torch, stream)
+            line["gsa_vs_glbfgs"] = leg("gsa", lambda: gsa_leg(g, torch, stream))
+        if not args.no_other_configs:
+            line["other_configs"] = leg("other configs", lambda: other_configs_leg(g, torch, stream, prec, case.name, not args.no_cpu_baseline))
         if args.characterise:
-            line["characterisation"] = characterise_leg(g, torch, stream, prec)
+            line["characterisation"] = leg("characterise", lambda: characterise_leg(g, torch, stream, prec))
         if not args.no_cpu_baseline:
-            v, dt, cores = oracle_leg(case, args.ref_sample)
-            v1, dt1 = oracle_leg_one_core(case)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": f"{args.ref_sample} of {K} plans of {case.name}, full {case.iters} "
-                                              f"iterations, {dt:.1f} s, OpenMP over plans",
-                                    "value_1core": v1, "sample_1core": f"4 plans one after the other, {dt1:.1f} s"}
+            def cpu():
+                v, dt, cores = oracle_leg(case, args.ref_sample)
+                v1, dt1 = oracle_leg_one_core(case)
+                return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"{args.ref_sample} of {K} plans of {case.name}, full {case.iters} "
+                                  f"iterations, {dt:.1f} s, OpenMP over plans",
+                        "value_1core": v1, "sample_1core": f"4 plans one after the other, {dt1:.1f} s"}
+            line["cpu_baseline"] = leg("cpu baseline", cpu)
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -418,6 +435,48 @@ def characterise_leg(g, torch, stream, prec):
             "paper_context": "Fig. 4a: 0.9 ms/plan at 1000 plans, 10000 plans within 9 s, 2.6 GB at 10000 plans (PAPER.md:180, :228); "
                              "Fig. 3a: eps 1e-7 -> 1e-2 gives non-dominated 100 % -> 89.3 %, speed-up 1 -> 10, 99.3 % at 1e-3 "
                              "(PAPER.md:170); Titan X (Pascal), clinical cases"}
+
+
+def other_configs_leg(g, torch, stream, prec, headline, with_oracle):
+    """the metric "plus the same for C1, C2, C4".  Outside the timed region of the headline: one pool per
+    configuration, inputs resident in HBM, CUDA events around create + optimize + result + destroy, best of 3 after a
+    warm-up (C4: best of 2).  C1 and C2 also time the oracle IN FULL (every plan, every iteration) on the host cores;
+    C4's oracle time is not taken here (hours of CPU work; the parity tests follow sampled plans)."""
+    import oracle
+    out = {}
+    for name in ("C1", "C2", "C4"):
+        if name == headline:
+            continue
+        c = gc.make_case(name)
+        D = torch.from_numpy(c.D).cuda(); T0 = torch.from_numpy(c.T0).cuda(); w = torch.from_numpy(c.weights).cuda()
+        best, stats = None, None
+        for i in range(3 if name == "C4" else 4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            h = g.gmco_create(D, c.structures, c.rx, g.binding.make_options(m=c.m, precision=prec), stream)
+            try:
+                g.gmco_optimize(h, T0, w, c.iters, stream)
+                g.gmco_result(h)
+                stats = g.gmco_get_stats(h)
+            finally:
+                g.gmco_destroy(h)
+            e1.record(stream); e1.synchronize()
+            if i:
+                best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        row = {"n_points": c.n_points, "n_dwell": c.n_dwell, "plans": c.n_plans, "iters": c.iters, "ms_per_pool": best,
+               "plans_per_s": c.n_plans / (best * 1e-3), "plan_iterations_per_s": c.n_plans * c.iters / (best * 1e-3),
+               "rounds": int(stats["rounds"]), "device_bytes": int(stats["device_bytes"]),
+               "dose_kernel": g.DOSE_KERNEL_NAMES.get(stats["dose_kernel"])}
+        if with_oracle and name in ("C1", "C2"):
+            oracle.build()
+            t0 = time.perf_counter()
+            oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=c.iters)
+            dt = time.perf_counter() - t0
+            row["oracle_full_s"] = dt
+            row["oracle_plans_per_s"] = c.n_plans / dt
+            row["oracle_cores"] = oracle.num_threads()
+        out[name] = row
+    return out
 
 
 def gsa_leg(g, torch, stream):
