@@ -69,8 +69,12 @@ int fake_launch(int i, char* name, int cap, unsigned* dims /* [6] */, unsigned l
   *smem = g_launch[i].smem; *captured = g_launch[i].captured;
   return 0;
 }
-/* write into "device" memory from the test (e.g. to plant an error word): range-checked like a copy */
-int fake_poke_int(void* dst, int v) { if (find(dst) < 0) return -1; memcpy(dst, &v, sizeof v); return 0; }
+/* Fault injection: the library clears its 4-int device error word with the only 16-byte memset it issues.  With a
+ * planted word that memset writes {code, site, block, detail} instead of zeros, as if a kernel had reported an error. */
+static int g_plant[4], g_plant_on;
+void fake_plant_error_word(int on, int code, int site, int block, int detail) {
+  g_plant_on = on; g_plant[0] = code; g_plant[1] = site; g_plant[2] = block; g_plant[3] = detail;
+}
 
 /* ---- registration (called from nvcc's static initialisers) ---- */
 void** __cudaRegisterFatBinary(void* bin) { (void)bin; static void* h; return &h; }
@@ -172,6 +176,7 @@ cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t st) {
   if (find(d) < 0) violation("cudaMemset of a pointer that is not device memory", d, n);
   check("cudaMemset", d, n);
   if (find(d) >= 0) memset(d, v, n);
+  if (g_plant_on && n == 16 && find(d) >= 0) memcpy(d, g_plant, 16);
   return cudaSuccess;
 }
 

@@ -133,6 +133,26 @@ try:
 except g.GmcoError as e:
     errs["nan_T0"] = e.code
 g.gmco_destroy(h)
+# a kernel that reported a protocol error through the device error word: GMCO_E_CUDA with kernel and wait site, then a state error
+F.fake_plant_error_word(1, 1, (3 << 8) | 6, 5 | (2 << 16), 77)
+h = g.gmco_create(c1.D, c1.structures, c1.rx)
+g.gmco_optimize(h, c1.T0, c1.weights, 3)
+try:
+    g.gmco_result(h, host=True)
+except g.GmcoError as e:
+    errs["error_word_result"] = [e.code, str(e)]
+try:
+    g.gmco_result(h, host=True)
+except g.GmcoError as e:
+    errs["error_word_result_again"] = e.code
+try:
+    g.gmco_evaluate(h, np.repeat(c1.T0[None], c1.n_plans, 0), c1.weights, host=True)
+except g.GmcoError as e:
+    errs["error_word_evaluate"] = e.code
+F.fake_plant_error_word(0, 0, 0, 0, 0)
+g.gmco_optimize(h, c1.T0, c1.weights, 3)                 # the handle is usable again once the word is clear
+g.gmco_result(h, host=True)
+g.gmco_destroy(h)
 report["errors"] = errs
 report["final_live"] = F.fake_live_allocations()
 report["tensor_maps"] = F.fake_tensor_maps()
@@ -160,7 +180,10 @@ def test_no_copy_leaves_its_allocation_and_nothing_leaks(report):
             assert rep["violations"] == 0, f"{tag}: {rep['message']}"
             assert rep["live"] == 0, f"{tag}: {rep['live']} device allocations alive after gmco_destroy"
     assert report["final_live"] == 0 and report["tensor_maps"] > 0
-    assert report["errors"] == {"result_before_optimize": -5, "nan_T0": -1}
+    errs = dict(report["errors"])
+    code, msg = errs.pop("error_word_result")
+    assert code == -3 and "k_dose_tc_pair" in msg and "accumulator free" in msg and "block (5, 2)" in msg and "detail 77" in msg
+    assert errs == {"result_before_optimize": -5, "nan_T0": -1, "error_word_result_again": -5, "error_word_evaluate": -3}
 
 
 def test_shapes_and_statistics_of_every_route(report):
