@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
     for (uint32_t spins = 1; !ok; ++spins) {
       asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                    : "=r"(ok) : "r"(bar) : "memory");
-      if (!ok && (spins & 63u) == 0u) {
+      if (!ok && (spins & 4095u) == 0u) {        // the clock is read rarely: this wait is on the kernel's critical path
         unsigned long long now;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
         if (t0 == 0) t0 = now;

@@ -92,20 +92,27 @@ __device__ __forceinline__ uint32_t ld_flag(uint32_t addr) {
 __device__ __forceinline__ void st_flag(uint32_t addr, uint32_t v) {
   asm volatile("st.volatile.shared::cta.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
+// The slow path must not slow a healthy wait down: between two polls of the barrier it does nothing; every 64th
+// failed poll it reads the CTA's abort flag (shared memory), and only every 4096th the error word (a global load) and
+// the clock.  A poll takes tens of cycles at least, so the bound is checked every few tens of microseconds at most.
 __device__ __noinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, int cluster_scope, int* err, uint32_t abort_addr,
                                             int site) {
-  const unsigned long long t0 = global_ns();
+  unsigned long long t0 = 0;
   for (uint32_t spins = 1;; ++spins) {
     if (cluster_scope ? mbar_try_wait_cluster_addr(bar, parity) : mbar_try_wait_addr(bar, parity)) return true;
-    if ((spins & 15u) == 0u) {
+    if ((spins & 63u) == 0u) {
       if (ld_flag(abort_addr)) return false;
-      const bool failed_elsewhere = *reinterpret_cast<volatile int*>(err) != 0;
-      if (failed_elsewhere || global_ns() - t0 > kWaitLimitNs) {
-        if (!failed_elsewhere && atomicCAS(err, 0, (int)DEVERR_WAIT_TIMEOUT) == 0) {
-          err[1] = site; err[2] = (int)(blockIdx.x | (blockIdx.y << 16)); err[3] = (int)(threadIdx.x | (parity << 16));
+      if ((spins & 4095u) == 0u) {
+        const bool failed_elsewhere = *reinterpret_cast<volatile int*>(err) != 0;
+        const unsigned long long now = global_ns();
+        if (t0 == 0) t0 = now;
+        if (failed_elsewhere || now - t0 > kWaitLimitNs) {
+          if (!failed_elsewhere && atomicCAS(err, 0, (int)DEVERR_WAIT_TIMEOUT) == 0) {
+            err[1] = site; err[2] = (int)(blockIdx.x | (blockIdx.y << 16)); err[3] = (int)(threadIdx.x | (parity << 16));
+          }
+          st_flag(abort_addr, 1u);
+          return false;
         }
-        st_flag(abort_addr, 1u);
-        return false;
       }
     }
   }
