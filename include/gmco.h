@@ -111,7 +111,17 @@ typedef struct gmco_options {
                          epilogue sums in fp32, which halves the tensor core's truncation error at
                          the price of a shallower operand ring (4 instead of 8 dwell groups of T_hi stay in TMEM);
                          0: one main accumulator.  Not yet validated on hardware.        default 0        */
-  int32_t reserved[1];/* must be 0                                                                */
+  int32_t line_search;/* 0: a rejected trial step is halved and evaluated in the next round's batched contraction
+                         (the plan rides along: one extra column per halving).  1: polynomial line search of
+                         north_star item (4): when the first trial step (alpha = 1) of an iteration is rejected, the
+                         dose columns d = D(x o x), a = D(x o p), b = D(p o p) of that plan are formed once and every
+                         further candidate alpha = 1/2, 1/4, ... is valued from d + 2 alpha a + alpha^2 b without a
+                         contraction; the first candidate that meets the acceptance rule becomes the next trial
+                         point, which is then evaluated afresh (an iteration with h rejected steps costs 2 rounds
+                         instead of 1 + h).  Same algorithm, same iteration counts.  On the stand-in cases no
+                         iteration has more than two rejected steps, so it saves 0.5 % of plan-rounds and costs
+                         two more launches per round: off by default.  Not yet validated on
+                         hardware.                                                default 0        */
 } gmco_options;
 
 /* Counters of the last gmco_optimize + gmco_result pair (host side, filled by gmco_result). */

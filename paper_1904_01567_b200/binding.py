@@ -26,7 +26,7 @@ class _Structure(C.Structure):
 class Options(C.Structure):
     _fields_ = [("m", C.c_int32), ("eps", C.c_float), ("c1", C.c_float), ("max_trials", C.c_int32),
                 ("precision", C.c_int32), ("eps_f", C.c_float), ("compaction", C.c_int32), ("dose_kernel", C.c_int32),
-                ("wide_accum", C.c_int32), ("reserved", C.c_int32 * 1)]
+                ("wide_accum", C.c_int32), ("line_search", C.c_int32)]
 
 
 class Criterion(C.Structure):
@@ -140,7 +140,7 @@ def _stream(stream):
 
 
 def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32X3, eps_f=None, compaction=None,
-                 dose_kernel=None, wide_accum=None) -> Options:
+                 dose_kernel=None, wide_accum=None, line_search=None) -> Options:
     o = Options()
     lib().gmco_default_options(C.byref(o))
     o.m, o.eps, o.c1, o.max_trials, o.precision = m, eps, c1, max_trials, precision
@@ -152,6 +152,8 @@ def make_options(m=10, eps=0.0, c1=1e-4, max_trials=20, precision=GMCO_PREC_TF32
         o.dose_kernel = int(dose_kernel)
     if wide_accum is not None:
         o.wide_accum = int(wide_accum)
+    if line_search is not None:
+        o.line_search = int(line_search)
     return o
 
 

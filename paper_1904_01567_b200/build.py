@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libgmco.so"
-SOURCES = ["gmco_api.cu", "kernels_simt.cu", "kernels_lbfgs.cu", "kernels_tc.cu", "kernels_sa.cu", "kernels_pool.cu", "kernels_doserate.cu"]
+SOURCES = ["gmco_api.cu", "kernels_simt.cu", "kernels_lbfgs.cu", "kernels_tc.cu", "kernels_sa.cu", "kernels_pool.cu", "kernels_doserate.cu", "kernels_ls.cu"]
 NVCC_FLAGS = ["-O3", "-Wno-deprecated-gpu-targets", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-I", str(ROOT / "include"), "-I", str(CSRC)]
 

@@ -164,6 +164,11 @@ void carve_plans(gmco_handle* h, int K, long long dose_stage_elems) {
   p.status = a.take<int>(kp);
   p.n_running = a.take<int>(2); p.bad_input = a.take<int>(1); p.rounds_done = a.take<int>(2); p.dev_err = a.take<int>(4);
   p.round_log = a.take<int>(kRoundLogCap);
+  if (h->opt.line_search == 1) {
+    p.ls_list = a.take<int>(kLsCap); p.ls_count = a.take<int>(2); p.ls_cols = a.take<float>((size_t)3 * kLsCap * c.N_alloc);
+  } else {
+    p.ls_list = nullptr; p.ls_count = nullptr; p.ls_cols = nullptr;
+  }
   p.tile_seg = a.take<int>(p.K_pad / kPlanTile + 1);
   // partials: the SIMT dose pass (also the final pass of gmco_result) needs [tiles][K_pad][2]
   const size_t f_simt = (size_t)(c.N_alloc / 64) * kp * 2;
@@ -237,6 +242,7 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
     sp.dose_pair = tc_dose_pair(h->tc);
   }
   sp.S = c.S;
+  sp.ls_cap = h->opt.line_search == 1 ? kLsCap : 0;
   return sp;
 }
 
@@ -278,6 +284,7 @@ int enqueue_round(gmco_handle* h, int parity, int log_idx, bool prof, const Step
   if (rc) return rc;
   if (prof) CK(h, cudaEventRecord(h->ev[h->ev_used + 2], st));
   LN(h, launch_step_parity(h->c, h->p, sp, parity, g_scale_of(h), st));
+  if (sp.ls_cap) LN(h, launch_ls(h->c, h->p, sp.max_trials, sp.c1, sp.eps_f, sp.compact_cap > 0, st));
   if (prof) { CK(h, cudaEventRecord(h->ev[h->ev_used + 3], st)); h->ev_used += 4; }
   return GMCO_OK;
 }
@@ -379,7 +386,7 @@ void gmco_default_options(gmco_options* o) {
   if (!o) return;
   memset(o, 0, sizeof(*o));
   o->m = 10; o->eps = 0.f; o->c1 = 1e-4f; o->max_trials = 20; o->precision = GMCO_PREC_TF32X3; o->eps_f = 1e-6f; o->compaction = 1;
-  o->dose_kernel = 0; o->wide_accum = 0;
+  o->dose_kernel = 0; o->wide_accum = 0; o->line_search = 0;
 }
 
 const char* gmco_last_error(const gmco_handle* h) { return h ? h->err : g_create_error; }
@@ -401,7 +408,8 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
       (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || (o.compaction != 0 && o.compaction != 1) ||
-      (o.dose_kernel != 0 && o.dose_kernel != 1) || (o.wide_accum != 0 && o.wide_accum != 1) || o.reserved[0])
+      (o.dose_kernel != 0 && o.dose_kernel != 1) || (o.wide_accum != 0 && o.wide_accum != 1) ||
+      (o.line_search != 0 && o.line_search != 1))
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
   // the plain-fp32 kernels (the paper's largest N_act is 385)

@@ -18,6 +18,7 @@ constexpr int kMaxApad = 480;     // 512 TMEM columns - at least one 32-point ch
 constexpr int kMaxApadTensor = 384; // tensor route: T_hi (A_pad TMEM columns) + one 128-column accumulator pair
 constexpr int kMaxNpl = kMaxApad / 32;  // dwell elements per lane in the warp-per-plan kernels
 constexpr int kRoundLogCap = 8192;      // rounds whose running-plan count is logged (profiling aid)
+constexpr int kLsCap = 128;             // polynomial line search (option): plans queued per round at most (kernels_ls.cu)
 
 // per-plan status codes on the device
 enum : int { PLAN_RUNNING = -1 };
@@ -77,6 +78,10 @@ struct PlanDev {
   int *rounds_done = nullptr;                                      // [2] rounds the device-driven loop has gone through (its bound) | rounds that had a running plan
   int *bad_input = nullptr;                                        // [1] set when T0 / weights hold NaN, inf or negatives
   int *dev_err = nullptr;                                          // [4] device error word (DevErr above)
+  // polynomial line search (gmco_options.line_search = 1; all null otherwise)
+  int *ls_list = nullptr;                                          // [kLsCap] plans whose first trial step was rejected this round
+  int *ls_count = nullptr;                                         // [2] how many | finished CTAs of k_ls_pick
+  float *ls_cols = nullptr;                                        // [3][kLsCap][N_alloc] dose columns d, a, b of the queued plans
   // partial results of one evaluation round
   float *Fpart = nullptr; float *Gpart = nullptr;
   float *R = nullptr;               // SIMT route: dF/dd [K_pad][N_alloc]; tensor route: dF/dd / 2 [N_alloc][K_pad]
@@ -99,6 +104,7 @@ struct StepParams {
   int compact_cap, total_ctas;        // compaction (tensor path): segment cap per tile and CTAs per grid; 0 = off
   int dose_pair;                      // the objective partials follow the CTA-pair split (kernels_tc.cu compact_remap_pair)
   int S;
+  int ls_cap;                         // > 0: a plan whose FIRST trial step is rejected is queued for the polynomial line search
 };
 
 // ---- kernel launchers (each returns the number of kernels it launched, or < 0 on CUDA error) ----
@@ -119,6 +125,8 @@ int launch_eval_finish_scaled(const CaseDev& c, const PlanDev& p, const StepPara
 int launch_result(const CaseDev& c, const PlanDev& p, const StructHost* sh, float* T_out, float* F_out,
                   float* dvh_out, float* terms_out, int* iters_out, int* status_out, cudaStream_t st);
 int launch_prepare_final(const CaseDev& c, const PlanDev& p, cudaStream_t st);
+// polynomial line search (kernels_ls.cu): dose columns of the queued plans, then the choice of their next trial step
+int launch_ls(const CaseDev& c, const PlanDev& p, int max_trials, float c1, float eps_f, bool use_slot, cudaStream_t st);
 
 // gSA (kernels_sa.cu): one CTA of kSaThreads per chain, draws staged kSaBlock steps at a time
 constexpr int kSaThreads = 512;

@@ -25,7 +25,7 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 struct PlanPtrs {
   float *x, *g, *p, *xt, *T, *T_lo, *Sh, *Yh, *rho, *gam, *F, *gp, *alpha;
-  int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input, *dev_err;
+  int *it_done, *trials, *hcount, *hhead, *status, *n_running, *bad_input, *dev_err, *ls_list, *ls_count;
   int K_pad;
   float *Weff, *WeffC;        // [K_pad][2S] effective weights by plan / by slot
   int* slot;                  // [K_pad] row of plan k in T, R and the partials (= k without compaction)
@@ -37,6 +37,7 @@ static PlanPtrs make_ptrs(const PlanDev& p) {
   q.Sh = p.Sh; q.Yh = p.Yh; q.rho = p.rho; q.gam = p.gam; q.F = p.F; q.gp = p.gp; q.alpha = p.alpha;
   q.it_done = p.it_done; q.trials = p.trials; q.hcount = p.hcount; q.hhead = p.hhead; q.status = p.status;
   q.n_running = p.n_running; q.bad_input = p.bad_input; q.dev_err = p.dev_err; q.K_pad = p.K_pad;
+  q.ls_list = p.ls_list; q.ls_count = p.ls_count;
   q.Weff = p.Weff; q.WeffC = p.WeffC; q.slot = p.slot;
   return q;
 }
@@ -81,6 +82,7 @@ int launch_init_plans(const CaseDev& c, const PlanDev& p, const float* T0, int t
   cudaMemsetAsync(p.bad_input, 0, sizeof(int), st);
   cudaMemsetAsync(p.rounds_done, 0, 2 * sizeof(int), st);
   cudaMemsetAsync(p.dev_err, 0, 4 * sizeof(int), st);
+  if (p.ls_count) cudaMemsetAsync(p.ls_count, 0, 2 * sizeof(int), st);
   k_init_plans<<<p.K_pad, 128, 0, st>>>(make_ptrs(p), p.K, c.A, c.A_pad, c.S, T0, t0_bcast, w_user, struct_scale,
                                         p.Weff);
   return cudaGetLastError() == cudaSuccess ? 1 : -1;
@@ -310,6 +312,12 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
             if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn_(t - tf32_rn_(t));
           }
         if (lane == 0) { pp.alpha[k] = a2; pp.trials[k] = tr; }
+        // option: the first rejection of an iteration queues the plan for the polynomial line search (kernels_ls.cu),
+        // which may replace the halved trial point written above by a later candidate before the next round
+        if (sp.ls_cap && tr == 1 && lane == 0) {
+          const int e = atomicAdd(pp.ls_count, 1);
+          if (e < sp.ls_cap) pp.ls_list[e] = k;
+        }
       }
     }
   }

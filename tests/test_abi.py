@@ -40,7 +40,7 @@ def test_version_and_default_options(built_lib):
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
-    assert o.compaction == 1 and o.dose_kernel == 0 and o.wide_accum == 0 and list(o.reserved) == [0]
+    assert o.compaction == 1 and o.dose_kernel == 0 and o.wide_accum == 0 and o.line_search == 0
 
 
 def test_struct_layouts_match_the_header(built_lib):

@@ -1,0 +1,58 @@
+"""-m gpu, sorted LAST on purpose: gmco_options.line_search = 1 (kernels_ls.cu, the polynomial line search of north_star
+item (4)) has never run on hardware.  Same algorithm as the default route: iteration counts must equal the oracle's,
+final objective within 1e-3, DVH within 0.5 pp; an iteration with h rejected steps costs 2 rounds instead of 1 + h, so the
+number of rounds may only go down.  If this file fails, the default path (tested by the files that run before it) is
+unaffected."""
+import numpy as np
+import pytest
+
+import gmco_cases as gc
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def g():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a B200"
+    import paper_1904_01567_b200 as g
+    from paper_1904_01567_b200 import build
+    build.build()
+    return g
+
+
+def _run(g, c, iters, **opt):
+    h = g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(m=c.m, **opt))
+    try:
+        g.gmco_optimize(h, c.T0, c.weights, iters)
+        out = g.gmco_result(h, host=True)
+        out["stats"] = g.gmco_get_stats(h)
+        return out
+    finally:
+        g.gmco_destroy(h)
+
+
+@pytest.mark.parametrize("prec", [1, 0], ids=["simt_fp32", "tf32x3"])
+@pytest.mark.parametrize("name,n_plans,iters", [("C1", 8, 50), ("C1", 300, 50), ("C2", 100, 120)])
+def test_polynomial_line_search_follows_the_oracle(g, prec, name, n_plans, iters):
+    c = gc.make_case(name, n_plans=n_plans)
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=iters)
+    base = _run(g, c, iters, precision=prec, line_search=0)
+    poly = _run(g, c, iters, precision=prec, line_search=1)
+    for out in (base, poly):
+        assert (out["iters_done"] == ref["iters_done"]).all()
+        assert (np.abs(out["objective"] - ref["F"]) / ref["F"]).max() < 1e-3
+        assert np.abs(out["dvh"] - ref["dvh"]).max() < 0.5
+        assert (out["T"] >= 0).all() and np.isfinite(out["T"]).all()
+    assert ref["n_backtracks"].sum() > 0                                   # the case does backtrack
+    assert poly["stats"]["rounds"] <= base["stats"]["rounds"]
+    # per plan: 1 + iterations + (iterations that backtracked) rounds at most, so the pool needs at most this many
+    assert poly["stats"]["rounds"] <= 1 + iters + int(ref["n_bt_iters"].max()) + 2
+
+
+def test_polynomial_line_search_is_deterministic(g):
+    c = gc.make_case("C1", n_plans=300)
+    a = _run(g, c, 40, line_search=1)
+    b = _run(g, c, 40, line_search=1)
+    assert (a["T"] == b["T"]).all() and (a["objective"] == b["objective"]).all()

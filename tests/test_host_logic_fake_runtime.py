@@ -98,6 +98,9 @@ scenario("pair_forced_single", pair, b.make_options(m=pair.m, dose_kernel=1))
 wide = gc.make_case("C1", n_cath=24, n_pos=16, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
 scenario("wide_streamed", wide, b.make_options(m=wide.m, eps=1e-3, compaction=0))
 scenario("wide_split_main", wide, b.make_options(m=wide.m, wide_accum=1))
+scenario("poly_ls_tf32", c1, b.make_options(m=c1.m, line_search=1))
+scenario("poly_ls_simt_profile", c1, b.make_options(m=c1.m, line_search=1, precision=1), profile=True)
+scenario("poly_ls_wide", wide, b.make_options(m=wide.m, line_search=1))
 c3 = gc.make_case("C3")
 scenario("c3_pair_static", c3, b.make_options(m=c3.m), iters=200)
 widest = gc.make_case("C1", n_cath=35, n_pos=11, counts=(300, 64, 100, 100), n_plans=5, seed_points=5)   # 385 dwell positions: SIMT route
@@ -203,6 +206,19 @@ def test_shapes_and_statistics_of_every_route(report):
     assert report["c1_profile"]["stats"]["eval_launches"] == 0        # nothing ran: no round had a running plan
     assert report["pool"]["sa_shape"] == [8, c1.n_dwell] and report["pool"]["D"] == [100, 7]
     assert any("k_sa" in k for k in report["pool"]["kernels"]) and any("k_pareto" in k for k in report["pool"]["kernels"])
+
+
+def test_polynomial_line_search_option_adds_its_two_kernels_to_every_round(report):
+    import gmco_cases as gc
+    c1 = gc.make_case("C1")
+    n_alloc = 256 * ((sum(64 * ((s.n_points + 63) // 64) for s in c1.structures) + 255) // 256)
+    rep = report["poly_ls_tf32"]
+    cols, pick = _one(rep, "k_ls_cols", captured=1), _one(rep, "k_ls_pick", captured=1)
+    assert cols["grid"] == [n_alloc // 64, 128 // 16, 1] and cols["block"] == [256, 1, 1]
+    assert pick["grid"] == [128, 1, 1] and pick["block"] == [256, 1, 1]
+    assert _one(report["poly_ls_simt_profile"], "k_ls_pick", captured=0) and _one(report["poly_ls_wide"], "k_ls_cols", captured=1)
+    for tag in ("c1_tf32", "c1_simt", "c3_pair_static", "wide_streamed"):          # off by default: not a single launch
+        assert not [k for k in report[tag]["kernels"] if "k_ls_" in k], tag
 
 
 def test_every_launch_is_the_one_the_schedule_announces(report):

@@ -170,6 +170,20 @@ def test_line_search_polynomial_identity(case_small):
         assert lhs == pytest.approx(rhs, rel=1e-12)
 
 
+def test_line_search_polynomial_slope_identity(case_small):
+    """phi'(alpha) = grad F(x + alpha p) . p = sum_i dF/dd_i (2 a_i + 2 alpha b_i) with a = D(x o p), b = D(p o p): what the
+    optional polynomial line search (kernels_ls.cu) uses for the slope condition of the approximate test, written with
+    the oracle's r = dF/dd and gradient."""
+    c = case_small
+    rng = np.random.default_rng(5)
+    x = np.sqrt(rng.uniform(0.5, 1.5, c.n_dwell)); p = rng.normal(size=c.n_dwell) * 0.2
+    Dd = c.D.astype(np.float64)
+    a_col, b_col = Dd @ (x * p), Dd @ (p * p)
+    for al in (1.0, 0.5, 0.25, 0.0625):
+        ev = oracle.eval_plan(c.D, c.structures, c.weights[0], x + al * p)
+        assert ev["g"] @ p == pytest.approx(ev["r"] @ (2 * a_col + 2 * al * b_col), rel=1e-10)
+
+
 def test_structure_sizes_must_add_up(case_small):
     c = case_small
     with pytest.raises(ValueError):
