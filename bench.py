@@ -215,6 +215,8 @@ def workload_config(case, args, stats):
            "l2": "flushed between timed steps (512 MiB write)", "parallelism": f"k-shard x{args.gpus}"}
     cfg["eps"] = getattr(args, "eps", 0.0)
     cfg["compaction"] = getattr(args, "compaction", 1)
+    cfg["line_search"] = getattr(args, "line_search", 0)
+    cfg["wide_accum"] = getattr(args, "wide_accum", 0)
     if stats:
         cfg["rounds"] = stats["rounds"]
         cfg["device_bytes"] = stats["device_bytes"]
@@ -234,6 +236,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-peak", action="store_true", help="skip the live tf32 matmul peak measurement (roofline falls back to the nominal ratio)")
     ap.add_argument("--dose-kernel", type=int, default=0, choices=[0, 1], help="gmco_options.dose_kernel (1 = keep the single-CTA dose kernel)")
+    ap.add_argument("--line-search", type=int, default=0, choices=[0, 1], help="gmco_options.line_search (1 = polynomial line search, an option that is off by default)")
+    ap.add_argument("--wide-accum", type=int, default=0, choices=[0, 1], help="gmco_options.wide_accum (1 = split main accumulator above 256 dwell positions)")
     ap.add_argument("--no-gsa", action="store_true", help="skip the gSA-vs-gL-BFGS comparison leg (C5)")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the C1 / C2 / C4 legs (SURVEY 8(d): 'plus the same for C1, C2, C4')")
     ap.add_argument("--clock-period", type=float, default=0.02, help="seconds between NVML clock samples (0 = off)")
@@ -280,7 +284,8 @@ def main():
 
     def step(host: bool, profile: bool = False):
         Dm, Tm, wm, om = (D_pin, T0_pin, w_pin, out_pin) if host else (D_dev, T0_dev, w_dev, out_dev)
-        opt = g.binding.make_options(m=case.m, precision=prec, eps=args.eps, compaction=args.compaction, dose_kernel=args.dose_kernel)
+        opt = g.binding.make_options(m=case.m, precision=prec, eps=args.eps, compaction=args.compaction, dose_kernel=args.dose_kernel,
+                                     line_search=args.line_search, wide_accum=args.wide_accum)
         h = g.gmco_create(Dm, case.structures, case.rx, opt, stream)
         try:
             if profile:
