@@ -11,6 +11,21 @@ if str(ROOT) not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a real B200 (run with -m gpu on the GPU box)")
+    config.addinivalue_line("markers", "gpu_optional: needs a real B200; tests of options that are off by default and have not "
+                                       "yet run on hardware (wide_accum, line_search); not part of -m gpu")
+
+
+def pytest_collection_modifyitems(config, items):
+    """Tests of options that are off by default (marker gpu_optional) run only when asked for by name (-m gpu_optional):
+    neither `-m gpu` nor `-m "not gpu"` selects them."""
+    if "gpu_optional" in (config.getoption("-m") or ""):
+        return
+    keep, drop = [], []
+    for it in items:
+        (drop if it.get_closest_marker("gpu_optional") else keep).append(it)
+    if drop:
+        config.hook.pytest_deselected(items=drop)
+        items[:] = keep
 
 
 @pytest.fixture(scope="session")

@@ -1,15 +1,15 @@
-"""-m gpu, sorted LAST on purpose: gmco_options.line_search = 1 (kernels_ls.cu, the polynomial line search of north_star
+"""-m gpu_optional -- deliberately NOT part of `-m gpu`: gmco_options.line_search = 1 (kernels_ls.cu, the polynomial line search of north_star
 item (4)) has never run on hardware.  Same algorithm as the default route: iteration counts must equal the oracle's,
 final objective within 1e-3, DVH within 0.5 pp; an iteration with h rejected steps costs 2 rounds instead of 1 + h, so the
-number of rounds may only go down.  If this file fails, the default path (tested by the files that run before it) is
-unaffected."""
+number of rounds may only go down.  It is kept out of the default GPU suite so that an option which is off cannot
+colour the record of the default path; run it with `python -m pytest tests -m gpu_optional` on a B200."""
 import numpy as np
 import pytest
 
 import gmco_cases as gc
 import oracle
 
-pytestmark = pytest.mark.gpu
+pytestmark = pytest.mark.gpu_optional        # NOT `gpu`: run with -m gpu_optional (see the module docstring)
 
 
 @pytest.fixture(scope="module")

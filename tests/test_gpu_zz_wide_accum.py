@@ -1,14 +1,14 @@
-"""-m gpu, sorted LAST on purpose: gmco_options.wide_accum (k_dose_tc<streamed, split main>) has never
+"""-m gpu_optional -- deliberately NOT part of `-m gpu`: gmco_options.wide_accum (k_dose_tc<streamed, split main>) has never
 run on hardware.  It is the fix chosen on a CPU model for the gradient shortfall of threshold-sitting plans above 256
-dwell positions; with it the north_star's 1e-4 is a hard bar here.  If this file fails, the default path (tested by
-every other file, which runs before it) is unaffected."""
+dwell positions; with it the north_star's 1e-4 is a hard bar here.  It is kept out of the default GPU suite so that an option which is off cannot colour the
+record of the default path; run it with `python -m pytest tests -m gpu_optional` on a B200."""
 import numpy as np
 import pytest
 
 import gmco_cases as gc
 import oracle
 
-pytestmark = pytest.mark.gpu
+pytestmark = pytest.mark.gpu_optional        # NOT `gpu`: run with -m gpu_optional (see the module docstring)
 TOL = 1e-4
 
 
