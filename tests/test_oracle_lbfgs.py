@@ -194,3 +194,65 @@ def test_dwell_starting_at_zero_stays_at_zero(case_small):
     T0 = np.repeat(c.T0[None], 1, axis=0).copy(); T0[0, [3, 17]] = 0.0
     res = oracle.optimize(c.D, c.structures, c.rx, T0, c.weights[:1], m=5, iters=30)
     assert (res["T"][0, [3, 17]] == 0).all() and (res["T"][0] >= 0).all()
+
+
+def test_polynomial_values_choose_the_step_the_halving_search_accepts(case_small):
+    """The optional polynomial line search (csrc/kernels_ls.cu) restated in numpy and held to the oracle:
+    along real gL-BFGS trajectories, in every iteration whose first trial step is rejected, the first candidate
+    alpha_j = 2^-j that meets the Armijo or the approximate test on the POLYNOMIAL values phi(alpha) = F(d + 2 alpha a +
+    alpha^2 b), phi'(alpha) = sum_i dF/dd_i (2 a_i + 2 alpha b_i) -- formed in fp32 as the kernel forms them -- is the step
+    the oracle's halving search accepts after evaluating every trial point in full."""
+    c = case_small
+    D32 = c.D.astype(np.float32)
+    n_checked = 0
+    for k in range(c.n_plans):
+        w = c.weights[k]
+        calls = []                                                    # every evaluation the driver asks for, in order
+
+        def fg(x):
+            ev = oracle.eval_plan(c.D, c.structures, w, x)
+            calls.append((x.copy(), ev["F"], ev["g"].copy()))
+            return ev["F"], ev["g"]
+        res = oracle.lbfgs(fg, np.sqrt(c.T0.astype(np.float64)), m=5, iters=60)
+        # split the call sequence into iterations: a call whose point is x_acc + alpha p with alpha = 1 starts one
+        i, x_acc, F_acc, g_acc = 1, calls[0][0], calls[0][1], calls[0][2]
+        while i < len(calls):
+            p = calls[i][0] - x_acc                                   # the alpha = 1 trial defines the direction
+            gp = float(g_acc @ p)
+            trials = [calls[i]]
+            al = 1.0
+            def accepted(t, al):
+                return t[1] <= F_acc + 1e-4 * al * gp or (t[1] <= F_acc + oracle.EPS_F * abs(F_acc) and t[2] @ p <= (2e-4 - 1.0) * gp)
+            while not accepted(trials[-1], al) and i + 1 < len(calls) and np.allclose(calls[i + 1][0], x_acc + 0.5 * al * p, rtol=0, atol=1e-12):
+                i += 1; al *= 0.5; trials.append(calls[i])
+            if not accepted(trials[-1], al):
+                break                                                 # the run ended inside a line search
+            if len(trials) > 1:                                       # the first trial was rejected: the polynomial route's case
+                xs, ps = x_acc.astype(np.float32), p.astype(np.float32)
+                d = D32 @ (xs * xs); a = D32 @ (xs * ps); b = D32 @ (ps * ps)
+                sid = np.repeat(np.arange(len(c.structures)), [s.n_points for s in c.structures])
+                dlo = np.array([c.structures[s].d_lo for s in sid], np.float32); dhi = np.array([c.structures[s].d_hi for s in sid], np.float32)
+                wl = np.array([w[s, 0] * c.structures[s].w_lo / c.structures[s].n_points for s in sid], np.float32)
+                wh = np.array([w[s, 1] * c.structures[s].w_hi / c.structures[s].n_points for s in sid], np.float32)
+
+                def phi(alj):
+                    dj = (d + np.float32(2 * alj) * a + np.float32(alj * alj) * b).astype(np.float32)
+                    lo, hi = np.minimum(dj - dlo, 0), np.maximum(dj - dhi, 0)
+                    val = float((wl * lo * lo + wh * hi * hi).sum(dtype=np.float32))
+                    slope = float((2 * (wl * lo + wh * hi) * 2 * (a + np.float32(alj) * b)).sum(dtype=np.float32))
+                    return val, slope
+                F0 = phi(0.0)[0]
+                pick, alj = 0, 1.0
+                for j in range(1, 20):
+                    alj *= 0.5
+                    Fj, sj = phi(alj)
+                    if Fj <= F0 + 1e-4 * alj * gp or (Fj <= F0 + oracle.EPS_F * abs(F0) and sj <= (2e-4 - 1.0) * gp):
+                        pick = j
+                        break
+                assert pick == len(trials) - 1, (k, pick, len(trials) - 1)
+                n_checked += 1
+            x_acc, F_acc, g_acc = trials[-1]
+            i += 1
+        assert res["iters_done"] > 0
+    print("iterations with a rejected first trial checked:", n_checked)
+    assert n_checked >= 3                                             # the trajectories do contain rejected first trials
