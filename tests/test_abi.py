@@ -97,3 +97,30 @@ def test_product_never_imports_the_oracle():
             txt = p.read_text()
             assert "import paper_1904_01567_b200" not in txt and "from paper_1904_01567_b200" not in txt
             assert "gmco.h" not in txt
+
+
+def test_ctypes_field_offsets_match_the_header_as_gcc_lays_it_out(tmp_path):
+    """Every field of the binding's ctypes mirrors sits where a C compiler puts it in include/gmco.h (a drifted binding
+    would read the wrong statistic or set the wrong option without any error)."""
+    import shutil
+    import subprocess
+    import paper_1904_01567_b200.binding as b
+    if not shutil.which("gcc"):
+        pytest.skip("gcc not available")
+    pairs = [("gmco_structure", b._Structure), ("gmco_options", b.Options), ("gmco_stats", b.Stats),
+             ("gmco_criterion", b.Criterion), ("gmco_tc_info", b.TcInfo)]
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "gmco.h"', 'int main(void) {']
+    for cname, ct in pairs:
+        lines.append(f'  printf("{cname} %zu\\n", sizeof({cname}));')
+        for fname, _ in ct._fields_:
+            lines.append(f'  printf("{cname}.{fname} %zu\\n", offsetof({cname}, {fname}));')
+    lines += ['  return 0;', '}']
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", str(ROOT / "include"), "-o", str(exe), str(src)], check=True)
+    out = dict(ln.split() for ln in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.splitlines())
+    for cname, ct in pairs:
+        assert int(out[cname]) == ctypes.sizeof(ct), cname
+        for fname, _ in ct._fields_:
+            assert int(out[f"{cname}.{fname}"]) == getattr(ct, fname).offset, f"{cname}.{fname}"
