@@ -124,3 +124,20 @@ def test_ctypes_field_offsets_match_the_header_as_gcc_lays_it_out(tmp_path):
         assert int(out[cname]) == ctypes.sizeof(ct), cname
         for fname, _ in ct._fields_:
             assert int(out[f"{cname}.{fname}"]) == getattr(ct, fname).offset, f"{cname}.{fname}"
+
+
+def test_binding_argument_counts_match_the_prototypes(built_lib):
+    """The number of arguments the binding marshals for each entry point equals the header's prototype."""
+    import paper_1904_01567_b200.binding as b
+    text = (ROOT / "include" / "gmco.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    protos = dict(re.findall(r"GMCO_API\s+[\w\s\*]+?\b(gmco_\w+)\s*\(([^;]*?)\)\s*;", text, flags=re.S))
+    L = b.lib()
+    checked = 0
+    for name, args in protos.items():
+        n = 0 if args.strip() in ("", "void") else len([a for a in args.split(",") if a.strip()])
+        fn = getattr(L, name)
+        if fn.argtypes is not None:
+            assert len(fn.argtypes) == n, (name, len(fn.argtypes), n)
+            checked += 1
+    assert checked >= 12
