@@ -8,14 +8,9 @@
 // running plan has exactly one trial point x + alpha p evaluated by the contraction kernels; this
 // kernel then either accepts it (history push, new direction, alpha = 1) or halves alpha.
 #include "gmco_internal.cuh"
+#include "gmco_ptx.cuh"
 
 namespace gmco {
-
-__device__ __forceinline__ float tf32_rn_(float v) {
-  uint32_t u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
-  return __uint_as_float(u);
-}
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -58,7 +53,7 @@ __global__ void k_init_plans(PlanPtrs pp, int K, int A, int A_pad, int S, const 
     const long long i = (long long)k * A_pad + a;
     pp.x[i] = x; pp.xt[i] = x; pp.g[i] = 0.f; pp.p[i] = 0.f;
     pp.T[i] = t;
-    if (pp.T_lo) pp.T_lo[i] = tf32_rn_(t - tf32_rn_(t));   // only the streamed dose layout (more than 256 dwell positions) reads it
+    if (pp.T_lo) pp.T_lo[i] = tf32_rn(t - tf32_rn(t));   // only the streamed dose layout (more than 256 dwell positions) reads it
   }
   for (int j = threadIdx.x; j < 2 * S; j += blockDim.x) {
     float w = 0.f;
@@ -147,13 +142,11 @@ __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, in
 // The history of a plan (m pairs, 2 m A_pad floats) is staged in shared memory by bulk asynchronous copies issued
 // at the very start, so the 2 m dependent dot products of the two-loop recursion read shared memory instead of
 // paying one HBM/L2 latency each.  wpb warps (= plans) per CTA; dynamic smem = wpb * 2 m A_pad floats.
-__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
 template <int NPL>
 __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int parity, float g_scale, int wpb) {
   extern __shared__ __align__(128) float s_hist[];
   __shared__ float s_a[4][GMCO_MAX_HISTORY];
-  __shared__ __align__(8) unsigned long long s_bar[4];
+  __shared__ __align__(8) uint64_t s_bar[4];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int k = blockIdx.x * wpb + warp;
   if (k >= sp.K) return;
@@ -188,34 +181,31 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
   float* hS = s_hist + (size_t)warp * 2 * sp.m * sp.A_pad;     // [m][A_pad] s vectors, by ring slot
   float* hY = hS + (size_t)sp.m * sp.A_pad;                    // [m][A_pad] y vectors
   {
-    const uint32_t bar = smem_addr(&s_bar[warp]);
+    uint64_t* bar = &s_bar[warp];
     const uint32_t bytes = (uint32_t)sp.A_pad * 4u;
     if (lane == 0) {
-      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * 2u * (uint32_t)sp.m) : "memory");
+      mbar_init(bar, 1);
+      fence_barrier_init();
+      mbar_expect_tx(bar, bytes * 2u * (uint32_t)sp.m);
     }
     __syncwarp();
     for (int i = lane; i < 2 * sp.m; i += 32) {                // one 4 A_pad byte row per lane
       const int slot = i < sp.m ? i : i - sp.m;
       const float* src = (i < sp.m ? pp.Sh : pp.Yh) + slot * hstride + (long long)k * sp.A_pad;
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(smem_addr(hS + (size_t)i * sp.A_pad)), "l"(src), "r"(bytes), "r"(bar) : "memory");
+      bulk_load(hS + (size_t)i * sp.A_pad, src, bytes, bar);
     }
   }
   // Every path below waits for the copies before the warp may leave (the CTA's shared memory must outlive them).
   // The wait is bounded: copies that have not landed after seconds are a fault of the machine, not a state to spin
   // in -- the device error word is set (the host reports GMCO_E_CUDA) and the warp goes on.
   auto hist_wait = [&]() {
-    const uint32_t bar = smem_addr(&s_bar[warp]);
-    uint32_t ok = 0;
+    const uint32_t bar = smem_u32(&s_bar[warp]);
+    bool ok = false;
     unsigned long long t0 = 0;
     for (uint32_t spins = 1; !ok; ++spins) {
-      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                   : "=r"(ok) : "r"(bar) : "memory");
+      ok = mbar_try_wait_addr(bar, 0);
       if (!ok && (spins & 4095u) == 0u) {        // the clock is read rarely: this wait is on the kernel's critical path
-        unsigned long long now;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+        const unsigned long long now = global_ns();
         if (t0 == 0) t0 = now;
         else if (now - t0 > 4000000000ull) {
           if (lane == 0 && atomicCAS(pp.dev_err, 0, (int)DEVERR_WAIT_TIMEOUT) == 0) {
@@ -309,7 +299,7 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
             const float pv = pp.p[row + 32 * j];
             const float xn = fmaf(a2, pv, x[j]), t = xn * xn;
             pp.xt[row + 32 * j] = xn; pp.T[trow + 32 * j] = t;
-            if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn_(t - tf32_rn_(t));
+            if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn(t - tf32_rn(t));
           }
         if (lane == 0) { pp.alpha[k] = a2; pp.trials[k] = tr; }
         // option: the first rejection of an iteration queues the plan for the polynomial line search (kernels_ls.cu),
@@ -392,7 +382,7 @@ __global__ void __launch_bounds__(128) k_step(StepParams sp, PlanPtrs pp, int pa
           const float xn = x[j] + pv, t = xn * xn;
           pp.p[row + 32 * j] = pv; pp.xt[row + 32 * j] = xn;
           pp.T[trow + 32 * j] = t;
-          if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn_(t - tf32_rn_(t));
+          if (pp.T_lo) pp.T_lo[trow + 32 * j] = tf32_rn(t - tf32_rn(t));
         }
       if (lane == 0) { pp.gp[k] = gpn; pp.alpha[k] = 1.f; pp.trials[k] = 0; }
     }

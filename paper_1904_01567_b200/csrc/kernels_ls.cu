@@ -18,17 +18,12 @@
 // (and the oracle's iteration count) is unchanged; an iteration with h rejected steps costs 2 rounds instead of 1 + h.
 // Plain fp32 FMA kernels: a few dozen plans per round at most.  Product code; shares nothing with oracle/.
 #include "gmco_internal.cuh"
+#include "gmco_ptx.cuh"
 #include "penalty.cuh"
 
 namespace gmco {
 
 namespace {
-
-__device__ __forceinline__ float tf32_rn_ls(float v) {
-  uint32_t u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
-  return __uint_as_float(u);
-}
 
 constexpr int kLsMaxCand = 19;      // candidates alpha_j = 2^-j, j = 1 .. min(max_trials - 1, kLsMaxCand)
 
@@ -166,7 +161,7 @@ __global__ void __launch_bounds__(256) k_ls_pick(LsPickArgs a) {
       for (int q = tid; q < a.A_pad; q += 256) {
         const float xn = fmaf(al, a.p[row + q], a.x[row + q]), t = xn * xn;
         a.xt[row + q] = xn; a.T[trow + q] = t;
-        if (a.T_lo) a.T_lo[trow + q] = tf32_rn_ls(t - tf32_rn_ls(t));
+        if (a.T_lo) a.T_lo[trow + q] = tf32_rn(t - tf32_rn(t));
       }
       if (tid == 0) { a.alpha[k] = al; a.trials[k] = pick; }
     }

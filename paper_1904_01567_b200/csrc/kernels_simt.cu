@@ -5,15 +5,10 @@
 // route that can hand dose to the caller (gmco_evaluate's debug output).  The production
 // contraction is the tcgen05 kernel in kernel_fused_tc.cu.
 #include "gmco_internal.cuh"
+#include "gmco_ptx.cuh"
 #include "penalty.cuh"
 
 namespace gmco {
-
-__device__ __forceinline__ float tf32_rn(float v) {
-  uint32_t u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
-  return __uint_as_float(u);
-}
 
 // ---------------------------------------------------------------------------------------------
 // a0: D_user [N][ldD] -> D [N_alloc][A_pad] (rows regrouped/padded via row_src), optional tf32 parts.
