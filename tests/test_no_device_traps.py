@@ -22,14 +22,23 @@ def test_sources_hold_no_trap_and_no_unbounded_spin():
         code = re.sub(r"//[^\n]*", "", p.read_text())            # comments may talk about traps
         assert "__trap" not in code and not re.search(r"\btrap\s*;", code) and "brkpt" not in code, p
         assert "getenv" not in code and "fprintf" not in code and "printf(" not in code.replace("snprintf(", ""), p
-    # every mbarrier wait of the tensor kernels goes through the bounded helpers: the raw try_wait wrappers are called
-    # from mbar_wait_slow / mbar_wait_addr / mbar_wait_cluster only (2 definitions + 4 calls)
+    # all inline assembly lives in gmco_ptx.cuh (the seam the CPU-side kernel emulation of tests/emu replaces)
+    for p in _sources():
+        if p.name != "gmco_ptx.cuh":
+            assert not re.search(r"\basm\b", re.sub(r"//[^\n]*", "", p.read_text())), p
+    ptx = re.sub(r"//[^\n]*", "", (CSRC / "gmco_ptx.cuh").read_text())
+    assert len(re.findall(r"try_wait\.parity", ptx)) == 2               # the two raw (unbounded-by-themselves) polls
+    # every mbarrier wait of the tensor kernels goes through the bounded helpers: the raw polls are called from
+    # mbar_wait_slow / mbar_wait_addr / mbar_wait_cluster only (4 calls), and from k_step's bounded history wait (1 call)
     tc = re.sub(r"//[^\n]*", "", (CSRC / "kernels_tc.cu").read_text())
     assert "kWaitLimitNs" in tc and "mbar_wait_slow" in tc and "drain_if_aborted" in tc
-    assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", tc)) == 6
-    assert len(re.findall(r"try_wait\.parity", tc)) == 2
+    assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", tc)) == 4
     lb = re.sub(r"//[^\n]*", "", (CSRC / "kernels_lbfgs.cu").read_text())
+    assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", lb)) == 1
     assert "4000000000ull" in lb and "DEVERR_W_HISTORY" in lb            # k_step's history wait is bounded too
+    for p in _sources():
+        if p.name not in ("gmco_ptx.cuh", "kernels_tc.cu", "kernels_lbfgs.cu"):
+            assert "mbar_try_wait" not in p.read_text(), p
 
 
 def test_sass_holds_no_trap_besides_the_tcgen05_alloc_stubs():
