@@ -1,0 +1,221 @@
+"""Runs libgmco's kernel SOURCE on the CPU emulation (tests/emu/_build/libgmco_emu.so) and reports, as one JSON line,
+how the results compare with the fp64 oracle.  TEST INFRASTRUCTURE ONLY; started as a subprocess by
+tests/test_emu_*.py so that the real library loaded by the other tests is untouched:
+
+    python tests/emu/driver.py '<json: {"scenario": name, ...options}>'
+
+Everything goes through the product's own Python binding (paper_1904_01567_b200.binding) pointed at the emulated
+library: same C ABI, same host code, same kernels; only the PTX layer and the CUDA runtime are the models of
+tests/emu/emu_ptx.h and emu_runtime.cc.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import json
+import sys
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parents[2]
+sys.path.insert(0, str(ROOT))
+
+import gmco_cases as gc  # noqa: E402
+import oracle  # noqa: E402
+import paper_1904_01567_b200.binding as b  # noqa: E402
+
+
+def load(lib: Path):
+    b.lib_path = lambda: lib
+    b._lib = None
+    b._stream = lambda stream: None          # no torch, no CUDA stream: the emulated runtime has one order of execution
+    import paper_1904_01567_b200 as g
+    E = C.CDLL(str(lib))
+    E.emu_violation_message.restype = C.c_char_p
+    E.emu_set.argtypes = [C.c_char_p, C.c_long]
+    E.emu_counter.argtypes = [C.c_char_p]
+    E.emu_counter.restype = C.c_long
+    return g, E
+
+
+def configure(E, a):
+    for key in ("seed", "max_delay", "dyn_misalign", "sm_count", "shuffle", "verbose"):
+        if key in a:
+            E.emu_set(key.encode(), int(a[key]))
+
+
+def custom_case(a):
+    """C1 by default; any field of gmco_cases.make_case may be overridden from the scenario's arguments."""
+    kw = {k: a[k] for k in ("n_plans", "n_cath", "n_pos", "counts", "m", "iters", "seed_points", "seed_weights") if k in a}
+    return gc.make_case(a.get("case", "C1"), **kw)
+
+
+def spread_start(c, seed=100):
+    """Non-converged evaluation points (as tests/test_gpu_zy_fullsize.py): a random start scaled per plan over 0.5 .. 1.5."""
+    return np.repeat(gc.random_starts(c, 1, seed=seed), c.n_plans, axis=0) * np.linspace(0.5, 1.5, c.n_plans)[:, None].astype(np.float32)
+
+
+def eval_errors(out, ref):
+    e_d = float((np.abs(out["dose"] - ref["dose"]) / np.abs(ref["dose"])).max())
+    e_f = float((np.abs(out["F"] - ref["F"]) / ref["F"]).max())
+    e_g = float((np.linalg.norm(out["grad_x"] - ref["grad_x"], axis=1) / np.linalg.norm(ref["grad_x"], axis=1)).max())
+    return dict(dose=e_d, F=e_f, grad=e_g)
+
+
+def options(a, c):
+    kw = {k: a[k] for k in ("precision", "eps", "compaction", "dose_kernel", "wide_accum", "line_search", "eps_f", "max_trials") if k in a}
+    return b.make_options(m=c.m, **kw)
+
+
+def digest(*arrays):
+    import hashlib
+    h = hashlib.sha256()
+    for x in arrays:
+        h.update(np.ascontiguousarray(x).tobytes())
+    return h.hexdigest()
+
+
+def report(E, **kw):
+    kw.update(violations=int(E.emu_violations()), violation=(E.emu_violation_message() or b"").decode(),
+              hangs=int(E.emu_counter(b"hangs")), mma=int(E.emu_counter(b"mma")), tma=int(E.emu_counter(b"tma")),
+              live_allocations=int(E.emu_live_allocations()))
+    return kw
+
+
+# ---- scenarios -----------------------------------------------------------------------------------------------------
+def sc_evaluate(g, E, a):
+    """One gmco_evaluate: dose, objective and gradient of every plan against the oracle."""
+    c = custom_case(a)
+    T = spread_start(c) if a.get("start", "spread") == "spread" else np.repeat(c.T0[None], c.n_plans, axis=0)
+    ref = oracle.evaluate(c.D, c.structures, T, c.weights)
+    sched = g.gmco_tc_schedule(c.n_dwell, [s.n_points for s in c.structures], c.n_plans, int(a.get("sm_count", 148)),
+                               int(a.get("dose_kernel", 0)), int(a.get("wide_accum", 0)))
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    try:
+        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
+    finally:
+        g.gmco_destroy(h)
+    return report(E, errors=eval_errors(out, ref), schedule={k: int(v) for k, v in sched.items()},
+                  digest=digest(out["dose"], out["F"], out["grad_x"]),
+                  kernels={k: int(E.emu_counter(k.encode())) for k in ("k_dose_tc<true>", "k_dose_tc<false>", "k_dose_tc<false, true>",
+                                                                       "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16>", "k_simt_dose", "k_simt_grad")})
+
+
+def sc_optimize(g, E, a):
+    """gmco_optimize + gmco_result (the device-side WHILE loop, or host-driven rounds in profiling mode) against the oracle's
+    optimisation of the same plans: final objective, DVH indices, iteration counts, exit statuses."""
+    c = custom_case(a)
+    eps = float(a.get("eps", 0.0))
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=c.iters, eps=eps)
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    try:
+        if a.get("profile"):
+            g.gmco_set_profiling(h, True)
+        g.gmco_optimize(h, c.T0, c.weights, c.iters)
+        out = g.gmco_result(h, host=True)
+        st = g.gmco_get_stats(h)
+    finally:
+        g.gmco_destroy(h)
+    rel_f = np.abs(out["objective"] - ref["F"]) / ref["F"]
+    dvh_pp = np.abs(out["dvh"] - ref["dvh"])
+    same_it = out["iters_done"] == ref["iters_done"]
+    return report(E, rel_F_max=float(rel_f.max()), rel_F_same_iters_max=float(rel_f[same_it].max()) if same_it.any() else None,
+                  dvh_pp_max=float(dvh_pp.max()), iters_gpu=out["iters_done"].tolist(), iters_ref=np.asarray(ref["iters_done"]).tolist(),
+                  status_gpu=out["plan_status"].tolist(), status_ref=np.asarray(ref["status"]).tolist(),
+                  rounds=int(st["rounds"]), launches=int(st["kernel_launches"]), dose_kernel=int(st["dose_kernel"]),
+                  digest=digest(out["T"], out["objective"], out["dvh"]),
+                  ls_launches=int(E.emu_counter(b"k_ls_pick")), step_launches=int(E.emu_counter(b"k_step")))
+
+
+def sc_fault(g, E, a):
+    """Fault injection: the n-th TMA completion (or tcgen05.commit) after the handle's creation is lost.  The kernels must
+    run into their bounded waits, leave through the normal teardown, and the ABI must report GMCO_E_CUDA -- no hang."""
+    c = custom_case(a)
+    T = np.repeat(c.T0[None], c.n_plans, axis=0)
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    err, code = "", 0
+    t0 = time.time()
+    try:
+        E.emu_set(a["drop"].encode(), int(a["nth"]))
+        try:
+            if a.get("via", "evaluate") == "evaluate":
+                g.gmco_evaluate(h, T, c.weights, want_dose=False, want_grad=True, host=True)
+            else:
+                g.gmco_optimize(h, c.T0, c.weights, int(a.get("iters", 3)))
+                g.gmco_result(h, host=True)
+        except b.GmcoError as ex:
+            err, code = str(ex), ex.code
+        E.emu_set(a["drop"].encode(), -1)
+        # the handle recovers: the same call succeeds once the fault is gone
+        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
+        ref = oracle.evaluate(c.D, c.structures, T, c.weights)
+    finally:
+        g.gmco_destroy(h)
+    return report(E, error=err, code=code, seconds=time.time() - t0, errors_after=eval_errors(out, ref))
+
+
+def sc_sa(g, E, a):
+    """gSA chains on the fp64 route: the whole trajectory must equal the oracle's (acceptance counts, dwell times)."""
+    c = custom_case(a)
+    K, steps = c.n_plans, int(a.get("steps", 300))
+    jdx, z, u = gc.sa_draws(c.n_dwell, K, steps, seed=5)
+    tau = float(c.T0[0])
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    try:
+        out = g.gmco_sa_run(h, c.T0, c.weights, jdx, z, u, tau, precision=int(a.get("sa_precision", 0)), host=True)
+    finally:
+        g.gmco_destroy(h)
+    acc_ref, t_err, f_err = [], 0.0, 0.0
+    for k in range(K):
+        r = oracle.sa_chain(c.D, c.structures, c.weights[k], c.T0, tau, jdx[k], z[k], u[k])
+        acc_ref.append(int(r["n_accepted"]))
+        t_err = max(t_err, float(np.abs(out["T"][k] - r["t"]).max()))
+        f_err = max(f_err, float(abs(out["objective"][k] - r["F"]) / r["F"]))
+    return report(E, accepted_gpu=out["n_accepted"].tolist(), accepted_ref=acc_ref, T_abs_err=t_err, F_rel_err=f_err)
+
+
+def sc_pool(g, E, a):
+    """Pareto filter and plan selection (comparisons only: bit-exact) and the dose-rate matrix (one fp32 ulp)."""
+    rng = np.random.Generator(np.random.PCG64(11))
+    K, M = int(a.get("K", 300)), 5
+    obj = rng.random((K, M)).astype(np.float32)
+    obj[rng.integers(0, K, 20)] = obj[rng.integers(0, K, 20)]          # exact duplicates
+    c = custom_case(a)
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    try:
+        pf = g.gmco_pareto_front(h, obj)
+        dvh = np.stack([rng.uniform(80, 100, K), rng.uniform(100, 125, K), rng.uniform(0, 3, K), rng.uniform(0, 3, K)], axis=1).astype(np.float32)
+        crit = [(0, +1, 90.0, 95.0, 0), (1, -1, 118.0, 115.0, 1), (2, -1, 1.5, 1.0, 2), (3, -1, 1.5, 1.0, 2)]
+        sel = g.gmco_select_plan(h, dvh, crit)
+    finally:
+        g.gmco_destroy(h)
+    ref_pf = oracle.pareto_front(obj)
+    ref_sel, ref_cls, ref_cnt = oracle.select_plan(dvh, crit)
+    D = g.gmco_dose_rate_matrix(c.points, c.dwell, gc.G_COEF, gc.SK_LAMBDA, gc.R_FLOOR_CM, host=True)
+    Dref = oracle.dose_rate_matrix(c.points, c.dwell, gc.G_COEF, gc.SK_LAMBDA, gc.R_FLOOR_CM)
+    ulp = np.abs(D.view(np.int32).astype(np.int64) - Dref.view(np.int32).astype(np.int64))
+    return report(E, pareto_equal=bool(np.array_equal(pf["nondominated"], ref_pf)), n_nondominated=int(pf["n_nondominated"]),
+                  selected=int(sel["selected"]), selected_ref=int(ref_sel), classes_equal=bool(np.array_equal(sel["plan_class"], ref_cls)),
+                  class_counts_equal=bool(np.array_equal(sel["class_counts"], ref_cnt)),
+                  dose_rate=dict(max_ulp=int(ulp.max()), exact_fraction=float((ulp == 0).mean())))
+
+
+SCENARIOS = {"evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
+
+
+def main():
+    a = json.loads(sys.argv[1])
+    lib = Path(a.get("lib", ROOT / "tests" / "emu" / "_build" / "libgmco_emu.so"))
+    g, E = load(lib)
+    configure(E, a)
+    t0 = time.time()
+    out = SCENARIOS[a["scenario"]](g, E, a)
+    out["seconds"] = out.get("seconds", time.time() - t0)
+    if a.get("times"):
+        E.emu_print_times()
+    print("EMU_RESULT " + json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

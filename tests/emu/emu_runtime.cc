@@ -10,6 +10,7 @@
 #include <stdarg.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <time.h>
 
 #include <deque>
 #include <map>
@@ -45,7 +46,8 @@ static char g_violation_msg[1024];
 static long g_tma_count, g_commit_count, g_mma_count, g_hangs;
 struct LaunchRec { std::string name; dim3 grid, block; size_t smem; int captured; };
 static std::vector<LaunchRec> g_launches;
-static std::map<std::string, long> g_kernel_runs;          // executions (outside capture + graph replays) by kernel name
+static std::map<std::string, long> g_kernel_runs;
+static std::map<std::string, double> g_kernel_secs;      // host seconds spent emulating each kernel          // executions (outside capture + graph replays) by kernel name
 static cudaError_t g_last_error = cudaSuccess, g_sticky = cudaSuccess;
 
 void violation(const char* fmt, ...) {
@@ -784,6 +786,11 @@ static std::map<const void*, int> g_smem_cap;
 static void execute(const LaunchCfg& cfg, const char* name, const std::function<void()>& body) {
   g_kernel_runs[name]++;
   if (g_sticky != cudaSuccess) return;
+  struct Timer {
+    const char* n; timespec t0;
+    explicit Timer(const char* nn) : n(nn) { clock_gettime(CLOCK_MONOTONIC, &t0); }
+    ~Timer() { timespec t1; clock_gettime(CLOCK_MONOTONIC, &t1); g_kernel_secs[n] += (double)(t1.tv_sec - t0.tv_sec) + 1e-9 * (double)(t1.tv_nsec - t0.tv_nsec); }
+  } timer(name);
   const int nthreads = (int)(cfg.block.x * cfg.block.y * cfg.block.z);
   const int cl = cfg.cluster_x;
   static uint64_t launch_seq = 0;
@@ -1023,7 +1030,7 @@ cudaError_t cudaGetDriverEntryPoint(const char* name, void** fn, unsigned long l
 #pragma GCC visibility push(default)
 int emu_violations(void) { return g_violations; }
 const char* emu_violation_message(void) { return g_violation_msg; }
-void emu_clear(void) { g_violations = 0; g_violation_msg[0] = 0; g_launches.clear(); g_kernel_runs.clear(); g_sticky = cudaSuccess; g_last_error = cudaSuccess; g_hangs = 0; }
+void emu_clear(void) { g_violations = 0; g_violation_msg[0] = 0; g_launches.clear(); g_kernel_runs.clear(); g_kernel_secs.clear(); g_sticky = cudaSuccess; g_last_error = cudaSuccess; g_hangs = 0; }
 int emu_live_allocations(void) { int n = 0; for (const Alloc& a : g_allocs) n += a.p != nullptr; return n; }
 long emu_counter(const char* what) {
   const std::string w(what);
@@ -1049,6 +1056,9 @@ int emu_set(const char* key, long v) {
   else if (k == "verbose") g_cfg.verbose = (int)v;
   else return -1;
   return 0;
+}
+void emu_print_times(void) {
+  for (const auto& kv : g_kernel_secs) fprintf(stderr, "[emu] %8.3f s  %6ld x  %s\n", kv.second, g_kernel_runs[kv.first], kv.first.c_str());
 }
 int emu_launch(int i, char* name, int cap, unsigned* dims, unsigned long long* smem, int* captured) {
   if (i < 0 || (size_t)i >= g_launches.size()) return -1;
