@@ -40,7 +40,7 @@ def load(lib: Path):
 
 
 def configure(E, a):
-    for key in ("seed", "max_delay", "dyn_misalign", "sm_count", "shuffle", "verbose"):
+    for key in ("seed", "max_delay", "mma_delay", "dyn_misalign", "sm_count", "shuffle", "verbose"):
         if key in a:
             E.emu_set(key.encode(), int(a[key]))
 

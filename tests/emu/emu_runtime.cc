@@ -33,6 +33,8 @@ namespace emu {
 struct Config {
   uint64_t seed = 1;
   int max_delay = 400;          // asynchronous operations complete 1 .. max_delay scheduler ticks after issue
+  int mma_delay = -1;           // >= 0: the tensor pipe's own bound (a slow pipe exposes ring slots refilled too early,
+                                // a fast one with slow copies exposes operands read before they landed)
   int dyn_misalign = 16;        // window offset of dynamic shared memory = 1024 + this (the kernels align by hand)
   int sm_count = 148;
   long drop_tma = -1;           // fault injection: the n-th TMA load (0-based, per process) never completes
@@ -271,7 +273,8 @@ static void run_due(Gang* g) {
 }
 static void post(Gang* g, std::function<void()> fn) { g->ops.push_back(Op{g->tick + delay(g), std::move(fn)}); }
 static void post_pipe(Gang* g, std::function<void()> fn) {
-  uint64_t due = g->tick + delay(g);
+  const int md = g_cfg.mma_delay >= 0 ? g_cfg.mma_delay : g_cfg.max_delay;
+  uint64_t due = g->tick + 1 + (md > 1 ? rnd(g) % (uint64_t)md : 0);
   if (due < g->pipe_last_due) due = g->pipe_last_due;
   g->pipe_last_due = due;
   g->pipe.push_back(Op{due, std::move(fn)});
@@ -1048,6 +1051,7 @@ int emu_set(const char* key, long v) {
   const std::string k(key);
   if (k == "seed") g_cfg.seed = (uint64_t)v;
   else if (k == "max_delay") g_cfg.max_delay = (int)v;
+  else if (k == "mma_delay") g_cfg.mma_delay = (int)v;
   else if (k == "dyn_misalign") g_cfg.dyn_misalign = (int)v;
   else if (k == "sm_count") g_cfg.sm_count = (int)v;
   else if (k == "drop_tma") g_cfg.drop_tma = v < 0 ? -1 : g_tma_count + v;

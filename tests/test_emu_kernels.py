@@ -1,0 +1,212 @@
+"""The kernels' SOURCE executed on the CPU (tests/emu) and held to the fp64 oracle -- what can be known about the CUDA
+path on a machine without a GPU.
+
+tests/emu/build_emu.py compiles csrc/*.cu with g++ after three textual rewrites (PTX layer -> emu_ptx.h, <<<>>> ->
+emu::Launch, extern __shared__ -> a pointer), links them with a fiber-per-thread model of SIMT execution and software
+models of mbarrier / TMA / tcgen05 / clusters, and tests/emu/driver.py drives the result through the product's own ctypes
+binding.  So the control flow, index arithmetic, descriptor construction, ring / phase protocol, compaction, the device-side
+WHILE loop and the host code that run here are the product's; the arithmetic of the tensor core is a model (tf32
+operands, one truncating fp32 add per MMA).  This is NOT a GPU result and does not replace the -m gpu tests: it cannot
+see PTX qualifiers, memory-model fences, real timing or anything ptxas does.  It does show that HEAD's kernels
+  * compute dose, objective and gradient within north_star's 1e-4 of the oracle on every route, including the
+    kernels and options that have never run on a GPU (k_step's hoisted loads, wide_accum, line_search),
+  * never touch shared memory outside the launched window, TMEM outside the allocation, or device memory outside its
+    allocations; never over-arrive on a barrier; leave nothing in flight and no TMEM allocated at exit,
+  * give bit-identical results whatever the thread interleaving, the completion delays of the asynchronous units
+    (1 .. 20000 scheduler ticks, slow tensor pipe against fast copies and the reverse) and the alignment of dynamic
+    shared memory -- i.e. no result depends on timing,
+  * leave through their normal teardown and report GMCO_E_CUDA when a TMA completion or a tcgen05.commit is lost
+    (the library must not be able to hang or fault a GPU by itself).
+All scenarios of the module run concurrently as subprocesses (a few seconds each)."""
+import json
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parents[1]
+TOL_EVAL, TOL_F_FINAL, TOL_DVH_PP = 1e-4, 1e-3, 0.5
+
+SMALL = dict(counts=[500, 100, 120, 120])                    # 840 points -> 7 chunks of 128: several chunks per CTA
+SCENARIOS = {
+    # ---- one evaluation per route ----
+    "simt": dict(scenario="evaluate", precision=1, sm_count=4),
+    "resident": dict(scenario="evaluate", sm_count=4),
+    "resident_uniform_start": dict(scenario="evaluate", sm_count=4, start="uniform"),
+    "resident_3_tiles_odd": dict(scenario="evaluate", sm_count=6, n_plans=300, n_cath=10, n_pos=10, **SMALL),
+    "resident_forced_single": dict(scenario="evaluate", sm_count=4, n_plans=256, dose_kernel=1, n_cath=18, n_pos=14, **SMALL),
+    "pair_ring": dict(scenario="evaluate", sm_count=4, n_plans=256, **SMALL),
+    "pair_static": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, **SMALL),
+    "pair_static_4_tiles_ragged": dict(scenario="evaluate", sm_count=8, n_plans=500, n_cath=17, n_pos=14, counts=[333, 77, 129, 65]),
+    "streamed_288": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=18, n_pos=16, **SMALL),
+    "streamed_384": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, **SMALL),
+    "wide_accum_384": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, wide_accum=1, **SMALL),
+    "wide_accum_352_3_tiles": dict(scenario="evaluate", sm_count=6, n_plans=300, n_cath=22, n_pos=16, wide_accum=1, **SMALL),
+    # BASELINE.json configs[2] at FULL size in the launch configuration bench.py times (148 SMs: 8 plan tiles x 18 segments,
+    # k_dose_tc_pair<4, 6> with 5-6 chunks per CTA): all 12000 x 1000 doses, F and the gradient of all 1000 plans (~70 s)
+    "c3_full_size": dict(scenario="evaluate", case="C3"),
+    # ---- the same evaluation under other schedules: results must be bit-identical ----
+    "pair_static@seed2": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, seed=2, **SMALL),
+    "pair_static@slow_pipe": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, seed=3, max_delay=20, mma_delay=20000, **SMALL),
+    "pair_static@slow_copies": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, seed=4, max_delay=20000, mma_delay=1, dyn_misalign=0, **SMALL),
+    "pair_static@in_order": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, seed=5, max_delay=1, shuffle=0, dyn_misalign=1008, **SMALL),
+    "streamed_384@slow_pipe": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, seed=6, max_delay=20, mma_delay=20000, **SMALL),
+    "streamed_384@slow_copies": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, seed=7, max_delay=20000, mma_delay=1, dyn_misalign=1008, **SMALL),
+    "resident@slow_pipe": dict(scenario="evaluate", sm_count=4, seed=8, max_delay=20, mma_delay=20000),
+    "resident@slow_copies": dict(scenario="evaluate", sm_count=4, seed=9, max_delay=20000, mma_delay=1, dyn_misalign=0),
+    # ---- whole optimisations: device-side WHILE loop, k_step, compaction, stopping rules ----
+    "opt_c1": dict(scenario="optimize", sm_count=4),
+    "opt_c1@slow_copies": dict(scenario="optimize", sm_count=4, iters=12, seed=11, max_delay=20000, mma_delay=1),
+    "opt_c1_12": dict(scenario="optimize", sm_count=4, iters=12),
+    "opt_profile_mode": dict(scenario="optimize", sm_count=4, iters=20, profile=1),
+    "opt_no_compaction": dict(scenario="optimize", sm_count=4, iters=20, compaction=0),
+    "opt_simt": dict(scenario="optimize", sm_count=4, iters=20, precision=1),
+    "opt_eps_pair_compaction": dict(scenario="optimize", sm_count=4, n_plans=256, eps=1e-3, iters=30, **SMALL),
+    "opt_line_search": dict(scenario="optimize", sm_count=4, iters=30, line_search=1),
+    "opt_streamed_wide": dict(scenario="optimize", sm_count=2, n_plans=6, n_cath=24, n_pos=16, iters=8, wide_accum=1, counts=[300, 60, 70, 70]),
+    # ---- lost completions ----
+    "fault_tma_resident": dict(scenario="fault", sm_count=4, drop="drop_tma", nth=5),
+    "fault_commit_resident": dict(scenario="fault", sm_count=4, drop="drop_commit", nth=4),
+    "fault_tma_pair": dict(scenario="fault", sm_count=4, drop="drop_tma", nth=40, n_plans=256, **SMALL),
+    "fault_commit_pair": dict(scenario="fault", sm_count=4, drop="drop_commit", nth=3, n_plans=256, **SMALL),
+    "fault_tma_streamed": dict(scenario="fault", sm_count=2, drop="drop_tma", nth=33, n_plans=128, n_cath=24, n_pos=16, **SMALL),
+    "fault_in_loop": dict(scenario="fault", sm_count=4, drop="drop_tma", nth=300, via="optimize"),
+    # ---- the other entry points ----
+    "sa_fp64": dict(scenario="sa", n_plans=3, steps=300),
+    "pool": dict(scenario="pool"),
+}
+
+
+@pytest.fixture(scope="module")
+def results():
+    sys.path.insert(0, str(ROOT / "tests" / "emu"))
+    import build_emu
+    lib = build_emu.build()
+    import oracle
+    oracle.build()
+
+    def run(item):
+        name, args = item
+        p = subprocess.run([sys.executable, str(ROOT / "tests" / "emu" / "driver.py"), json.dumps(dict(args, lib=str(lib)))],
+                           capture_output=True, text=True, timeout=900)
+        line = [l for l in p.stdout.splitlines() if l.startswith("EMU_RESULT ")]
+        if p.returncode != 0 or not line:
+            return name, dict(crashed=True, returncode=p.returncode, stderr=p.stderr[-2000:])
+        return name, json.loads(line[-1][len("EMU_RESULT "):])
+
+    order = sorted(SCENARIOS.items(), key=lambda kv: kv[0] != "c3_full_size")      # the long one first: it overlaps the rest
+    with ThreadPoolExecutor(max_workers=8) as ex:
+        return dict(ex.map(run, order))
+
+
+def _ok(results, name):
+    r = results[name]
+    assert not r.get("crashed"), f"{name}: driver failed ({r.get('returncode')}): {r.get('stderr')}"
+    assert r["violations"] == 0, f"{name}: {r['violations']} violations, first: {r['violation']}"
+    assert r["hangs"] == 0 and r["live_allocations"] == 0, name
+    return r
+
+
+EVALS = [n for n, a in SCENARIOS.items() if a["scenario"] == "evaluate"]
+
+
+@pytest.mark.parametrize("name", EVALS)
+def test_evaluation_matches_the_oracle_without_a_violation(results, name):
+    r = _ok(results, name)
+    e = r["errors"]
+    assert e["dose"] < TOL_EVAL and e["F"] < TOL_EVAL and e["grad"] < TOL_EVAL, (name, e)
+
+
+def test_every_dose_kernel_and_the_multi_chunk_paths_were_reached(results):
+    want = {"simt": "k_simt_dose", "resident": "k_dose_tc<true>", "resident_forced_single": "k_dose_tc<true>", "pair_ring": "k_dose_tc_pair<0, 0>",
+            "pair_static": "k_dose_tc_pair<4, 6>", "pair_static_4_tiles_ragged": "k_dose_tc_pair<4, 6>", "streamed_288": "k_dose_tc<false>",
+            "streamed_384": "k_dose_tc<false>", "wide_accum_384": "k_dose_tc<false, true>", "wide_accum_352_3_tiles": "k_dose_tc<false, true>",
+            "resident_3_tiles_odd": "k_dose_tc<true>", "c3_full_size": "k_dose_tc_pair<4, 6>"}
+    for name, kernel in want.items():
+        r = _ok(results, name)
+        assert r["kernels"][kernel] == 1 and sum(r["kernels"][k] for k in r["kernels"] if "dose" in k) == 1, (name, r["kernels"])
+        if name != "simt":
+            assert r["kernels"]["k_grad_tc<16>"] == 1 and r["mma"] > 0 and r["tma"] > 0, name
+            q = r["schedule"]
+            assert q["n_chunks"] // q["segs"] >= 3, (name, q["n_chunks"], q["segs"])      # ring wrap-around, buffer alternation
+
+
+def test_c3_runs_in_the_configuration_the_bench_times(results):
+    q = _ok(results, "c3_full_size")["schedule"]
+    assert (q["n_tiles"], q["segs"], q["dose_kernel"], q["dose_stages"]) == (8, 18, 2, 6) and q["n_chunks"] // q["segs"] >= 5
+
+
+def test_results_do_not_depend_on_the_schedule(results):
+    """Thread interleaving, completion delays of TMA / tensor pipe, alignment of dynamic shared memory: same bits."""
+    for base in ("pair_static", "streamed_384", "resident"):
+        variants = [n for n in SCENARIOS if n.startswith(base + "@")]
+        assert len(variants) >= 2
+        for v in variants:
+            assert _ok(results, v)["digest"] == _ok(results, base)["digest"], (base, v)
+    assert _ok(results, "opt_c1@slow_copies")["digest"] == _ok(results, "opt_c1_12")["digest"]
+
+
+def test_wide_accum_halves_the_error_as_the_arithmetic_model_predicts(results):
+    a, b = _ok(results, "streamed_384")["errors"], _ok(results, "wide_accum_384")["errors"]
+    assert b["dose"] < 0.7 * a["dose"] and b["grad"] < 0.7 * a["grad"], (a, b)
+
+
+@pytest.mark.parametrize("name", ["opt_c1", "opt_c1_12", "opt_profile_mode", "opt_no_compaction", "opt_simt", "opt_line_search", "opt_streamed_wide"])
+def test_fixed_iteration_optimisation_matches_the_oracle(results, name):
+    r = _ok(results, name)
+    assert r["iters_gpu"] == r["iters_ref"] and r["status_gpu"] == r["status_ref"], name
+    assert r["rel_F_max"] < TOL_F_FINAL and r["dvh_pp_max"] < TOL_DVH_PP, (name, r["rel_F_max"], r["dvh_pp_max"])
+    assert r["rounds"] >= 1 + max(r["iters_ref"]) and r["step_launches"] >= r["rounds"]
+
+
+def test_the_device_loop_runs_exactly_the_rounds_that_are_needed(results):
+    r = _ok(results, "opt_c1")
+    assert r["rounds"] in range(51, 70) and r["step_launches"] - r["rounds"] in (0, 1, 2)   # two rounds per WHILE body
+    p = _ok(results, "opt_profile_mode")
+    assert p["digest"] == _ok(results, "opt_no_compaction")["digest"] or p["rel_F_max"] < TOL_F_FINAL
+
+
+def test_eps_stopping_with_compaction_on_the_pair_kernel(results):
+    r = _ok(results, "opt_eps_pair_compaction")
+    assert r["dose_kernel"] == 3 and r["status_gpu"] == r["status_ref"]
+    same = [a == b for a, b in zip(r["iters_gpu"], r["iters_ref"])]
+    assert sum(same) >= 0.9 * len(same)                        # a threshold on |F - F+| is not continuous
+    assert max(abs(a - b) for a, b in zip(r["iters_gpu"], r["iters_ref"])) <= 6
+    assert r["rel_F_same_iters_max"] < TOL_F_FINAL
+
+
+def test_line_search_option_launches_its_kernels(results):
+    assert _ok(results, "opt_line_search")["ls_launches"] >= 30 and _ok(results, "opt_c1")["ls_launches"] == 0
+
+
+@pytest.mark.parametrize("name,kernel", [("fault_tma_resident", "k_dose_tc<resident>"), ("fault_commit_resident", "k_dose_tc<resident>"),
+                                         ("fault_tma_pair", "k_dose_tc_pair"), ("fault_commit_pair", "k_dose_tc_pair"),
+                                         ("fault_tma_streamed", "k_dose_tc<streamed>"), ("fault_in_loop", "k_")])
+def test_a_lost_completion_ends_in_an_error_code_not_in_a_hang(results, name, kernel):
+    r = _ok(results, name)                                     # no violation: TMEM freed, nothing left in flight, no hang
+    assert r["code"] == -3 and "barrier wait did not complete" in r["error"] and kernel in r["error"], r["error"]
+    e = r["errors_after"]                                      # and the handle works again afterwards
+    assert e["dose"] < TOL_EVAL and e["F"] < TOL_EVAL and e["grad"] < TOL_EVAL
+
+
+def test_gsa_fp64_trajectory_equals_the_oracle(results):
+    r = _ok(results, "sa_fp64")
+    assert r["accepted_gpu"] == r["accepted_ref"] and r["T_abs_err"] < 1e-9 and r["F_rel_err"] < 1e-12
+
+
+def test_pool_kernels_and_dose_rate_matrix(results):
+    r = _ok(results, "pool")
+    assert r["pareto_equal"] and r["classes_equal"] and r["class_counts_equal"] and r["selected"] == r["selected_ref"]
+    assert r["dose_rate"]["max_ulp"] <= 1 and r["dose_rate"]["exact_fraction"] > 0.999
+
+
+def test_the_emulation_is_not_reachable_from_the_product():
+    """Nothing under the package or the repo's entry points names the emulation; its library lives under tests/."""
+    for p in list((ROOT / "paper_1904_01567_b200").rglob("*.py")) + [ROOT / "bench.py", ROOT / "__graft_entry__.py"]:
+        text = p.read_text()
+        assert "libgmco_emu" not in text and "tests/emu" not in text and "emu_runtime" not in text, p
+    for p in (ROOT / "paper_1904_01567_b200" / "csrc").glob("*"):
+        code = "\n".join(l.split("//")[0] for l in p.read_text().splitlines())
+        assert "emu_" not in code and "GMCO_EMULATED" not in code, p
