@@ -83,11 +83,17 @@ __device__ __noinline__ bool mbar_wait_slow(uint32_t bar, uint32_t parity, int c
     }
   }
 }
+// The verdict is WARP-UNIFORM (a vote): every role that waits here is a whole warp in uniform control flow and goes on
+// to warp-synchronous operations (elect.sync, tcgen05.ld / st .sync.aligned, __syncwarp).  Without the vote a lane that
+// gave up (abort flag seen) could leave the role while a lane whose last poll still succeeded went on to wait for the
+// full warp in such an operation for ever -- found by the CPU emulation of the kernels with a planted protocol error
+// (tests/test_emu_mutants.py); the abort path must itself be unable to hang.
 __device__ __forceinline__ bool mbar_wait_addr(const Watch& w, uint32_t bar, uint32_t parity, int site) {
+  bool ok = false;
 #pragma unroll 1
-  for (int i = 0; i < kFastSpins; ++i)
-    if (mbar_try_wait_addr(bar, parity)) return true;
-  return mbar_wait_slow(bar, parity, 0, w.err, w.abort_addr, (w.kernel << 8) | site);
+  for (int i = 0; i < kFastSpins && !ok; ++i) ok = mbar_try_wait_addr(bar, parity);
+  if (!ok) ok = mbar_wait_slow(bar, parity, 0, w.err, w.abort_addr, (w.kernel << 8) | site);
+  return __all_sync(0xffffffffu, ok) != 0;
 }
 __device__ __forceinline__ bool mbar_wait(const Watch& w, uint64_t* bar, uint32_t parity, int site) {
   return mbar_wait_addr(w, smem_u32(bar), parity, site);
@@ -95,10 +101,11 @@ __device__ __forceinline__ bool mbar_wait(const Watch& w, uint64_t* bar, uint32_
 // a barrier of this CTA on which threads of the peer CTA arrive (shared::cluster arrivals)
 __device__ __forceinline__ bool mbar_wait_cluster(const Watch& w, uint64_t* bar, uint32_t parity, int site) {
   const uint32_t b = smem_u32(bar);
+  bool ok = false;
 #pragma unroll 1
-  for (int i = 0; i < kFastSpins; ++i)
-    if (mbar_try_wait_cluster_addr(b, parity)) return true;
-  return mbar_wait_slow(b, parity, 1, w.err, w.abort_addr, (w.kernel << 8) | site);
+  for (int i = 0; i < kFastSpins && !ok; ++i) ok = mbar_try_wait_cluster_addr(b, parity);
+  if (!ok) ok = mbar_wait_slow(b, parity, 1, w.err, w.abort_addr, (w.kernel << 8) | site);
+  return __all_sync(0xffffffffu, ok) != 0;       // warp-uniform, see mbar_wait_addr
 }
 // inside a role's lambda: give the role up when the wait was abandoned
 #define GMCO_WAIT(call) do { if (!(call)) return; } while (0)

@@ -91,5 +91,89 @@ def build(force: bool = False, sanitize: bool = False) -> Path:
     return lib
 
 
+# ---- mutants: the emulation must notice planted protocol and indexing errors (tests/test_emu_mutants.py) ----------------
+# name -> (file, text to find, replacement, occurrences expected)
+MUTANTS = {
+    # producer refills a ring slot without waiting for the commit of the MMAs that read it
+    "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));", "", 3),
+    # MMAs issued before the TMA bytes of their operands have landed
+    "issuer_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));", "", 2),
+    # gradient MMAs issued before the converter warps have split the R tile (and before it has landed)
+    "grad_issuer_skips_conv_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));", "", 1),
+    # epilogue reads the accumulator without waiting for the chunk's last commit
+    "epilogue_skips_acc_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, acc_full + b, use & 1, DEVERR_W_ACC_FULL));", "", 2),
+    # issuer overwrites the accumulator without waiting for the epilogue to hand it back
+    "issuer_skips_acc_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));", "", 1),
+    # the epilogue hands the accumulator back before it has read it
+    "accumulator_handed_back_too_early": ("kernels_tc.cu", "        tmem_ld32(t_main, v[0]);\n        tmem_ld32(t_main + 32, v[1]);\n        if (a.sep_corr) {",
+                                          "        mbar_arrive(acc_empty + b);\n        tmem_ld32(t_main, v[0]);\n        tmem_ld32(t_main + 32, v[1]);\n        if (a.sep_corr) {", 1),
+    # the host launches 4 KB less dynamic shared memory than the kernel's carve-up needs (caught by the kernel's self-check)
+    "host_smem_too_small": ("tc_layout.h", "t.dose_smem = fixed + t.dose_stages * probe.stage_bytes;", "t.dose_smem = fixed + t.dose_stages * probe.stage_bytes - 4096;", 1),
+    # ... and the same with the self-check gone: the emulated hardware's window check is what is left
+    "host_smem_too_small_unchecked": ("*", None, None, 0),
+    # producer's ring phase never flips: the second trip round the ring waits for ever -> bounded wait -> error word
+    "producer_phase_never_flips": ("kernels_tc.cu", "if (++st == a.n_stage) { st = 0; ph ^= 1; }", "if (++st == a.n_stage) { st = 0; }", 4),
+    # TMEM is never given back
+    "tmem_never_freed": ("kernels_tc.cu", "tc_fence_after(); tmem_dealloc(tmem, 512); }", "tc_fence_after(); }", 2),
+    # the D slab of the wrong chunk is loaded (index error: wrong numbers, nothing else)
+    "wrong_chunk_loaded": ("kernels_tc.cu", "tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, c * kPC, g, polD);", "tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, (c + (c & 1)) * kPC, g, polD);", 1),
+    # a K-step of the main product uses the wrong 32 B of the swizzled row
+    "wrong_k_step_descriptor": ("kernels_tc.cu", "mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);", "mma_ts2(acc, thi + 8 * j, bd + 2 * (j ^ 1), dhi, idesc, 1);", 1),
+    # k_step pushes the history pair without waiting for the staged copies it overwrites
+    "step_skips_history_wait": ("kernels_lbfgs.cu", "      hist_wait();                                           // the staged copy of slot hh is about to be replaced\n", "", 1),
+}
+
+
+def build_mutant(name: str) -> Path:
+    """libgmco_emu with one planted error.  Only the mutated translation units are recompiled."""
+    plain = build()
+    lib = OUT / f"libgmco_emu_mut_{name}.so"
+    if lib.exists() and lib.stat().st_mtime >= plain.stat().st_mtime and lib.stat().st_mtime >= Path(__file__).stat().st_mtime:
+        return lib
+    gen = OUT / "gen" / f"mut_{name}"
+    gen.mkdir(parents=True, exist_ok=True)
+    edits = []
+    if name == "host_smem_too_small_unchecked":
+        edits = [MUTANTS["host_smem_too_small"][:4],
+                 ("kernels_tc.cu", "const bool smem_ok = pad + (uint32_t)smem_end <= dynamic_smem_size(), tmem_ok", "const bool smem_ok = true, tmem_ok", 1)]
+    else:
+        edits = [MUTANTS[name]]
+    texts = {}
+    for fname, old, new, count in edits:
+        text = texts.get(fname) or (CSRC / fname).read_text()
+        assert text.count(old) == count, f"mutant {name}: expected {count} occurrences of the target in {fname}, found {text.count(old)}"
+        texts[fname] = text.replace(old, new)
+    # a mutated header reaches every translation unit that includes it: put it first on the include path
+    flags = ["-std=c++17", "-O2", "-g", "-fPIC", "-mfma", "-mavx2", "-fvisibility=hidden", "-w",
+             "-I", str(gen), "-I", str(HERE), "-I", str(CSRC), "-I", str(ROOT / "include"), "-I", str(CUDA_INC), "-DGMCO_EMULATED=1"]
+    headers = [f for f in texts if not f.endswith(".cu")]
+    for f in headers:
+        (gen / f).write_text(texts[f])
+    redo = [s for s in sorted(CSRC.glob("*.cu")) if s.name in texts or (headers and any(f'"{h}"' in s.read_text() for h in headers))]
+    objs, procs = [], []
+    for src in sorted(CSRC.glob("*.cu")):
+        if src in redo:
+            cc = gen / (src.stem + ".cc")
+            text = texts.get(src.name) or src.read_text()
+            if headers:                                   # quote-includes look beside the including file first: the copy is in gen
+                pass
+            cc.write_text(transform(text))
+            obj = gen / f"{src.stem}.o"
+            procs.append(subprocess.Popen(["g++", *flags, "-c", str(cc), "-o", str(obj)], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+            objs.append(str(obj))
+        else:
+            objs.append(str(OUT / "gen" / f"{src.stem}.plain.o"))
+    objs.append(str(OUT / "gen" / "emu_runtime.plain.o"))
+    for p in procs:
+        out, _ = p.communicate()
+        if p.returncode:
+            raise RuntimeError(f"mutant {name} does not compile:\n{out[-3000:]}")
+    subprocess.run(["g++", "-shared", "-o", str(lib), *objs], check=True)
+    return lib
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, sanitize="--asan" in sys.argv))
+    if len(sys.argv) > 2 and sys.argv[1] == "--mutant":
+        print(build_mutant(sys.argv[2]))
+    else:
+        print(build(force="--force" in sys.argv, sanitize="--asan" in sys.argv))

@@ -40,7 +40,7 @@ def load(lib: Path):
 
 
 def configure(E, a):
-    for key in ("seed", "max_delay", "mma_delay", "dyn_misalign", "sm_count", "shuffle", "verbose"):
+    for key in ("seed", "max_delay", "mma_delay", "dyn_misalign", "sm_count", "shuffle", "verbose", "starve_mask", "starve_period"):
         if key in a:
             E.emu_set(key.encode(), int(a[key]))
 
@@ -148,11 +148,13 @@ def sc_fault(g, E, a):
             err, code = str(ex), ex.code
         E.emu_set(a["drop"].encode(), -1)
         # the handle recovers: the same call succeeds once the fault is gone
-        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
-        ref = oracle.evaluate(c.D, c.structures, T, c.weights)
+        after = None
+        if not a.get("no_recovery"):
+            out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
+            after = eval_errors(out, oracle.evaluate(c.D, c.structures, T, c.weights))
     finally:
         g.gmco_destroy(h)
-    return report(E, error=err, code=code, seconds=time.time() - t0, errors_after=eval_errors(out, ref))
+    return report(E, error=err, code=code, seconds=time.time() - t0, errors_after=after)
 
 
 def sc_sa(g, E, a):
@@ -210,7 +212,10 @@ def main():
     g, E = load(lib)
     configure(E, a)
     t0 = time.time()
-    out = SCENARIOS[a["scenario"]](g, E, a)
+    try:
+        out = SCENARIOS[a["scenario"]](g, E, a)
+    except b.GmcoError as ex:                  # a scenario that does not expect an error: report it instead of dying
+        out = report(E, error=str(ex), code=ex.code)
     out["seconds"] = out.get("seconds", time.time() - t0)
     if a.get("times"):
         E.emu_print_times()

@@ -20,6 +20,7 @@
 #include <vector>
 
 #if defined(__SANITIZE_ADDRESS__)
+#include <sanitizer/asan_interface.h>
 #include <sanitizer/common_interface_defs.h>
 #define EMU_ASAN 1
 #else
@@ -40,6 +41,8 @@ struct Config {
   long drop_tma = -1;           // fault injection: the n-th TMA load (0-based, per process) never completes
   long drop_commit = -1;        // fault injection: the n-th tcgen05.commit never arrives
   int shuffle = 1;              // randomise the order in which the fibers of a CTA are resumed
+  unsigned starve_mask = 0;     // warps (bit = warp index) that only get a turn every starve_period-th round: a slow
+  int starve_period = 1;        // producer, issuer or epilogue must change nothing but the time it takes
   int verbose = 0;
 };
 static Config g_cfg;
@@ -111,6 +114,8 @@ struct Fiber {
   bool done = false;
   ThreadCtx ctx{};
   int bulk_pending = 0;         // bulk stores of this thread whose shared-memory source has not been read yet
+  const char* where = "running"; // what the thread last blocked on (reported when a CTA hangs)
+  uint32_t where_arg = 0;
   Gang* gang = nullptr;
 };
 thread_local ThreadCtx* g_cur = nullptr;
@@ -156,7 +161,12 @@ struct Cta {
   Gang* gang = nullptr;
 };
 
-struct Op { uint64_t due; std::function<void()> fn; };
+// What an operation in flight will touch, for the hazard checks made when OTHER operations are issued: a correct kernel
+// orders them through its barriers, so an overlap found at issue time is a protocol error whatever the timing.
+struct Range { const Cta* cta; uint32_t lo, hi; };             // shared-memory window addresses [lo, hi) of one CTA
+struct Cols { const Cta* cta; uint32_t lo, hi; };              // TMEM columns [lo, hi) of one CTA (all 128 lanes)
+struct Touch { std::vector<Range> smem_w, smem_r; std::vector<Cols> tmem_w, tmem_r; };
+struct Op { uint64_t due; std::function<void()> fn; Touch touch; };
 
 struct Gang {
   std::vector<std::unique_ptr<Cta>> ctas;
@@ -271,14 +281,53 @@ static void run_due(Gang* g) {
     fn(); g->progress++;
   }
 }
-static void post(Gang* g, std::function<void()> fn) { g->ops.push_back(Op{g->tick + delay(g), std::move(fn)}); }
-static void post_pipe(Gang* g, std::function<void()> fn) {
+static void post(Gang* g, std::function<void()> fn, Touch touch = Touch()) { g->ops.push_back(Op{g->tick + delay(g), std::move(fn), std::move(touch)}); }
+static void post_pipe(Gang* g, std::function<void()> fn, Touch touch = Touch()) {
   const int md = g_cfg.mma_delay >= 0 ? g_cfg.mma_delay : g_cfg.max_delay;
   uint64_t due = g->tick + 1 + (md > 1 ? rnd(g) % (uint64_t)md : 0);
   if (due < g->pipe_last_due) due = g->pipe_last_due;
   g->pipe_last_due = due;
-  g->pipe.push_back(Op{due, std::move(fn)});
+  g->pipe.push_back(Op{due, std::move(fn), std::move(touch)});
 }
+
+static bool overlaps(const std::vector<Range>& a, const Cta* c, uint32_t lo, uint32_t hi) {
+  for (const Range& r : a) if (r.cta == c && r.lo < hi && lo < r.hi) return true;
+  return false;
+}
+static bool overlaps(const std::vector<Cols>& a, const Cta* c, uint32_t lo, uint32_t hi) {
+  for (const Cols& r : a) if (r.cta == c && r.lo < hi && lo < r.hi) return true;
+  return false;
+}
+// an asynchronous WRITE of shared memory [lo, hi) is being issued: nothing in flight may still read or write it
+static void check_smem_write_issue(Gang* g, const Cta* c, uint32_t lo, uint32_t hi, const char* what) {
+  for (const Op& o : g->pipe)
+    if (overlaps(o.touch.smem_r, c, lo, hi)) { violation("%s: %s into shared memory [0x%x, 0x%x) while MMAs that read it are still in flight (slot refilled before its consumer's commit)", g->kernel, what, lo, hi); return; }
+  for (const Op& o : g->ops)
+    if (overlaps(o.touch.smem_w, c, lo, hi)) { violation("%s: %s into shared memory [0x%x, 0x%x) while another copy into it is still in flight", g->kernel, what, lo, hi); return; }
+}
+// an MMA that READS shared memory [lo, hi) is being issued: every copy into it must have landed
+static void check_smem_read_issue(Gang* g, const Cta* c, uint32_t lo, uint32_t hi, const char* what) {
+  for (const Op& o : g->ops)
+    if (overlaps(o.touch.smem_w, c, lo, hi)) { violation("%s: %s reads shared memory [0x%x, 0x%x) while a copy into it is still in flight (issued before the full barrier)", g->kernel, what, lo, hi); return; }
+}
+// a thread reads / writes TMEM columns: no MMA in flight may write (read: or read) them
+static void check_tmem_thread_access(Gang* g, const Cta* c, uint32_t lo, uint32_t hi, bool write, const char* what) {
+  for (const Op& o : g->pipe) {
+    if (overlaps(o.touch.tmem_w, c, lo, hi)) { violation("%s: %s of TMEM columns [%u, %u) while MMAs that write them are in flight (accumulator touched before its commit arrived)", g->kernel, what, lo, hi); return; }
+    if (write && overlaps(o.touch.tmem_r, c, lo, hi)) { violation("%s: %s of TMEM columns [%u, %u) while MMAs that read them as an operand are in flight", g->kernel, what, lo, hi); return; }
+  }
+}
+#if EMU_ASAN
+// while a copy into shared memory is in flight the kernel's own loads and stores must stay away from its destination
+static void asan_guard(Cta* c, uint32_t addr, size_t bytes, bool on) {
+  const uint32_t off = addr & 0xffffffu;
+  if (off < c->dyn_base || (size_t)off + bytes > (size_t)c->dyn_base + c->dyn_bytes) return;
+  if (on) __asan_poison_memory_region(c->dyn + (off - c->dyn_base), bytes);
+  else __asan_unpoison_memory_region(c->dyn + (off - c->dyn_base), bytes);
+}
+#else
+static void asan_guard(Cta*, uint32_t, size_t, bool) {}
+#endif
 
 unsigned long long virtual_ns() { return g_gang ? 1000000ull + g_gang->tick * 20ull + g_gang->vtime_jump : 0ull; }
 void sleep_ns(unsigned ns) {
@@ -292,6 +341,7 @@ static void run_gang(Gang* g) {
   std::vector<Fiber*> order;
   for (auto& f : g->fibers) order.push_back(f.get());
   long stagnant = 0;
+  uint64_t round = 0;
   while (g->live > 0) {
     const uint64_t p0 = g->progress;
     if (g_cfg.shuffle && order.size() > 1) {
@@ -300,13 +350,16 @@ static void run_gang(Gang* g) {
       std::rotate(order.begin(), order.begin() + (long)r, order.end());
       for (int i = 0; i < 4; ++i) std::swap(order[rnd(g) % order.size()], order[rnd(g) % order.size()]);
     }
+    const bool full_round = g_cfg.starve_period <= 1 || (++round % (uint64_t)g_cfg.starve_period) == 0;
     for (Fiber* f : order) {
       if (f->done) continue;
+      if (!full_round && ((g_cfg.starve_mask >> (f->ctx.warp & 31)) & 1u)) continue;
       resume(f);
       g->tick++;
       run_due(g);
     }
     if (g->progress != p0) { stagnant = 0; continue; }
+    if (!full_round) continue;                      // only a round in which every thread had its turn can show a standstill
     if (!g->ops.empty() || !g->pipe.empty()) {      // everybody waits for a hardware unit: let its time come
       uint64_t next = ~0ull;
       for (const Op& o : g->ops) next = std::min(next, o.due);
@@ -321,6 +374,12 @@ static void run_gang(Gang* g) {
     if (++stagnant >= 3) g->vtime_jump += 250000000ull;
     if (stagnant > 120000) {
       g->hung = true; g_hangs++;
+      if (g_cfg.verbose) {
+        std::map<std::string, int> stuck;
+        for (auto& f : g->fibers)
+          if (!f->done) { char b[160]; snprintf(b, sizeof b, "cta %d warp %d: %s 0x%x", f->ctx.cta->rank, f->ctx.warp, f->where, f->where_arg); stuck[b]++; }
+        for (auto& kv : stuck) fprintf(stderr, "[emu] stuck: %3d threads  %s\n", kv.second, kv.first.c_str());
+      }
       violation("%s: CTA (%u,%u) hangs: no thread can make progress and nothing is in flight", g->kernel,
                 g->ctas[0]->bid.x, g->ctas[0]->bid.y);
       break;
@@ -344,6 +403,7 @@ void cta_barrier() {
   const uint32_t gen = c->bar_gen;
   c->bar_arrived++;
   cta_try_release(c);
+  g_fiber->where = "__syncthreads"; g_fiber->where_arg = 0;
   while (c->bar_gen == gen) yield();
 }
 void cluster_barrier() {
@@ -351,6 +411,7 @@ void cluster_barrier() {
   const uint32_t gen = g->cl_gen;
   g->cl_arrived++;
   cluster_try_release(g);
+  g_fiber->where = "cluster barrier"; g_fiber->where_arg = 0;
   while (g->cl_gen == gen) yield();
 }
 void warp_barrier(unsigned mask) {
@@ -361,6 +422,7 @@ void warp_barrier(unsigned mask) {
   w.mask = mask;
   w.arrived |= 1u << t->lane;
   warp_try_release(w);
+  g_fiber->where = "warp-synchronous operation (arrived mask in arg)"; g_fiber->where_arg = w.arrived;
   while (w.gen == gen) yield();
 }
 void warp_exchange(unsigned mask, const void* in, void* out, int bytes, int src_lane) {
@@ -503,6 +565,7 @@ bool mbar_try_wait(uint32_t addr, uint32_t parity) {
     Mbar* b = mbar_at(self, addr, "mbarrier.try_wait");
     if (!b) return true;                       // recorded; do not spin on it
     if (b->phase != (parity & 1)) { note_progress(); return true; }
+    g_fiber->where = "mbarrier.try_wait"; g_fiber->where_arg = addr;
     if (attempt == 0) yield();                 // potentially blocking: gives the others one turn, then reports
   }
   return false;
@@ -541,7 +604,11 @@ void tma_load(const CUtensorMap* map, uint32_t dst, uint32_t bar, int c0, int c1
   if (!bar_cta) return;
   const long id = g_tma_count++;
   const int coord[3] = {c0, c1, c2};
+  check_smem_write_issue(g, c, dst, dst + (uint32_t)bytes, "TMA load");
+  asan_guard(c, dst, bytes, true);
+  Touch touch; touch.smem_w.push_back(Range{c, dst, dst + (uint32_t)bytes});
   post(g, [=]() {
+    asan_guard(c, dst, bytes, false);
     uint8_t* base = window_ptr(c, dst, bytes, "TMA load");
     if (base) {
       for (uint32_t i2 = 0; i2 < m.box[2]; ++i2)
@@ -563,7 +630,7 @@ void tma_load(const CUtensorMap* map, uint32_t dst, uint32_t bar, int c0, int c1
     }
     if (id == g_cfg.drop_tma) return;                                  // injected fault: the completion is lost
     mbar_complete_tx(bar_cta, bar, (uint32_t)bytes, "TMA complete_tx");
-  });
+  }, std::move(touch));
 }
 
 // plain bulk copies
@@ -573,12 +640,19 @@ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   if ((dst & 15u) || ((uintptr_t)src & 15u) || (bytes & 15u) || bytes == 0) { violation("%s: cp.async.bulk needs 16-byte aligned addresses and size (dst 0x%x, src %p, %u bytes)", g->kernel, dst, src, bytes); return; }
   if (!in_device(src, bytes)) { violation("%s: cp.async.bulk reads [%p, +%u) outside every device allocation", g->kernel, src, bytes); return; }
   const long id = g_tma_count++;
+  check_smem_write_issue(g, c, dst, dst + bytes, "cp.async.bulk");
+  asan_guard(c, dst, bytes, true);
+  Touch touch; touch.smem_w.push_back(Range{c, dst, dst + bytes});
+  // the copy engine may read its source any time between issue and completion: either extreme, by the schedule's seed
+  std::shared_ptr<std::vector<uint8_t>> early;
+  if (rnd(g) & 1) early = std::make_shared<std::vector<uint8_t>>((const uint8_t*)src, (const uint8_t*)src + bytes);
   post(g, [=]() {
+    asan_guard(c, dst, bytes, false);
     uint8_t* p = window_ptr(c, dst, bytes, "cp.async.bulk (global -> shared)");
-    if (p) memcpy(p, src, bytes);
+    if (p) memcpy(p, early ? early->data() : (const uint8_t*)src, bytes);
     if (id == g_cfg.drop_tma) return;
     mbar_complete_tx(c, bar, bytes, "cp.async.bulk complete_tx");
-  });
+  }, std::move(touch));
 }
 void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
   Cta* c = cur()->cta;
@@ -640,6 +714,7 @@ void tmem_ld32(uint32_t taddr, uint32_t* v) {
   Cta* c = t->cta;
   warp_barrier(0xffffffffu);
   const uint32_t lane0 = taddr >> 16, col = taddr & 0xffffu;
+  check_tmem_thread_access(c->gang, c, col, col + 32, false, "tcgen05.ld");
   if (lane0 != (uint32_t)(t->warp & 3) * 32u) violation("%s: tcgen05.ld from lanes %u.. by warp %d (a warp may only touch lane quadrant warp %% 4)", c->gang->kernel, lane0, t->warp);
   for (uint32_t j = 0; j < 32; ++j) {
     uint32_t* p = tmem_cell(c, lane0 + (uint32_t)t->lane, col + j, "tcgen05.ld");
@@ -651,6 +726,7 @@ void tmem_st32(uint32_t taddr, const uint32_t* v) {
   Cta* c = t->cta;
   warp_barrier(0xffffffffu);
   const uint32_t lane0 = taddr >> 16, col = taddr & 0xffffu;
+  check_tmem_thread_access(c->gang, c, col, col + 32, true, "tcgen05.st");
   if (lane0 != (uint32_t)(t->warp & 3) * 32u) violation("%s: tcgen05.st to lanes %u.. by warp %d (a warp may only touch lane quadrant warp %% 4)", c->gang->kernel, lane0, t->warp);
   for (uint32_t j = 0; j < 32; ++j) {
     uint32_t* p = tmem_cell(c, lane0 + (uint32_t)t->lane, col + j, "tcgen05.st");
@@ -725,6 +801,25 @@ void tc_mma(uint32_t d_tmem, bool a_in_tmem, uint32_t a_tmem, uint64_t a_desc, u
   Cta* c = cur()->cta;
   Gang* g = c->gang;
   g_mma_count++;
+  // what this MMA will touch (decoded the way the execution below decodes it), checked against the copies in flight
+  Touch touch;
+  {
+    const int N = (int)((idesc >> 17) & 0x3f) << 3, a_mn = (int)(idesc >> 15) & 1, b_mn = (int)(idesc >> 16) & 1;
+    const int ncta = pair ? 2 : 1;
+    auto operand = [&](const Cta* cc, uint64_t desc, bool mn, int rows) {
+      const uint32_t start = (uint32_t)(desc & 0x3fff) << 4, lbo = (uint32_t)((desc >> 16) & 0x3fff) << 4, sbo = (uint32_t)((desc >> 32) & 0x3fff) << 4;
+      if (!mn) touch.smem_r.push_back(Range{cc, start & ~127u, (start & ~127u) + (uint32_t)((rows + 7) / 8 - 1) * sbo + 1024u});
+      else for (int grp = 0; grp < (rows + 31) / 32; ++grp) touch.smem_r.push_back(Range{cc, start + (uint32_t)grp * lbo, start + (uint32_t)grp * lbo + sbo + 512u});
+    };
+    for (int h = 0; h < ncta && (size_t)(pair ? h : c->rank) < g->ctas.size(); ++h) {
+      const Cta* cc = g->ctas[(size_t)(pair ? h : c->rank)].get();
+      operand(cc, b_desc, b_mn != 0, N / ncta);
+      if (a_in_tmem) touch.tmem_r.push_back(Cols{cc, a_tmem & 0xffffu, (a_tmem & 0xffffu) + 8u});
+      else operand(cc, a_desc, a_mn != 0, 128);
+      touch.tmem_w.push_back(Cols{cc, d_tmem & 0xffffu, (d_tmem & 0xffffu) + (uint32_t)N});
+    }
+    for (const Range& r : touch.smem_r) check_smem_read_issue(g, r.cta, r.lo, r.hi, "tcgen05.mma");
+  }
   post_pipe(g, [=]() {
     const int M = (int)((idesc >> 24) & 0x1f) << 4, N = (int)((idesc >> 17) & 0x3f) << 3;
     const int a_mn = (int)(idesc >> 15) & 1, b_mn = (int)(idesc >> 16) & 1;
@@ -769,7 +864,7 @@ void tc_mma(uint32_t d_tmem, bool a_in_tmem, uint32_t a_tmem, uint64_t a_desc, u
         }
       }
     }
-  });
+  }, std::move(touch));
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -815,6 +910,11 @@ static void execute(const LaunchCfg& cfg, const char* name, const std::function<
           c->region = (uint8_t*)region;
           c->dyn = c->region + c->dyn_base;                  // a kernel that aligns the generic pointer aligns the window address
           memset(c->region, 0xCD, kWindowBytes);             // shared memory is not zero at kernel start
+#if EMU_ASAN
+          // memcheck for the kernels' own (generic) loads and stores: only the launched bytes are addressable
+          __asan_poison_memory_region(c->region, kWindowBytes);
+          __asan_unpoison_memory_region(c->dyn, cfg.smem);
+#endif
           c->tmem.assign((size_t)kTmemLanes * kTmemCols, 0x7fc00000u);
           c->nthreads = c->live = nthreads;
           c->warps.resize((size_t)(nthreads + 31) / 32);
@@ -835,7 +935,12 @@ static void execute(const LaunchCfg& cfg, const char* name, const std::function<
           g.ctas.push_back(std::move(c));
         }
         run_gang(&g);
-        for (auto& c : g.ctas) free(c->region);
+        for (auto& c : g.ctas) {
+#if EMU_ASAN
+          __asan_unpoison_memory_region(c->region, kWindowBytes);
+#endif
+          free(c->region);
+        }
         if (g.hung) { g_sticky = cudaErrorLaunchFailure; return; }
       }
 }
@@ -1057,6 +1162,8 @@ int emu_set(const char* key, long v) {
   else if (k == "drop_tma") g_cfg.drop_tma = v < 0 ? -1 : g_tma_count + v;
   else if (k == "drop_commit") g_cfg.drop_commit = v < 0 ? -1 : g_commit_count + v;
   else if (k == "shuffle") g_cfg.shuffle = (int)v;
+  else if (k == "starve_mask") g_cfg.starve_mask = (unsigned)v;
+  else if (k == "starve_period") g_cfg.starve_period = (int)v;
   else if (k == "verbose") g_cfg.verbose = (int)v;
   else return -1;
   return 0;
