@@ -157,6 +157,36 @@ def sc_fault(g, E, a):
     return report(E, error=err, code=code, seconds=time.time() - t0, errors_after=after)
 
 
+def sc_fault_sweep(g, E, a):
+    """Every one of `count` consecutive TMA completions (or commits) of an evaluation lost in turn.  Each run must end
+    either in GMCO_E_CUDA or -- where the lost completion is one nobody waits for -- in a correct result; never in a hang."""
+    c = custom_case(a)
+    T = np.repeat(c.T0[None], c.n_plans, axis=0)
+    ref = oracle.evaluate(c.D, c.structures, T, c.weights)
+    h = g.gmco_create(c.D, c.structures, c.rx, options(a, c))
+    contained = harmless = wrong = 0
+    sites = {}
+    try:
+        first = int(a.get("first", 0))
+        for nth in range(first, first + int(a["count"]) * int(a.get("stride", 1)), int(a.get("stride", 1))):
+            E.emu_set(a["drop"].encode(), nth)
+            try:
+                out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
+                if max(eval_errors(out, ref).values()) < 1e-4:
+                    harmless += 1
+                else:
+                    wrong += 1
+            except b.GmcoError as ex:
+                contained += 1
+                key = str(ex).split("did not complete in ")[-1].split(", block")[0]
+                sites[key] = sites.get(key, 0) + 1
+            E.emu_set(a["drop"].encode(), -1)
+        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=True, host=True)
+    finally:
+        g.gmco_destroy(h)
+    return report(E, contained=contained, harmless=harmless, wrong=wrong, sites=sites, errors_after=eval_errors(out, ref))
+
+
 def sc_sa(g, E, a):
     """gSA chains on the fp64 route: the whole trajectory must equal the oracle's (acceptance counts, dwell times)."""
     c = custom_case(a)
@@ -203,7 +233,7 @@ def sc_pool(g, E, a):
                   dose_rate=dict(max_ulp=int(ulp.max()), exact_fraction=float((ulp == 0).mean())))
 
 
-SCENARIOS = {"evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
+SCENARIOS = {"fault_sweep": sc_fault_sweep, "evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
 
 
 def main():

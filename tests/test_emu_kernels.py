@@ -54,6 +54,13 @@ SCENARIOS = {
     "pair_static@in_order": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, seed=5, max_delay=1, shuffle=0, dyn_misalign=1008, **SMALL),
     "streamed_384@slow_pipe": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, seed=6, max_delay=20, mma_delay=20000, **SMALL),
     "streamed_384@slow_copies": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, seed=7, max_delay=20000, mma_delay=1, dyn_misalign=1008, **SMALL),
+    # a starved producer (warp 0), issuer (warp 1) or epilogue (warps 2-9): one turn in 40 rounds
+    "pair_static@starved_producer": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, starve_mask=1, starve_period=40, **SMALL),
+    "pair_static@starved_issuer": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, starve_mask=2, starve_period=40, **SMALL),
+    "pair_static@starved_epilogue": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, starve_mask=1020, starve_period=40, **SMALL),
+    "streamed_384@starved_producer": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, starve_mask=1, starve_period=40, **SMALL),
+    "streamed_384@starved_issuer": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, starve_mask=2, starve_period=40, **SMALL),
+    "streamed_384@starved_epilogue": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, starve_mask=1020, starve_period=40, mma_delay=1, **SMALL),
     "resident@slow_pipe": dict(scenario="evaluate", sm_count=4, seed=8, max_delay=20, mma_delay=20000),
     "resident@slow_copies": dict(scenario="evaluate", sm_count=4, seed=9, max_delay=20000, mma_delay=1, dyn_misalign=0),
     # ---- whole optimisations: device-side WHILE loop, k_step, compaction, stopping rules ----
@@ -73,6 +80,15 @@ SCENARIOS = {
     "fault_commit_pair": dict(scenario="fault", sm_count=4, drop="drop_commit", nth=3, n_plans=256, **SMALL),
     "fault_tma_streamed": dict(scenario="fault", sm_count=2, drop="drop_tma", nth=33, n_plans=128, n_cath=24, n_pos=16, **SMALL),
     "fault_in_loop": dict(scenario="fault", sm_count=4, drop="drop_tma", nth=300, via="optimize"),
+    # every one of 40 consecutive completions lost in turn, per kernel family and per unit
+    "sweep_tma_streamed": dict(scenario="fault_sweep", drop="drop_tma", count=40, sm_count=2, n_plans=128, n_cath=24, n_pos=16, counts=[300, 60, 70, 70]),
+    "sweep_commit_streamed": dict(scenario="fault_sweep", drop="drop_commit", count=40, sm_count=2, n_plans=128, n_cath=24, n_pos=16, counts=[300, 60, 70, 70]),
+    "sweep_tma_pair": dict(scenario="fault_sweep", drop="drop_tma", count=40, sm_count=2, n_plans=256, n_cath=18, n_pos=14, counts=[300, 60, 70, 70]),
+    "sweep_commit_pair": dict(scenario="fault_sweep", drop="drop_commit", count=40, sm_count=2, n_plans=256, n_cath=18, n_pos=14, counts=[300, 60, 70, 70]),
+    "sweep_tma_resident_and_grad": dict(scenario="fault_sweep", drop="drop_tma", count=40, stride=2, sm_count=2),
+    "sweep_commit_resident_and_grad": dict(scenario="fault_sweep", drop="drop_commit", count=40, stride=2, sm_count=2),
+    # a lost history copy of k_step inside the device-side loop
+    "fault_step_history": dict(scenario="fault", sm_count=2, drop="drop_tma", nth=377, via="optimize", iters=6),
     # ---- the other entry points ----
     "sa_fp64": dict(scenario="sa", n_plans=3, steps=300),
     "pool": dict(scenario="pool"),
@@ -189,6 +205,21 @@ def test_a_lost_completion_ends_in_an_error_code_not_in_a_hang(results, name, ke
     assert r["code"] == -3 and "barrier wait did not complete" in r["error"] and kernel in r["error"], r["error"]
     e = r["errors_after"]                                      # and the handle works again afterwards
     assert e["dose"] < TOL_EVAL and e["F"] < TOL_EVAL and e["grad"] < TOL_EVAL
+
+
+@pytest.mark.parametrize("name", [n for n in SCENARIOS if n.startswith("sweep_")])
+def test_no_lost_completion_anywhere_can_hang_or_corrupt(results, name):
+    r = _ok(results, name)                                     # 40 faults in a row on one handle: no hazard, no hang, nothing leaks
+    assert r["wrong"] == 0, r                                  # never a silently wrong result
+    assert r["contained"] + r["harmless"] == 40 and r["contained"] >= 20, r
+    assert all(k.startswith("k_") and "wait:" in k for k in r["sites"]), r["sites"]
+    e = r["errors_after"]
+    assert e["dose"] < TOL_EVAL and e["F"] < TOL_EVAL and e["grad"] < TOL_EVAL
+
+
+def test_lost_history_copy_of_k_step_is_contained(results):
+    r = _ok(results, "fault_step_history")
+    assert r["code"] == -3 and "barrier wait did not complete" in r["error"], r["error"]
 
 
 def test_gsa_fp64_trajectory_equals_the_oracle(results):
