@@ -107,6 +107,19 @@ __device__ __forceinline__ bool mbar_wait_cluster(const Watch& w, uint64_t* bar,
   if (!ok) ok = mbar_wait_slow(b, parity, 1, w.err, w.abort_addr, (w.kernel << 8) | site);
   return __all_sync(0xffffffffu, ok) != 0;       // warp-uniform, see mbar_wait_addr
 }
+// Waits of a role that ONE thread runs alone (the MMA issue loops: one elected lane walks the whole loop, the other
+// lanes of its warp wait at the role's closing __syncwarp).  No vote, no elect and no reconvergence per ring entry:
+// the fast path is one poll and one branch, everything else is out of line.  (The issuing thread's instruction stream,
+// not the tensor pipe, bounds the dose kernel: profiles/r1_ncu_dose_pair.md, profiles/r2_issue_loop_sass.md.)
+__device__ __forceinline__ bool mbar_wait1_addr(const Watch& w, uint32_t bar, uint32_t parity, int site) {
+  if (mbar_try_wait_addr(bar, parity)) return true;
+  return mbar_wait_slow(bar, parity, 0, w.err, w.abort_addr, (w.kernel << 8) | site);
+}
+__device__ __forceinline__ bool mbar_wait1_cluster(const Watch& w, uint64_t* bar, uint32_t parity, int site) {
+  const uint32_t b = smem_u32(bar);
+  if (mbar_try_wait_cluster_addr(b, parity)) return true;
+  return mbar_wait_slow(b, parity, 1, w.err, w.abort_addr, (w.kernel << 8) | site);
+}
 // inside a role's lambda: give the role up when the wait was abandoned
 #define GMCO_WAIT(call) do { if (!(call)) return; } while (0)
 
@@ -323,8 +336,8 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   } else if (warp == 1) {
     auto issuer = [&]() {
       if (c1 <= c0) return;
-      // Issue loop.  Everything is warp-uniform (uniform datapath); one elected lane issues.  Per ring entry: one wait, 8 or 4
-      // MMAs whose descriptors differ by 32-bit adds, one commit.
+      // Issue loop, run by ONE elected lane (see below): per ring entry one poll of the full barrier, 8 or 4 MMAs whose
+      // descriptors differ by 32-bit adds, one commit -- no vote, elect or reconvergence per entry.
       constexpr uint32_t idesc = instr_desc(kPC, 0, 0);
       constexpr uint32_t dhi = desc_hi(1024, kSwz128);
       const int n_stage = a.n_stage, n_acc = a.n_acc;
@@ -334,15 +347,15 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
       int st = 0; uint32_t ph = 0;
       for (int c = c0; c < c1; ++c) {
         const int b = n_acc == 2 ? (c - c0) & 1 : 0, use = n_acc == 2 ? (c - c0) >> 1 : c - c0;
-        GMCO_WAIT(mbar_wait(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
+        GMCO_WAIT(mbar_wait1_addr(w, smem_u32(acc_empty + b), (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
         tc_fence_after();
         const uint32_t acc0 = t_acc + b * (a.sep_corr ? (uint32_t)(n_main + 1) * kPC : kPC), acc_c = a.sep_corr ? acc0 + corr_off : acc0;
         uint32_t thi = t_thi, alo = tlo_lo0;   // alo: resident T_lo slab g, or (streamed) T_hi tail slab g - kTg
         for (int g = 0; g < G; thi += 32, alo += (kResident || g >= kTg) ? kTloBox >> 4 : 0, ++g) {
           // entry 2 g: D_hi slab (+ the streamed T_lo slab behind it): T_hi D_hi and T_lo D_hi
-          if (c == c0) { GMCO_WAIT(mbar_wait(w, tg_ready + g, 0, DEVERR_W_TG_READY)); tc_fence_after(); }   // first chunk overlaps the prologue
-          GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
-          if (elect_one()) {
+          if (c == c0) { GMCO_WAIT(mbar_wait1_addr(w, smem_u32(tg_ready + g), 0, DEVERR_W_TG_READY)); tc_fence_after(); }   // first chunk overlaps the prologue
+          GMCO_WAIT(mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
+          {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             const uint32_t ad = kResident ? alo : bd + (kSlabBytes >> 4);
             const uint32_t acc = g < g_half ? acc0 : acc0 + kPC;                 // main accumulator A or B
@@ -366,11 +379,10 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
             }
             tc_commit_addr(empty0 + 8 * st);
           }
-          __syncwarp();
           if (++st == n_stage) { st = 0; ph ^= 1; }
           // entry 2 g + 1: D_lo slab: T_hi D_lo
-          GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
-          if (elect_one()) {
+          GMCO_WAIT(mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));
+          {
             const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
             if (kResident || g < kTg) {
 #pragma unroll
@@ -382,12 +394,12 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
             tc_commit_addr(empty0 + 8 * st);
             if (g == G - 1) tc_commit(acc_full + b);
           }
-          __syncwarp();
           if (++st == n_stage) { st = 0; ph ^= 1; }
         }
       }
     };
-    issuer();
+    if (elect_one()) issuer();                        // one lane issues every MMA and commit of the CTA
+    __syncwarp();
   } else {
     const int e = warp - 2;                         // 0..7
     const int q = warp & 3;                         // TMEM lane quadrant this warp may access
@@ -669,12 +681,12 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
       const uint32_t tlo_lo0 = desc_lo(smem_u32(tlo), 16);
       const uint32_t full0 = smem_u32(full), empty0 = smem_u32(empty);
       constexpr uint32_t kG1 = (uint32_t)kHalfSlab >> 4;       // second dwell group of an entry
-      // One ring entry: wait, 4 or 8 MMAs, commit.  kind 0: T_hi D_lo, 1: T_lo D_hi, 2: T_hi D_hi.  false: wait abandoned.
+      // This whole role is run by ONE elected lane (see below).  One ring entry: wait, 4 or 8 MMAs, commit.  kind 0: T_hi D_lo, 1: T_lo D_hi, 2: T_hi D_hi.  false: wait abandoned.
       auto entry = [&](const int kind, const int gp, const int st, const uint32_t ph, const uint32_t acc, const bool two,
                        const uint32_t acc_full_bar) -> bool {
-        if (!mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL)) return false;
+        if (!mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL)) return false;
         tc_fence_after();
-        if (elect_one()) {
+        {
           const uint32_t bd = ring_lo + (uint32_t)st * ring_step;
           const uint32_t thi = t_thi + 64 * gp, alo = tlo_lo0 + 2 * (kTloBox >> 4) * gp;
           if (kind == 1) {
@@ -696,7 +708,6 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
           tc_commit_pair(empty0 + 8 * st);
           if (acc_full_bar) tc_commit_pair(acc_full_bar);
         }
-        __syncwarp();
         return true;
       };
       if constexpr (GP > 0) {
@@ -708,15 +719,15 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         const bool odd = (G & 1) != 0;
         for (int c = c0; c < c1; ++c) {
           const int b = (c - c0) & 1, use = (c - c0) >> 1;
-          GMCO_WAIT(mbar_wait_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
+          GMCO_WAIT(mbar_wait1_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
           tc_fence_after();
           const uint32_t acc = t_acc + (uint32_t)b * kPC;
 #pragma unroll
           for (int gp = 0; gp < GP; ++gp) {
             const bool two = gp < GP - 1 || !odd;
             if (c == c0) {                            // the first chunk overlaps the prologue, group by group
-              GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
-              if (two) GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
+              GMCO_WAIT(mbar_wait1_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
+              if (two) GMCO_WAIT(mbar_wait1_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
               tc_fence_after();
             }
             GMCO_WAIT(entry(0, gp, (2 * gp) % NS, chunk_par ^ (((2 * gp) / NS) & 1), acc, two, 0u));
@@ -734,14 +745,14 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         int st = 0; uint32_t ph = 0;
         for (int c = c0; c < c1; ++c) {
           const int b = (c - c0) & 1, use = (c - c0) >> 1;
-          GMCO_WAIT(mbar_wait_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
+          GMCO_WAIT(mbar_wait1_cluster(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));
           tc_fence_after();
           const uint32_t acc = t_acc + (uint32_t)b * kPC;
           for (int gp = 0; gp < Gp; ++gp) {           // corrections first
             const bool two = 2 * gp + 1 < G;
             if (c == c0) {
-              GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
-              if (two) GMCO_WAIT(mbar_wait_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
+              GMCO_WAIT(mbar_wait1_cluster(w, tg_ready + 2 * gp, 0, DEVERR_W_TG_READY));
+              if (two) GMCO_WAIT(mbar_wait1_cluster(w, tg_ready + 2 * gp + 1, 0, DEVERR_W_TG_READY));
               tc_fence_after();
             }
             GMCO_WAIT(entry(0, gp, st, ph, acc, two, 0u));
@@ -756,7 +767,8 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
         }
       }
     };
-    issuer();
+    if (elect_one()) issuer();                        // one lane issues every MMA and commit of the CTA pair
+    __syncwarp();
   } else {
     const int e = warp - 2;                           // 0..7
     const int q = warp & 3;                           // TMEM lane quadrant this warp may access
@@ -919,7 +931,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
       if (s1 <= s0) return;
       // The accumulator is A_pad columns wide; one MMA covers at most 256 of them.  When the columns last (A_pad <= 256)
       // the two correction products go into a separate accumulator at column 256 (see k_dose_tc: the tensor core's
-      // accumulate truncates).  Lean issue loop: descriptors differ by 32-bit adds.
+      // accumulate truncates).  Lean issue loop run by ONE elected lane: descriptors differ by 32-bit adds.
       const int n0 = a.A_pad <= 256 ? a.A_pad : 256, n1 = a.A_pad - n0;
       const uint32_t idesc0 = instr_desc(n0, 1, 1), idesc1 = instr_desc(n1 > 0 ? n1 : 16, 1, 1);
       constexpr uint32_t dhi = desc_hi(512, kSwz128Base32);
@@ -931,9 +943,9 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
       const uint32_t conv0 = smem_u32(conv), empty0 = smem_u32(empty);
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        GMCO_WAIT(mbar_wait_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));
+        GMCO_WAIT(mbar_wait1_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));
         tc_fence_after();
-        if (elect_one()) {
+        {
           const uint32_t r = base_lo + (uint32_t)st * stage_step;
 #pragma unroll
           for (int j = 0; j < PS / 8; ++j) {        // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
@@ -951,11 +963,11 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
           tc_commit_addr(empty0 + 8 * st);
           if (s == s1 - 1) tc_commit(acc_full);
         }
-        __syncwarp();
         if (++st == n_stage) { st = 0; ph ^= 1; }
       }
     };
-    issuer();
+    if (elect_one()) issuer();                        // one lane issues every MMA and commit of the CTA
+    __syncwarp();
   } else {
     const int q = warp & 3;
     const int L = q * 32 + lane;

@@ -97,13 +97,13 @@ MUTANTS = {
     # producer refills a ring slot without waiting for the commit of the MMAs that read it
     "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));", "", 3),
     # MMAs issued before the TMA bytes of their operands have landed
-    "issuer_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));", "", 2),
+    "issuer_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));", "", 2),
     # gradient MMAs issued before the converter warps have split the R tile (and before it has landed)
-    "grad_issuer_skips_conv_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));", "", 1),
+    "grad_issuer_skips_conv_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, conv0 + 8 * st, ph, DEVERR_W_CONV));", "", 1),
     # epilogue reads the accumulator without waiting for the chunk's last commit
     "epilogue_skips_acc_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, acc_full + b, use & 1, DEVERR_W_ACC_FULL));", "", 2),
     # issuer overwrites the accumulator without waiting for the epilogue to hand it back
-    "issuer_skips_acc_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, acc_empty + b, (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));", "", 1),
+    "issuer_skips_acc_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, smem_u32(acc_empty + b), (use & 1) ^ 1, DEVERR_W_ACC_EMPTY));", "", 1),
     # the epilogue hands the accumulator back before it has read it
     "accumulator_handed_back_too_early": ("kernels_tc.cu", "        tmem_ld32(t_main, v[0]);\n        tmem_ld32(t_main + 32, v[1]);\n        if (a.sep_corr) {",
                                           "        mbar_arrive(acc_empty + b);\n        tmem_ld32(t_main, v[0]);\n        tmem_ld32(t_main + 32, v[1]);\n        if (a.sep_corr) {", 1),

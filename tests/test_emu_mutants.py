@@ -85,4 +85,6 @@ def test_hazard_messages_name_what_happened(results):
     assert "before its consumer's commit" in results["issuer_skips_full_wait"]["violation"] or "in flight" in results["issuer_skips_full_wait"]["violation"]
     assert "accumulator touched before its commit arrived" in results["issuer_skips_acc_empty_wait"]["violation"]
     assert "without tcgen05.dealloc" in results["tmem_never_freed"]["violation"]
-    assert "outside the CTA's window" in results["host_smem_too_small_unchecked"]["violation"]
+    # barriers and ring then overlap / run past the launched window: whichever consequence comes first under the schedule
+    v = results["host_smem_too_small_unchecked"]["violation"]
+    assert any(t in v for t in ("outside the CTA's window", "still in flight", "was overwritten", "no initialised mbarrier", "hangs")), v

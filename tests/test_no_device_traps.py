@@ -29,10 +29,12 @@ def test_sources_hold_no_trap_and_no_unbounded_spin():
     ptx = re.sub(r"//[^\n]*", "", (CSRC / "gmco_ptx.cuh").read_text())
     assert len(re.findall(r"try_wait\.parity", ptx)) == 2               # the two raw (unbounded-by-themselves) polls
     # every mbarrier wait of the tensor kernels goes through the bounded helpers: the raw polls are called from
-    # mbar_wait_slow / mbar_wait_addr / mbar_wait_cluster only (4 calls), and from k_step's bounded history wait (1 call)
+    # mbar_wait_slow / mbar_wait_addr / mbar_wait_cluster / mbar_wait1_addr / mbar_wait1_cluster only (6 calls, each
+    # followed by the bounded slow path), and from k_step's bounded history wait (1 call)
     tc = re.sub(r"//[^\n]*", "", (CSRC / "kernels_tc.cu").read_text())
     assert "kWaitLimitNs" in tc and "mbar_wait_slow" in tc and "drain_if_aborted" in tc
-    assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", tc)) == 4
+    assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", tc)) == 6
+    assert len(re.findall(r"return mbar_wait_slow\(", tc)) == 2 and len(re.findall(r"ok = mbar_wait_slow\(", tc)) == 2
     lb = re.sub(r"//[^\n]*", "", (CSRC / "kernels_lbfgs.cu").read_text())
     assert len(re.findall(r"mbar_try_wait(?:_cluster)?_addr\(", lb)) == 1
     assert "4000000000ull" in lb and "DEVERR_W_HISTORY" in lb            # k_step's history wait is bounded too
