@@ -112,8 +112,10 @@ def sc_optimize(g, E, a):
     try:
         if a.get("profile"):
             g.gmco_set_profiling(h, True)
+        executed0 = int(E.emu_counter(b"executed"))
         g.gmco_optimize(h, c.T0, c.weights, c.iters)
         out = g.gmco_result(h, host=True)
+        executed = int(E.emu_counter(b"executed")) - executed0       # kernels that really ran, graph replays included
         st = g.gmco_get_stats(h)
     finally:
         g.gmco_destroy(h)
@@ -123,7 +125,7 @@ def sc_optimize(g, E, a):
     return report(E, rel_F_max=float(rel_f.max()), rel_F_same_iters_max=float(rel_f[same_it].max()) if same_it.any() else None,
                   dvh_pp_max=float(dvh_pp.max()), iters_gpu=out["iters_done"].tolist(), iters_ref=np.asarray(ref["iters_done"]).tolist(),
                   status_gpu=out["plan_status"].tolist(), status_ref=np.asarray(ref["status"]).tolist(),
-                  rounds=int(st["rounds"]), launches=int(st["kernel_launches"]), dose_kernel=int(st["dose_kernel"]),
+                  rounds=int(st["rounds"]), launches=int(st["kernel_launches"]), executed=executed, dose_kernel=int(st["dose_kernel"]),
                   digest=digest(out["T"], out["objective"], out["dvh"]),
                   ls_launches=int(E.emu_counter(b"k_ls_pick")), step_launches=int(E.emu_counter(b"k_step")))
 

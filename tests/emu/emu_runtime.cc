@@ -1147,6 +1147,7 @@ long emu_counter(const char* what) {
   if (w == "mma") return g_mma_count;
   if (w == "hangs") return g_hangs;
   if (w == "launches") return (long)g_launches.size();
+  if (w == "executed") { long n = 0; for (const auto& kv : g_kernel_runs) n += kv.second; return n; }   // kernels run, graph replays included
   auto it = g_kernel_runs.find(w);
   long n = 0;
   for (const auto& kv : g_kernel_runs) if (kv.first.find(w) != std::string::npos) n += kv.second;

@@ -184,6 +184,15 @@ def test_the_device_loop_runs_exactly_the_rounds_that_are_needed(results):
     assert p["digest"] == _ok(results, "opt_no_compaction")["digest"] or p["rel_F_max"] < TOL_F_FINAL
 
 
+@pytest.mark.parametrize("name", ["opt_c1", "opt_profile_mode", "opt_no_compaction", "opt_simt", "opt_line_search", "opt_eps_pair_compaction"])
+def test_claimed_kernel_launches_equal_the_kernels_that_ran(results, name):
+    """gmco_stats.kernel_launches (bench.py's `gpu_launches`) is reconstructed from a device round counter when the rounds
+    run inside the WHILE graph ("a claim").  The emulated runtime counts every kernel it executes,
+    graph replays included: the two must agree on every route."""
+    r = _ok(results, name)
+    assert r["launches"] == r["executed"] > 0, (name, r["launches"], r["executed"])
+
+
 def test_eps_stopping_with_compaction_on_the_pair_kernel(results):
     r = _ok(results, "opt_eps_pair_compaction")
     assert r["dose_kernel"] == 3 and r["status_gpu"] == r["status_ref"]
