@@ -209,6 +209,43 @@ def sc_sa(g, E, a):
     return report(E, accepted_gpu=out["n_accepted"].tolist(), accepted_ref=acc_ref, T_abs_err=t_err, F_rel_err=f_err)
 
 
+def sc_smoke(g, E, a):
+    """The call sequence of __graft_entry__.smoke() (same cases, same arguments, same bars), on the emulation."""
+    c = gc.make_case("C1")
+    ref = oracle.optimize(c.D, c.structures, c.rx, c.T0, c.weights, m=c.m, iters=c.iters)
+    legs = {}
+    for prec, name in ((b.GMCO_PREC_TF32X3, "tf32x3"), (b.GMCO_PREC_SIMT_FP32, "simt_fp32")):
+        h = g.gmco_create(c.D, c.structures, c.rx, b.make_options(m=c.m, precision=prec))
+        try:
+            ev = g.gmco_evaluate(h, c.T0, c.weights, want_dose=True, host=True)       # 1-D T0: broadcast to all plans
+            g.gmco_optimize(h, c.T0, c.weights, c.iters)
+            out = g.gmco_result(h, host=True)
+        finally:
+            g.gmco_destroy(h)
+        ref_ev = oracle.evaluate(c.D, c.structures, c.T0, c.weights)
+        legs[name] = dict(dose=float(np.abs(ev["dose"] / ref_ev["dose"] - 1).max()), F=float(np.abs(out["objective"] / ref["F"] - 1).max()),
+                          dvh_pp=float(np.abs(out["dvh"] - ref["dvh"]).max()))
+    c2 = gc.make_case("C1", n_plans=256)
+    T = np.repeat(c2.T0[None], 256, axis=0) * np.linspace(0.7, 1.3, 256)[:, None].astype(np.float32)
+    h = g.gmco_create(c2.D, c2.structures, c2.rx)
+    try:
+        ev = g.gmco_evaluate(h, T, c2.weights, want_dose=True, host=True)
+    finally:
+        g.gmco_destroy(h)
+    ref_ev = oracle.evaluate(c2.D, c2.structures, T, c2.weights)
+    legs["pair_256"] = dict(dose=float(np.abs(ev["dose"] / ref_ev["dose"] - 1).max()), F=float(np.abs(ev["F"] / ref_ev["F"] - 1).max()),
+                            pair_kernel_ran=int(E.emu_counter(b"k_dose_tc_pair")))
+    h = g.gmco_create(c.D, c.structures, c.rx)
+    try:
+        jdx, z, u = gc.sa_draws(c.n_dwell, c.n_plans, 2000, seed=5)
+        sa = g.gmco_sa_run(h, c.T0, c.weights, jdx, z, u, float(c.T0[0]), host=True)
+    finally:
+        g.gmco_destroy(h)
+    r = oracle.sa_chain(c.D, c.structures, c.weights[0], c.T0, float(c.T0[0]), jdx[0], z[0], u[0])
+    legs["gsa"] = dict(accepted=int(sa["n_accepted"][0]), accepted_ref=int(r["n_accepted"]), F=float(abs(sa["objective"][0] / r["F"] - 1)))
+    return report(E, legs=legs)
+
+
 def sc_pool(g, E, a):
     """Pareto filter and plan selection (comparisons only: bit-exact) and the dose-rate matrix (one fp32 ulp)."""
     rng = np.random.Generator(np.random.PCG64(11))
@@ -235,7 +272,7 @@ def sc_pool(g, E, a):
                   dose_rate=dict(max_ulp=int(ulp.max()), exact_fraction=float((ulp == 0).mean())))
 
 
-SCENARIOS = {"fault_sweep": sc_fault_sweep, "evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
+SCENARIOS = {"smoke": sc_smoke, "fault_sweep": sc_fault_sweep, "evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
 
 
 def main():

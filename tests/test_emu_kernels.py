@@ -90,6 +90,7 @@ SCENARIOS = {
     # a lost history copy of k_step inside the device-side loop
     "fault_step_history": dict(scenario="fault", sm_count=2, drop="drop_tma", nth=377, via="optimize", iters=6),
     # ---- the other entry points ----
+    "smoke": dict(scenario="smoke"),                           # the call sequence of __graft_entry__.smoke()
     "sa_fp64": dict(scenario="sa", n_plans=3, steps=300),
     "pool": dict(scenario="pool"),
 }
@@ -229,6 +230,15 @@ def test_no_lost_completion_anywhere_can_hang_or_corrupt(results, name):
 def test_lost_history_copy_of_k_step_is_contained(results):
     r = _ok(results, "fault_step_history")
     assert r["code"] == -3 and "barrier wait did not complete" in r["error"], r["error"]
+
+
+def test_the_call_sequence_of_smoke_meets_its_bars(results):
+    """__graft_entry__.smoke() itself needs cuda:0; its calls, cases and bars are repeated on the emulation."""
+    legs = _ok(results, "smoke")["legs"]
+    for name in ("tf32x3", "simt_fp32"):
+        assert legs[name]["dose"] < 1e-4 and legs[name]["F"] < 1e-3 and legs[name]["dvh_pp"] < 0.5, legs[name]
+    assert legs["pair_256"]["dose"] < 1e-4 and legs["pair_256"]["F"] < 1e-4 and legs["pair_256"]["pair_kernel_ran"] == 1
+    assert legs["gsa"]["accepted"] == legs["gsa"]["accepted_ref"] and legs["gsa"]["F"] < 1e-9
 
 
 def test_gsa_fp64_trajectory_equals_the_oracle(results):
