@@ -173,9 +173,11 @@ inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, in
     t.grad_smem = kAlign + grad_smem(t.grad_ps, G, t.grad_stages).end;
     t.n_slabs = N_pad / t.grad_ps;
   }
-  // CTA-pair dose kernel: resident layout, an even number of plan tiles and of dwell groups.  The kernel handles an
-  // odd group count (zero-filled half entry), but that path has no GPU parity record, so such shapes stay on k_dose_tc.
-  t.dose_pair = (t.tlo_resident && t.n_tiles % 2 == 0 && G % 2 == 0 && !force_single) ? 1 : 0;
+  // CTA-pair dose kernel: resident layout and an even number of plan tiles.  With an odd number of dwell groups the last
+  // ring entry of a pass is half empty (the TMA box's second group lies outside the tensor and is zero-filled; its MMAs
+  // are skipped): executed against the oracle on the CPU emulation for G = 1, 3, 5, 7 (tests/test_emu_kernels.py); the
+  // GPU parity test of that path is tests/test_gpu_zz_pair.py.
+  t.dose_pair = (t.tlo_resident && t.n_tiles % 2 == 0 && !force_single) ? 1 : 0;
   if (t.dose_pair) {
     const int fixedp = G * kTloBox + slack;
     t.pair_stages = (kSmemMax - fixedp) / kPairEntry;

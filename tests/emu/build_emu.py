@@ -51,6 +51,15 @@ def transform(text: str) -> str:
 
 
 def build(force: bool = False, sanitize: bool = False) -> Path:
+    """Builds are serialised by a lock file: pytest-xdist workers and concurrent sessions may all ask for the library."""
+    import fcntl
+    OUT.mkdir(parents=True, exist_ok=True)
+    with open(OUT / ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        return _build(force, sanitize)
+
+
+def _build(force: bool, sanitize: bool) -> Path:
     lib = OUT / ("libgmco_emu_asan.so" if sanitize else "libgmco_emu.so")
     srcs = sorted(CSRC.glob("*.cu"))
     deps = srcs + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + [ROOT / "include" / "gmco.h"] + \
@@ -84,10 +93,12 @@ def build(force: bool = False, sanitize: bool = False) -> Path:
             failed = True
     if failed:
         raise RuntimeError("emulation build failed")
-    link = ["g++", "-shared", "-o", str(lib), *objs]
+    tmp = lib.with_suffix(f".{os.getpid()}.tmp")
+    link = ["g++", "-shared", "-o", str(tmp), *objs]
     if sanitize:
         link += ["-fsanitize=address,undefined"]
     subprocess.run(link, check=True)
+    os.replace(tmp, lib)                                   # processes that have the old library open keep it
     return lib
 
 
@@ -126,7 +137,14 @@ MUTANTS = {
 
 def build_mutant(name: str) -> Path:
     """libgmco_emu with one planted error.  Only the mutated translation units are recompiled."""
+    import fcntl
     plain = build()
+    with open(OUT / f".lock_{name}", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        return _build_mutant(name, plain)
+
+
+def _build_mutant(name: str, plain: Path) -> Path:
     lib = OUT / f"libgmco_emu_mut_{name}.so"
     if lib.exists() and lib.stat().st_mtime >= plain.stat().st_mtime and lib.stat().st_mtime >= Path(__file__).stat().st_mtime:
         return lib

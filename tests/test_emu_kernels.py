@@ -39,6 +39,10 @@ SCENARIOS = {
     "resident_forced_single": dict(scenario="evaluate", sm_count=4, n_plans=256, dose_kernel=1, n_cath=18, n_pos=14, **SMALL),
     "pair_ring": dict(scenario="evaluate", sm_count=4, n_plans=256, **SMALL),
     "pair_static": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, **SMALL),
+    # odd numbers of dwell groups on the pair kernel: the last ring entry of a pass is half empty (zero-filled TMA box)
+    "pair_ring_5_groups": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=16, n_pos=10, counts=[900, 210, 300, 270]),
+    "pair_static_7_groups": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=14, n_pos=16, counts=[900, 210, 300, 270]),
+    "pair_ring_1_group": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=3, n_pos=10, **SMALL),
     "pair_static_4_tiles_ragged": dict(scenario="evaluate", sm_count=8, n_plans=500, n_cath=17, n_pos=14, counts=[333, 77, 129, 65]),
     "streamed_288": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=18, n_pos=16, **SMALL),
     "streamed_384": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, **SMALL),
@@ -140,7 +144,8 @@ def test_every_dose_kernel_and_the_multi_chunk_paths_were_reached(results):
     want = {"simt": "k_simt_dose", "resident": "k_dose_tc<true>", "resident_forced_single": "k_dose_tc<true>", "pair_ring": "k_dose_tc_pair<0, 0>",
             "pair_static": "k_dose_tc_pair<4, 6>", "pair_static_4_tiles_ragged": "k_dose_tc_pair<4, 6>", "streamed_288": "k_dose_tc<false>",
             "streamed_384": "k_dose_tc<false>", "wide_accum_384": "k_dose_tc<false, true>", "wide_accum_352_3_tiles": "k_dose_tc<false, true>",
-            "resident_3_tiles_odd": "k_dose_tc<true>", "c3_full_size": "k_dose_tc_pair<4, 6>"}
+            "resident_3_tiles_odd": "k_dose_tc<true>", "c3_full_size": "k_dose_tc_pair<4, 6>", "pair_ring_5_groups": "k_dose_tc_pair<0, 0>",
+            "pair_static_7_groups": "k_dose_tc_pair<4, 6>", "pair_ring_1_group": "k_dose_tc_pair<0, 0>"}
     for name, kernel in want.items():
         r = _ok(results, name)
         assert r["kernels"][kernel] == 1 and sum(r["kernels"][k] for k in r["kernels"] if "dose" in k) == 1, (name, r["kernels"])

@@ -28,7 +28,7 @@ def _eval(g, c, T):
         g.gmco_destroy(h)
 
 
-@pytest.mark.parametrize("n_cath,n_pos", [(4, 10), (5, 20), (16, 10)], ids=["A40_2groups_pair", "A100_4groups_pair", "A160_5groups_single_cta"])
+@pytest.mark.parametrize("n_cath,n_pos", [(4, 10), (5, 20), (16, 10)], ids=["A40_2groups_pair", "A100_4groups_pair", "A160_5groups_pair_half_empty_entry"])
 def test_pair_kernel_evaluation_parity(g, n_cath, n_pos):
     c = gc.make_case("C1", n_cath=n_cath, n_pos=n_pos, counts=(900, 210, 300, 270), n_plans=256, seed_points=5, seed_weights=6)
     T = np.repeat(c.T0[None], c.n_plans, axis=0) * np.linspace(0.6, 1.4, c.n_plans)[:, None].astype(np.float32)

@@ -48,7 +48,7 @@ def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel, wi
             # ring entries hold their TMA boxes; every operand area starts 1024-aligned (SWIZZLE_128B atoms)
             assert q["dose_stages"] >= 2 and q["grad_stages"] >= 2
             if q["dose_kernel"] in (2, 3):
-                assert G % 2 == 0 and tiles % 2 == 0 and G <= 8 and dose_kernel == 0
+                assert tiles % 2 == 0 and G <= 8 and dose_kernel == 0             # any dwell-group count, odd ones included
                 assert q["dose_stage_bytes"] == K_PAIR_ENTRY == 32 * 4 * 64 * 2       # box {32 dwell, 64 points, 2 groups}
                 assert q["dose_tmem_cols"] == 32 * G + 256
                 if q["dose_kernel"] == 2:
