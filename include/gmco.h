@@ -105,7 +105,10 @@ typedef struct gmco_options {
   int32_t dose_kernel;/* 0: automatic -- CTA pairs (tcgen05 cta_group::2) where the shape allows, else one CTA per
                          plan tile; 1: always one CTA per plan tile.  Both compute the same products; they differ
                          in partial-sum order (low-order bits).  gmco_stats.dose_kernel says which one ran.
-                                                                                  default 0        */
+                         2: as 0, and the GRADIENT contraction runs on CTA pairs as well (k_grad_tc_pair: each CTA
+                         loads half of every D slab) where the shape allows -- at most 256 dwell positions, even
+                         numbers of plan tiles and of 32-dwell groups; else as 0.  Not the default: it has run
+                         on the CPU emulation of the kernels only.     default 0        */
   int32_t wide_accum; /* above 256 dwell positions (streamed T_lo layout) only.  1: the main product T_hi D_hi is
                          accumulated in TWO TMEM accumulators (first / second half of the dwell groups) that the
                          epilogue sums in fp32, which halves the tensor core's truncation error at
@@ -152,6 +155,8 @@ typedef struct gmco_tc_info {
   int32_t grad_threads, grad_ps, grad_stages, grad_stage_bytes, grad_smem_bytes, grad_smem_end, grad_staging_bytes,
       grad_tmem_cols;
   int32_t smem_limit, tmem_limit;        /* 232448 B opt-in dynamic shared memory per CTA, 512 TMEM columns       */
+  int32_t grad_pair;        /* 1: the gradient kernel is k_grad_tc_pair (dose_kernel = 2 and the shape allows it); the
+                               grad_* fields above then describe that kernel                                       */
 } gmco_tc_info;
 
 

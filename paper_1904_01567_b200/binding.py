@@ -47,7 +47,7 @@ class TcInfo(C.Structure):
         "dose_threads", "dose_stages", "dose_stage_bytes", "dose_smem_bytes", "dose_smem_end", "dose_scr_slot", "dose_tmem_cols",
         "dose_tmem_groups", "dose_n_main",
         "grad_threads", "grad_ps", "grad_stages", "grad_stage_bytes", "grad_smem_bytes", "grad_smem_end", "grad_staging_bytes",
-        "grad_tmem_cols", "smem_limit", "tmem_limit")]
+        "grad_tmem_cols", "smem_limit", "tmem_limit", "grad_pair")]
 
 DOSE_KERNEL_NAMES = {-1: "k_simt_dose", 0: "k_dose_tc<resident>", 1: "k_dose_tc<streamed>", 2: "k_dose_tc_pair<4,6>",
                      3: "k_dose_tc_pair<0,0>"}

@@ -95,14 +95,14 @@ int fail(gmco_handle* h, int code, const char* fmt, const char* a = "") {
 // the device error word (gmco_internal.cuh DevErr) as a GMCO_E_CUDA message; GMCO_OK when it is clear
 int check_dev_err(gmco_handle* h, const int* e) {
   if (e[0] == DEVERR_NONE) return GMCO_OK;
-  static const char* const kern[] = {"?", "k_dose_tc<resident>", "k_dose_tc<streamed>", "k_dose_tc_pair", "k_grad_tc", "k_step"};
+  static const char* const kern[] = {"?", "k_dose_tc<resident>", "k_dose_tc<streamed>", "k_dose_tc_pair", "k_grad_tc", "k_step", "k_grad_tc_pair"};
   static const char* const wait[] = {"-", "ring slot free", "ring slot filled", "T group ready", "T tile landed", "accumulator full",
                                      "accumulator free", "R tile split", "history copies"};
   static const char* const what[] = {"?", "a barrier wait did not complete", "the shared-memory carve-up does not fit the launch",
                                      "the TMEM columns do not fit"};
   const int k = (e[1] >> 8) & 0xff, wsite = e[1] & 0xff;
   snprintf(h->err, sizeof(h->err), "device error word: %s in %s (wait: %s), block (%d, %d), detail %d; results are invalid",
-           what[e[0] >= 1 && e[0] <= 3 ? e[0] : 0], kern[k >= 1 && k <= 5 ? k : 0], wait[wsite >= 1 && wsite <= 8 ? wsite : 0],
+           what[e[0] >= 1 && e[0] <= 3 ? e[0] : 0], kern[k >= 1 && k <= 6 ? k : 0], wait[wsite >= 1 && wsite <= 8 ? wsite : 0],
            e[2] & 0xffff, (e[2] >> 16) & 0xffff, e[3]);
   return GMCO_E_CUDA;
 }
@@ -217,7 +217,7 @@ int ensure_plans(gmco_handle* h, int K, cudaStream_t st) {
   carve_plans(h, K, 0);
   h->plan_capacity_K = K;
   if (h->opt.precision == GMCO_PREC_TF32X3 && K > 0) {
-    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->opt.dose_kernel == 1, h->opt.wide_accum == 1, st, h->err,
+    h->tc = tc_plan_create(h->c, h->p, h->sh.data(), h->num_sms, h->opt.dose_kernel == 1, h->opt.wide_accum == 1, h->opt.dose_kernel == 2, st, h->err,
                            sizeof(h->err));
     if (!h->tc) return GMCO_E_UNSUPPORTED;
   }
@@ -239,7 +239,7 @@ StepParams make_step_params(const gmco_handle* h, int iters) {
     sp.nG = 0; sp.g_slot_stride = (long long)kPlanTile * c.A_pad;
     sp.tile_local = 1; sp.tile_seg = tc_tile_seg_dev(h->tc);
     if (h->opt.compaction) { sp.compact_cap = tc_compact_cap(h->tc); sp.total_ctas = tc_num_segments(h->tc); }
-    sp.dose_pair = tc_dose_pair(h->tc);
+    sp.dose_pair = tc_dose_pair(h->tc); sp.grad_pair = tc_grad_pair(h->tc);
   }
   sp.S = c.S;
   sp.ls_cap = h->opt.line_search == 1 ? kLsCap : 0;
@@ -408,7 +408,7 @@ int gmco_create(gmco_handle** out, const float* D, int64_t n_points, int64_t n_d
   if (o.m < 1 || o.m > GMCO_MAX_HISTORY || o.max_trials < 1 || !(o.c1 > 0.f) || !(o.c1 < 1.f) || !(o.eps >= 0.f) ||
       !(o.eps_f >= 0.f) || !(o.eps_f < 1.f) ||
       (o.precision != GMCO_PREC_TF32X3 && o.precision != GMCO_PREC_SIMT_FP32) || (o.compaction != 0 && o.compaction != 1) ||
-      (o.dose_kernel != 0 && o.dose_kernel != 1) || (o.wide_accum != 0 && o.wide_accum != 1) ||
+      o.dose_kernel < 0 || o.dose_kernel > 2 || (o.wide_accum != 0 && o.wide_accum != 1) ||
       (o.line_search != 0 && o.line_search != 1))
     return fail(nullptr, GMCO_E_INVALID, "bad gmco_options%s");
   // the tensor layout holds T_hi (A_pad columns) plus an accumulator pair in 512 TMEM columns: wider cases take
@@ -895,7 +895,7 @@ int gmco_pareto_front(gmco_handle* h, const float* objectives, int32_t K, int32_
 int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_structs, int32_t K, int32_t num_sms,
                      int32_t dose_kernel, int32_t wide_accum, gmco_tc_info* out) {
   if (!out || !struct_points || n_dwell < 1 || n_structs < 1 || n_structs > GMCO_MAX_STRUCTS || K < 1 || num_sms < 1 ||
-      (dose_kernel != 0 && dose_kernel != 1) || (wide_accum != 0 && wide_accum != 1))
+      dose_kernel < 0 || dose_kernel > 2 || (wide_accum != 0 && wide_accum != 1))
     return fail(nullptr, GMCO_E_INVALID, "gmco_tc_schedule: NULL or non-positive argument%s");
   memset(out, 0, sizeof(*out));
   long long n_pad = 0;
@@ -908,7 +908,7 @@ int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_st
   out->a_pad = round_up(n_dwell, 32); out->n_pad = (int)n_pad; out->n_alloc = round_up(n_pad, kRowAlloc);
   out->k_pad = round_up(K, kPlanTile);
   if (out->a_pad > kMaxApadTensor) return GMCO_OK;   // ok = 0: the SIMT route takes the case
-  const tcl::Schedule q = tcl::choose_schedule(out->a_pad, out->n_pad, out->k_pad, num_sms, dose_kernel == 1, wide_accum == 1);
+  const tcl::Schedule q = tcl::choose_schedule(out->a_pad, out->n_pad, out->k_pad, num_sms, dose_kernel == 1, wide_accum == 1, dose_kernel == 2);
   if (!q.ok) return GMCO_OK;
   out->ok = 1;
   out->n_tiles = q.n_tiles; out->segs = q.segs; out->n_chunks = q.n_chunks; out->n_slabs = q.n_slabs;
@@ -929,6 +929,12 @@ int gmco_tc_schedule(int64_t n_dwell, const int32_t* struct_points, int32_t n_st
   out->grad_ps = q.grad_ps; out->grad_stages = q.grad_stages; out->grad_stage_bytes = gl.stage_bytes;
   out->grad_smem_bytes = q.grad_smem; out->grad_smem_end = gl.end; out->grad_staging_bytes = gl.staging_bytes;
   out->grad_tmem_cols = tcl::grad_tmem_cols(out->a_pad);
+  if (q.grad_pair) {                                 // the gradient kernel that would launch is k_grad_tc_pair
+    const tcl::GradSmem gp = tcl::grad_pair_smem(q.grad_ps, q.G, q.gpair_stages);
+    out->grad_stages = q.gpair_stages; out->grad_stage_bytes = gp.stage_bytes; out->grad_smem_bytes = q.gpair_smem;
+    out->grad_smem_end = gp.end; out->grad_staging_bytes = gp.staging_bytes;
+  }
+  out->grad_pair = q.grad_pair;
   return GMCO_OK;
 }
 

@@ -28,7 +28,7 @@ enum : int { PLAN_RUNNING = -1 };
 // without a bound: a wait that does not complete, or a shared-memory / TMEM carve-up that does not fit, is written here,
 // the kernel runs through its normal teardown, and the host turns the word into GMCO_E_CUDA after its next synchronise.
 enum DevErr : int { DEVERR_NONE = 0, DEVERR_WAIT_TIMEOUT = 1, DEVERR_SMEM_LAYOUT = 2, DEVERR_TMEM_LAYOUT = 3 };
-enum DevErrKernel : int { DEVERR_K_DOSE_RESIDENT = 1, DEVERR_K_DOSE_STREAMED = 2, DEVERR_K_DOSE_PAIR = 3, DEVERR_K_GRAD = 4, DEVERR_K_STEP = 5 };
+enum DevErrKernel : int { DEVERR_K_DOSE_RESIDENT = 1, DEVERR_K_DOSE_STREAMED = 2, DEVERR_K_DOSE_PAIR = 3, DEVERR_K_GRAD = 4, DEVERR_K_STEP = 5, DEVERR_K_GRAD_PAIR = 6 };
 enum DevErrWait : int {
   DEVERR_W_EMPTY = 1, DEVERR_W_FULL = 2, DEVERR_W_TG_READY = 3, DEVERR_W_TIN_FULL = 4, DEVERR_W_ACC_FULL = 5,
   DEVERR_W_ACC_EMPTY = 6, DEVERR_W_CONV = 7, DEVERR_W_HISTORY = 8
@@ -103,6 +103,7 @@ struct StepParams {
   const int* tile_seg;                // [n_tiles + 1] slot range of each plan tile (tensor path)
   int compact_cap, total_ctas;        // compaction (tensor path): segment cap per tile and CTAs per grid; 0 = off
   int dose_pair;                      // the objective partials follow the CTA-pair split (kernels_tc.cu compact_remap_pair)
+  int grad_pair;                      // so do the gradient partials (k_grad_tc_pair, gmco_options.dose_kernel = 2)
   int S;
   int ls_cap;                         // > 0: a plan whose FIRST trial step is rejected is queued for the polynomial line search
 };
@@ -163,10 +164,11 @@ int launch_select(const float* dvh, int K, int S, const SelectArgs& c, int* plan
 // tensor path (kernels_tc.cu)
 struct TcPlan;                                   // host-side schedule + tensor maps
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
-                       int wide_accum, cudaStream_t st, char* err, int errlen);
+                       int wide_accum, int want_grad_pair, cudaStream_t st, char* err, int errlen);
 void tc_plan_destroy(TcPlan*);
 int tc_num_segments(const TcPlan*);
 int tc_dose_pair(const TcPlan*);           // 1: the dose kernel runs as CTA pairs (its compaction split is per tile PAIR)
+int tc_grad_pair(const TcPlan*);           // 1: the gradient kernel runs as CTA pairs as well
 int tc_dose_kernel(const TcPlan*);         // tcl::DoseKernelId of the dose kernel that is dispatched
 int tc_choose_segs(int n_tiles, int n_pad_points, int num_sms);
 const int* tc_tile_seg_dev(const TcPlan*);

@@ -118,6 +118,7 @@ __device__ __forceinline__ float reduce_partials(const StepParams& sp, int k, in
       if (sa > sp.compact_cap) sa = sp.compact_cap;
     }
     f0 = (row >> 7) * sa; f1 = f0 + sa;
+    if (sp.grad_pair) { g0 = f0; g1 = f1; }                // k_grad_tc_pair deals its CTA pairs the same way
   } else if (sp.tile_local) { f0 = g0 = sp.tile_seg[k >> 7]; f1 = g1 = sp.tile_seg[(k >> 7) + 1]; prow = k & 127; }
   const int nfe = (f1 - f0) * sp.nFcomp;                   // SIMT: (lo, hi) pairs per slot
   auto f_at = [&](int i) {

@@ -1039,6 +1039,173 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
 }
 
 // ---------------------------------------------------------------------------------------------
+// a5 on tensor cores, CTA-PAIR variant (tcgen05 cta_group::2; gmco_options.dose_kernel = 2, off by default: it has not
+// run on a GPU).  k_grad_tc needs 40 KB of operands per 16-point stage for 768 tensor-pipe cycles = 52 B/clk of a
+// measured 57 B/clk from L2 (profiles/r1_tma_bw.md): it is bound by operand delivery, not by the tensor pipe.  Here
+// the two CTAs of a cluster (2, 1, 1) own two adjacent plan tiles and the same point slabs.  One MMA spans both:
+// M = 256 plans (each CTA's own R tile is its half of the MN-major A operand), N = A_pad dwell positions whose D slab
+// is split between the CTAs by dwell group (each loads G / 2 groups: its half of the MN-major B operand), so a CTA
+// loads 8 + 8 + 8 = 24 KB per stage on C3 instead of 8 + 16 + 16 and the ring holds 6 stages instead of 4.
+// Each CTA's TMEM holds the accumulators of its own 128 plans (main at column 0, corrections at column 256).
+// Barriers: `full` (own CTA: bytes of its R tile and D halves), `conv` (in the leader: 256 arrivals, the converter
+// threads of both CTAs, which have waited for their own `full`), `empty` / `acc_full` (multicast commits).
+__host__ __device__ constexpr uint32_t instr_desc_pair_mn(int n) {   // M = 256, both operands MN-major
+  return (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+}
+
+template <int PS>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmD_hi,
+               const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
+  if (a.gate && *a.gate == 0) return;                 // both CTAs of a pair take every early exit together
+  const int rank = (int)cluster_ctarank();
+  const bool leader = rank == 0;
+  int seg = blockIdx.y, tile = blockIdx.x, segs = a.segs;   // grid (tiles, segs): a 2-CTA MMA pair is adjacent in x
+  if (a.compact_cap && !compact_remap_pair(*a.gate, a.compact_cap, rank, seg, tile, segs)) return;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem0 = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int G = a.A_pad >> 5, Gh = G >> 1;            // dwell groups; this CTA loads groups [rank Gh, rank Gh + Gh)
+  const tcl::GradSmem lay = tcl::grad_pair_smem(PS, G, a.n_stage);
+  if (!layout_fits(a.err, DEVERR_K_GRAD_PAIR, (uint32_t)(smem0 - smem_raw), lay.end, tcl::grad_tmem_cols(a.A_pad))) return;
+  uint8_t* smem = smem0 + lay.ring_off;               // [barriers 1 KB | ring | (epilogue row staging may run past the ring)]
+  constexpr int kRBytes = 4 * PS * 128;               // R part: 4 plan groups x PS points x 128 B
+  const int dBytes = lay.d_bytes;                     // D part: G / 2 dwell groups x PS points x 128 B
+  const int stageBytes = lay.stage_bytes;             // [R | R_lo | D_hi half | D_lo half]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem0);
+  uint64_t* full = bars;                              // [n_stage]  in each CTA: its own TMA bytes
+  uint64_t* empty = bars + a.n_stage;                 // [n_stage]  in each CTA: multicast commit
+  uint64_t* conv = bars + 2 * a.n_stage;              // [n_stage]  used in the leader: 256 arrivals (both CTAs' converters)
+  uint64_t* acc_full = bars + 3 * a.n_stage;          //            in each CTA: multicast commit
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+  const Watch w{a.err, smem_u32(tmem_slot + 1), DEVERR_K_GRAD_PAIR};
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int s0 = (int)((long long)seg * a.n_slabs / segs), s1 = (int)((long long)(seg + 1) * a.n_slabs / segs);
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < a.n_stage; ++i) { mbar_init(full + i, 1); mbar_init(empty + i, 1); mbar_init(conv + i, 256); }
+    mbar_init(acc_full, 1);
+    tmem_slot[1] = 0u;                                // abort flag
+    fence_barrier_init();
+  }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmR); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); }
+  if (warp == 1) tmem_alloc_pair(tmem_slot, 512);
+  tc_fence_before();
+  cluster_sync_all();                                 // barriers of both CTAs exist before anything arrives on them
+  tc_fence_after();
+  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+
+  if (warp == 0) {
+    auto producer = [&]() {
+      const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
+        if (elect_one()) {
+          uint8_t* dst = smem + (size_t)st * stageBytes;
+          mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
+          tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
+          tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, rank * Gh, polD);
+          tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, rank * Gh, polD);
+        }
+        __syncwarp();
+        if (++st == a.n_stage) { st = 0; ph ^= 1; }
+      }
+    };
+    producer();
+  } else if (warp == 1) {
+    auto issuer = [&]() {                             // run by ONE elected lane of the leader
+      if (!leader || s1 <= s0) return;
+      const uint32_t idesc = instr_desc_pair_mn(a.A_pad);
+      constexpr uint32_t dhi = desc_hi(512, kSwz128Base32);
+      const int n_stage = a.n_stage;
+      const uint32_t base_lo = desc_lo(smem_u32(smem), PS * 128), stage_step = (uint32_t)stageBytes >> 4;
+      const uint32_t o_rlo = kRBytes >> 4, o_dhi = (2 * kRBytes) >> 4, o_dlo = (uint32_t)(2 * kRBytes + dBytes) >> 4;
+      const uint32_t empty0 = smem_u32(empty);
+      int st = 0; uint32_t ph = 0;
+      for (int s = s0; s < s1; ++s) {
+        GMCO_WAIT(mbar_wait1_cluster(w, conv + st, ph, DEVERR_W_CONV));
+        tc_fence_after();
+        const uint32_t r = base_lo + (uint32_t)st * stage_step;
+#pragma unroll
+        for (int j = 0; j < PS / 8; ++j) {            // K-steps of 8 points = two 4-row swizzle atoms (1024 B)
+          const uint32_t rh = r + j * 64, rl = rh + o_rlo, dh = rh + o_dhi, dl = rh + o_dlo;
+          const uint32_t first = (s > s0 || j > 0) ? 1u : 0u;
+          mma_ss2_pair(tmem, rh, dhi, dh, dhi, idesc, first);
+          mma_ss2_pair(tmem + 256, rh, dhi, dl, dhi, idesc, first);
+          mma_ss2_pair(tmem + 256, rl, dhi, dh, dhi, idesc, 1);
+        }
+        tc_commit_pair(empty0 + 8 * st);
+        if (s == s1 - 1) tc_commit_pair(smem_u32(acc_full));
+        if (++st == n_stage) { st = 0; ph ^= 1; }
+      }
+    };
+    if (elect_one()) issuer();
+    __syncwarp();
+  } else {
+    const int q = warp & 3;
+    const int L = q * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    auto converter_and_epilogue = [&]() {
+      {
+        const uint32_t l_conv = leader_addr(conv);
+        const int t = threadIdx.x - 64;               // 0..127
+        int st = 0; uint32_t ph = 0;
+        for (int s = s0; s < s1; ++s) {
+          GMCO_WAIT(mbar_wait(w, full + st, ph, DEVERR_W_FULL));   // this CTA's R tile AND its D halves have landed
+          uint8_t* base = smem + (size_t)st * stageBytes + t * 16;
+#pragma unroll
+          for (int i = 0; i < kRBytes / 2048; ++i) {
+            const float4 v = *reinterpret_cast<const float4*>(base + i * 2048);
+            float4 hi, lo;
+            hi.x = __uint_as_float(__float_as_uint(v.x) & 0xffffe000u); lo.x = v.x - hi.x;
+            hi.y = __uint_as_float(__float_as_uint(v.y) & 0xffffe000u); lo.y = v.y - hi.y;
+            hi.z = __uint_as_float(__float_as_uint(v.z) & 0xffffe000u); lo.z = v.z - hi.z;
+            hi.w = __uint_as_float(__float_as_uint(v.w) & 0xffffe000u); lo.w = v.w - hi.w;
+            *reinterpret_cast<float4*>(base + i * 2048) = hi;
+            *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
+          }
+          fence_proxy_async();
+          mbar_arrive_cluster(l_conv + 8u * (uint32_t)st);         // releasing arrive at cluster scope
+          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        }
+      }
+      float* grow = a.Gpart + (((size_t)tile * segs + seg) * 128 + L) * a.A_pad;
+      if (s1 > s0) {
+        GMCO_WAIT(mbar_wait(w, acc_full, 0, DEVERR_W_ACC_FULL));
+        tc_fence_after();
+        float* srow = reinterpret_cast<float*>(smem) + (size_t)L * (a.A_pad + 4);
+        for (int g = 0; g < G; ++g) {
+          uint32_t v[32], vc[32];
+          tmem_ld32(tmem + lane_base + g * 32, v);
+          tmem_ld32(tmem + lane_base + 256 + g * 32, vc);
+          tmem_ld_wait();
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = __float_as_uint(__uint_as_float(v[j]) + __uint_as_float(vc[j]));
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            *reinterpret_cast<float4*>(srow + g * 32 + 4 * i) =
+                make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]), __uint_as_float(v[4 * i + 2]),
+                            __uint_as_float(v[4 * i + 3]));
+        }
+        fence_proxy_async();
+        bulk_store(grow, srow, (uint32_t)a.A_pad * 4u);
+        bulk_commit_group();
+        bulk_wait_group_read0();
+      } else {
+        float4* dst = reinterpret_cast<float4*>(grow);
+        for (int i = 0; i < a.A_pad / 4; ++i) dst[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    };
+    converter_and_epilogue();
+  }
+  tc_fence_before();
+  if (warp == 1) drain_if_aborted(w.abort_addr);
+  cluster_sync_all();                                 // neither CTA's shared memory, TMEM or barriers may go before both are done
+  if (warp == 1) { tc_fence_after(); tmem_dealloc_pair(tmem, 512); }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 PFN_cuTensorMapEncodeTiled get_encode() {
   static PFN_cuTensorMapEncodeTiled fn = nullptr;
@@ -1073,6 +1240,7 @@ struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
   CUtensorMap pair_D_hi, pair_D_lo;                // 64-point boxes of the CTA-pair dose kernel
+  CUtensorMap gpair_D_hi, gpair_D_lo;              // G / 2 dwell groups per box: the CTA-pair gradient kernel
   tcl::Schedule sch{};                             // every size the host chose (tc_layout.h)
   int* tile_seg_dev = nullptr;
   Thresholds thr{};
@@ -1091,15 +1259,16 @@ static cudaError_t tc_set_smem_caps() {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc_pair<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   done = e;
   return e;
 }
 
 TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh, int num_sms, int force_single,
-                       int wide_accum, cudaStream_t st, char* err, int errlen) {
+                       int wide_accum, int want_grad_pair, cudaStream_t st, char* err, int errlen) {
   if (c.A_pad > kMaxApadTensor) { snprintf(err, errlen, "tensor path supports n_dwell <= 384"); return nullptr; }
   TcPlan* t = new TcPlan();
-  t->sch = tcl::choose_schedule(c.A_pad, c.N_pad, p.K_pad, num_sms, force_single, wide_accum);
+  t->sch = tcl::choose_schedule(c.A_pad, c.N_pad, p.K_pad, num_sms, force_single, wide_accum, want_grad_pair);
   const tcl::Schedule& q = t->sch;
   if (!q.ok) { snprintf(err, errlen, "shared memory too small for the tensor kernels' rings at this shape"); delete t; return nullptr; }
   for (int s = 0; s < c.S; ++s) { t->thr.d_lo[s] = sh[s].d_lo; t->thr.d_hi[s] = sh[s].d_hi; }
@@ -1115,6 +1284,9 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
   if (q.dose_pair)
     ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
          make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
+  if (q.grad_pair)
+    ok = ok && make_map(&t->gpair_D_hi, c.D_hi, c.N_alloc, c.A_pad, q.grad_ps, G / 2, sMN) &&
+         make_map(&t->gpair_D_lo, c.D_lo, c.N_alloc, c.A_pad, q.grad_ps, G / 2, sMN);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
   if (q.tlo_resident) t->dose_T_lo = t->dose_T;   // the resident layout splits T in the kernel; the map is never used for a load
   cudaError_t e = tc_set_smem_caps();
@@ -1133,6 +1305,7 @@ void tc_plan_destroy(TcPlan* t) {
 
 int tc_num_segments(const TcPlan* t) { return t->sch.n_tiles * t->sch.segs; }
 int tc_dose_pair(const TcPlan* t) { return t->sch.dose_pair; }
+int tc_grad_pair(const TcPlan* t) { return t->sch.grad_pair; }
 int tc_dose_kernel(const TcPlan* t) { return t->sch.dose_kernel; }
 const int* tc_tile_seg_dev(const TcPlan* t) { return t->tile_seg_dev; }
 
@@ -1171,7 +1344,12 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
     GradArgs ga{};
     ga.Gpart = p.Gpart; ga.gate = gate; ga.A_pad = c.A_pad; ga.n_slabs = q.n_slabs; ga.segs = q.segs;
     ga.n_stage = q.grad_stages; ga.compact_cap = cap; ga.err = p.dev_err;
-    k_grad_tc<16><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+    if (q.grad_pair) {
+      ga.n_stage = q.gpair_stages;
+      k_grad_tc_pair<16><<<dim3(q.n_tiles, q.segs), kThreads, q.gpair_smem, st>>>(t->grad_R, t->gpair_D_hi, t->gpair_D_lo, ga);
+    } else {
+      k_grad_tc<16><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+    }
     if (cudaGetLastError() != cudaSuccess) return -1;
     ++n;
   }

@@ -109,6 +109,22 @@ GMCO_HD GradSmem grad_smem(int PS, int G, int n_stage) {
 }
 GMCO_HD int grad_tmem_cols(int A_pad) { return A_pad <= 256 ? 256 + A_pad : A_pad; }
 
+// ---- k_grad_tc_pair<PS> (gmco_options.dose_kernel = 2; at most 256 dwell positions, even tile and group counts) ------
+// Two CTAs of a cluster own two adjacent plan tiles and the same point slabs; each loads its own R tile and HALF of the
+// dwell groups of every D slab, so a stage is [R | R_lo | D_hi half | D_lo half].
+GMCO_HD GradSmem grad_pair_smem(int PS, int G, int n_stage) {
+  GradSmem s;
+  s.r_bytes = 4 * PS * 128;
+  s.d_bytes = (G / 2) * PS * 128;
+  s.stage_bytes = 2 * s.r_bytes + 2 * s.d_bytes;
+  s.ring_off = kGradBarBytes;
+  s.ring_bytes = n_stage * s.stage_bytes;
+  s.n_bars = 3 * n_stage + 1;
+  s.staging_bytes = 128 * (G * 32 + 4) * 4;
+  s.end = s.ring_off + (s.ring_bytes > s.staging_bytes ? s.ring_bytes : s.staging_bytes);
+  return s;
+}
+
 // ---- host-side schedule -------------------------------------------------------------------------------------------------
 // Point segments per plan tile.  Up to num_sms / n_tiles the grid is one wave of CTAs.  With many tiles one wave leaves
 // SMs idle (79 tiles of a 10 000-plan pool: 79 of 148) or unevenly loaded (C4: 32 tiles x 4 = 128 CTAs), so the grid
@@ -136,13 +152,16 @@ struct Schedule {
   int dose_tmem_groups, dose_n_main;   // streamed layout only: 4 groups of T_hi in TMEM and two main accumulators when wide_accum is on
   int dose_pair, pair_static, pair_stages, pair_smem;
   int grad_ps, grad_stages, grad_smem, n_slabs;
+  int grad_pair, gpair_stages, gpair_smem;   // CTA-pair gradient kernel (option): ring depth and launched bytes
   int dose_kernel;         // DoseKernelId of the kernel that launch_tc_eval dispatches
 };
 
 // Every size the host chooses for a case of A_pad dwell columns, N_pad padded points and K_pad padded plans.
 // force_single != 0 keeps the single-CTA dose kernel where the CTA-pair kernel would be eligible.  wide_accum != 0
 // selects the split-main layout for the streamed dose kernel (more than 256 dwell positions).
-inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, int force_single, int wide_accum = 0) {
+// want_grad_pair != 0 (gmco_options.dose_kernel = 2) also runs the gradient contraction on CTA pairs where the shape allows.
+inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, int force_single, int wide_accum = 0,
+                                int want_grad_pair = 0) {
   Schedule t{};
   t.G = A_pad / 32;
   t.n_tiles = K_pad / 128;
@@ -186,6 +205,16 @@ inline Schedule choose_schedule(int A_pad, int N_pad, int K_pad, int num_sms, in
     // static issue schedule for the production shape (A_pad 193..256: 12 entries per chunk, ring of 6)
     t.pair_static = ((G + 1) / 2 == 4 && t.pair_stages >= 6) ? 1 : 0;
     if (t.pair_static) { t.pair_stages = 6; t.pair_smem = fixedp + 6 * kPairEntry; }
+  }
+  // CTA-pair gradient kernel: the split of D over the pair is by dwell group, so their number must be even; the
+  // accumulator pair (main + corrections) needs A_pad <= 256; the CTA split must be the dose kernel's (k_step reads both)
+  t.grad_pair = (want_grad_pair && t.dose_pair && G % 2 == 0 && A_pad <= 256) ? 1 : 0;
+  if (t.grad_pair) {
+    const GradSmem probe = grad_pair_smem(t.grad_ps, G, 0);
+    t.gpair_stages = (kSmemMax - 2 * kGradBarBytes) / probe.stage_bytes;
+    if (t.gpair_stages > kGradMaxStages) t.gpair_stages = kGradMaxStages;
+    if (t.gpair_stages < 2) t.grad_pair = 0;
+    else t.gpair_smem = kAlign + grad_pair_smem(t.grad_ps, G, t.gpair_stages).end;
   }
   t.dose_kernel = t.dose_pair ? (t.pair_static ? kDosePairStatic : kDosePairRing)
                               : (t.tlo_resident ? kDoseResident : kDoseStreamed);

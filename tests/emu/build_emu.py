@@ -106,7 +106,7 @@ def _build(force: bool, sanitize: bool) -> Path:
 # name -> (file, text to find, replacement, occurrences expected)
 MUTANTS = {
     # producer refills a ring slot without waiting for the commit of the MMAs that read it
-    "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));", "", 3),
+    "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));", "", 4),
     # MMAs issued before the TMA bytes of their operands have landed
     "issuer_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));", "", 2),
     # gradient MMAs issued before the converter warps have split the R tile (and before it has landed)
@@ -123,13 +123,17 @@ MUTANTS = {
     # ... and the same with the self-check gone: the emulated hardware's window check is what is left
     "host_smem_too_small_unchecked": ("*", None, None, 0),
     # producer's ring phase never flips: the second trip round the ring waits for ever -> bounded wait -> error word
-    "producer_phase_never_flips": ("kernels_tc.cu", "if (++st == a.n_stage) { st = 0; ph ^= 1; }", "if (++st == a.n_stage) { st = 0; }", 4),
+    "producer_phase_never_flips": ("kernels_tc.cu", "if (++st == a.n_stage) { st = 0; ph ^= 1; }", "if (++st == a.n_stage) { st = 0; }", 6),
     # TMEM is never given back
     "tmem_never_freed": ("kernels_tc.cu", "tc_fence_after(); tmem_dealloc(tmem, 512); }", "tc_fence_after(); }", 2),
     # the D slab of the wrong chunk is loaded (index error: wrong numbers, nothing else)
     "wrong_chunk_loaded": ("kernels_tc.cu", "tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, c * kPC, g, polD);", "tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, (c + (c & 1)) * kPC, g, polD);", 1),
     # a K-step of the main product uses the wrong 32 B of the swizzled row
     "wrong_k_step_descriptor": ("kernels_tc.cu", "mma_ts2(acc, thi + 8 * j, bd + 2 * j, dhi, idesc, 1);", "mma_ts2(acc, thi + 8 * j, bd + 2 * (j ^ 1), dhi, idesc, 1);", 1),
+    # pair gradient kernel: the converters split the R tile without waiting for it (and the D halves) to land
+    "gpair_converter_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, full + st, ph, DEVERR_W_FULL));   // this CTA's R tile AND its D halves have landed", "", 1),
+    # pair gradient kernel: the peer CTA loads the leader's half of the dwell groups (index error)
+    "gpair_peer_loads_wrong_half": ("kernels_tc.cu", "tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, rank * Gh, polD);", "tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);", 1),
     # k_step pushes the history pair without waiting for the staged copies it overwrites
     "step_skips_history_wait": ("kernels_lbfgs.cu", "      hist_wait();                                           // the staged copy of slot hh is about to be replaced\n", "", 1),
 }

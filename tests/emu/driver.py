@@ -99,7 +99,7 @@ def sc_evaluate(g, E, a):
     return report(E, errors=eval_errors(out, ref), schedule={k: int(v) for k, v in sched.items()},
                   digest=digest(out["dose"], out["F"], out["grad_x"]),
                   kernels={k: int(E.emu_counter(k.encode())) for k in ("k_dose_tc<true>", "k_dose_tc<false>", "k_dose_tc<false, true>",
-                                                                       "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16>", "k_simt_dose", "k_simt_grad")})
+                                                                       "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16>", "k_grad_tc_pair<16>", "k_simt_dose", "k_simt_grad")})
 
 
 def sc_optimize(g, E, a):
@@ -127,7 +127,8 @@ def sc_optimize(g, E, a):
                   status_gpu=out["plan_status"].tolist(), status_ref=np.asarray(ref["status"]).tolist(),
                   rounds=int(st["rounds"]), launches=int(st["kernel_launches"]), executed=executed, dose_kernel=int(st["dose_kernel"]),
                   digest=digest(out["T"], out["objective"], out["dvh"]),
-                  ls_launches=int(E.emu_counter(b"k_ls_pick")), step_launches=int(E.emu_counter(b"k_step")))
+                  ls_launches=int(E.emu_counter(b"k_ls_pick")), step_launches=int(E.emu_counter(b"k_step")),
+                  grad_pair_launches=int(E.emu_counter(b"k_grad_tc_pair")))
 
 
 def sc_fault(g, E, a):

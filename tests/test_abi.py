@@ -46,7 +46,7 @@ def test_version_and_default_options(built_lib):
 def test_struct_layouts_match_the_header(built_lib):
     import paper_1904_01567_b200.binding as b
     assert ctypes.sizeof(b._Structure) == 28 and ctypes.sizeof(b.Options) == 40 and ctypes.sizeof(b.Stats) == 56
-    assert ctypes.sizeof(b.TcInfo) == 30 * 4
+    assert ctypes.sizeof(b.TcInfo) == 31 * 4
     assert ctypes.sizeof(b.Criterion) == 20
 
 
@@ -67,7 +67,7 @@ def test_argument_errors_are_reported_without_a_gpu(built_lib):
         g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(compaction=2))
     assert e.value.code == -1 and "options" in str(e.value)
     with pytest.raises(g.GmcoError) as e:
-        g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(dose_kernel=2))
+        g.gmco_create(c.D, c.structures, c.rx, g.binding.make_options(dose_kernel=3))
     assert e.value.code == -1 and "options" in str(e.value)
     with pytest.raises(g.GmcoError) as e:
         g.gmco_create(np.zeros((8, 500), np.float32), [gc.Structure("s", 8, 1, 2, 1, 1, 0, 0)], 15.0)

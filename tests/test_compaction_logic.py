@@ -32,8 +32,9 @@ def remap_pair(gx, gy, bx, by, n_running, cap):
     return (pt < tap), 2 * pt + rank, c - pt * sa, sa
 
 
-def reader_range(total_ctas, cap, n_running, row, pair):
-    """reduce_partials: slot range [f0, f1) of the objective partials and [g0, g1) of the gradient partials."""
+def reader_range(total_ctas, cap, n_running, row, pair, grad_pair=False):
+    """reduce_partials: slot range [f0, f1) of the objective partials and [g0, g1) of the gradient partials
+    (grad_pair: k_grad_tc_pair deals its CTA pairs like the dose pair kernel, gmco_options.dose_kernel = 2)."""
     ta = (n_running + 127) >> 7
     sa = min(total_ctas // ta, cap)
     g0 = (row >> 7) * sa
@@ -41,6 +42,8 @@ def reader_range(total_ctas, cap, n_running, row, pair):
     if pair:
         sa = min((total_ctas >> 1) // ((ta + 1) >> 1), cap)
     f0 = (row >> 7) * sa
+    if grad_pair:
+        g = (f0, f0 + sa)
     return (f0, f0 + sa), g
 
 
@@ -88,6 +91,8 @@ def test_pair_remap_keeps_pairs_together_and_matches_the_reader(tiles, segs):
         for row in range(0, n_running, 53):
             f, _ = reader_range(tiles * segs, cap, n_running, row, pair=True)
             assert sorted(t * sa + s for (t, s) in owners if t == row >> 7) == list(range(*f))
+            f2, g2 = reader_range(tiles * segs, cap, n_running, row, pair=True, grad_pair=True)
+            assert f2 == f and g2 == f                                   # the pair gradient kernel writes the same slots
 
 
 @pytest.mark.parametrize("n_chunks,segs", [(12, 148), (94, 18), (94, 36), (94, 5), (313, 9), (47, 74), (1, 3)])

@@ -48,6 +48,16 @@ SCENARIOS = {
     "streamed_384": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, **SMALL),
     "wide_accum_384": dict(scenario="evaluate", sm_count=2, n_plans=128, n_cath=24, n_pos=16, wide_accum=1, **SMALL),
     "wide_accum_352_3_tiles": dict(scenario="evaluate", sm_count=6, n_plans=300, n_cath=22, n_pos=16, wide_accum=1, **SMALL),
+    # gmco_options.dose_kernel = 2: the gradient contraction on CTA pairs as well (k_grad_tc_pair, off by default)
+    "gpair_ring": dict(scenario="evaluate", sm_count=4, n_plans=256, dose_kernel=2, **SMALL),
+    "gpair_static": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, **SMALL),
+    "gpair_static_4_tiles_ragged": dict(scenario="evaluate", sm_count=8, n_plans=500, n_cath=17, n_pos=14, dose_kernel=2, counts=[333, 77, 129, 65]),
+    "gpair_odd_groups_falls_back": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=14, n_pos=16, dose_kernel=2, **SMALL),
+    "gpair_static@slow_pipe": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, seed=3, max_delay=20, mma_delay=20000, **SMALL),
+    "gpair_static@slow_copies": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, seed=4, max_delay=20000, mma_delay=1, dyn_misalign=0, **SMALL),
+    "gpair_static@starved_issuer": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, starve_mask=2, starve_period=40, **SMALL),
+    "gpair_static@starved_converters": dict(scenario="evaluate", sm_count=4, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, starve_mask=60, starve_period=40, **SMALL),
+    "c3_full_size_gpair": dict(scenario="evaluate", case="C3", dose_kernel=2),
     # BASELINE.json configs[2] at FULL size in the launch configuration bench.py times (148 SMs: 8 plan tiles x 18 segments,
     # k_dose_tc_pair<4, 6> with 5-6 chunks per CTA): all 12000 x 1000 doses, F and the gradient of all 1000 plans (~70 s)
     "c3_full_size": dict(scenario="evaluate", case="C3"),
@@ -75,6 +85,8 @@ SCENARIOS = {
     "opt_no_compaction": dict(scenario="optimize", sm_count=4, iters=20, compaction=0),
     "opt_simt": dict(scenario="optimize", sm_count=4, iters=20, precision=1),
     "opt_eps_pair_compaction": dict(scenario="optimize", sm_count=4, n_plans=256, eps=1e-3, iters=30, **SMALL),
+    "opt_eps_gpair_compaction": dict(scenario="optimize", sm_count=4, n_plans=256, eps=1e-3, iters=30, dose_kernel=2, **SMALL),
+    "opt_gpair_no_compaction": dict(scenario="optimize", sm_count=4, n_plans=256, iters=10, dose_kernel=2, compaction=0, **SMALL),
     "opt_line_search": dict(scenario="optimize", sm_count=4, iters=30, line_search=1),
     "opt_streamed_wide": dict(scenario="optimize", sm_count=2, n_plans=6, n_cath=24, n_pos=16, iters=8, wide_accum=1, counts=[300, 60, 70, 70]),
     # ---- lost completions ----
@@ -89,6 +101,8 @@ SCENARIOS = {
     "sweep_commit_streamed": dict(scenario="fault_sweep", drop="drop_commit", count=40, sm_count=2, n_plans=128, n_cath=24, n_pos=16, counts=[300, 60, 70, 70]),
     "sweep_tma_pair": dict(scenario="fault_sweep", drop="drop_tma", count=40, sm_count=2, n_plans=256, n_cath=18, n_pos=14, counts=[300, 60, 70, 70]),
     "sweep_commit_pair": dict(scenario="fault_sweep", drop="drop_commit", count=40, sm_count=2, n_plans=256, n_cath=18, n_pos=14, counts=[300, 60, 70, 70]),
+    "sweep_tma_both_pair_kernels": dict(scenario="fault_sweep", drop="drop_tma", count=40, stride=9, sm_count=2, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, counts=[300, 60, 70, 70]),
+    "sweep_commit_both_pair_kernels": dict(scenario="fault_sweep", drop="drop_commit", count=40, stride=2, sm_count=2, n_plans=256, n_cath=18, n_pos=14, dose_kernel=2, counts=[300, 60, 70, 70]),
     "sweep_tma_resident_and_grad": dict(scenario="fault_sweep", drop="drop_tma", count=40, stride=2, sm_count=2),
     "sweep_commit_resident_and_grad": dict(scenario="fault_sweep", drop="drop_commit", count=40, stride=2, sm_count=2),
     # a lost history copy of k_step inside the device-side loop
@@ -117,7 +131,7 @@ def results():
             return name, dict(crashed=True, returncode=p.returncode, stderr=p.stderr[-2000:])
         return name, json.loads(line[-1][len("EMU_RESULT "):])
 
-    order = sorted(SCENARIOS.items(), key=lambda kv: kv[0] != "c3_full_size")      # the long one first: it overlaps the rest
+    order = sorted(SCENARIOS.items(), key=lambda kv: not kv[0].startswith("c3_full_size"))      # the long one first: it overlaps the rest
     with ThreadPoolExecutor(max_workers=8) as ex:
         return dict(ex.map(run, order))
 
@@ -153,6 +167,28 @@ def test_every_dose_kernel_and_the_multi_chunk_paths_were_reached(results):
             assert r["kernels"]["k_grad_tc<16>"] == 1 and r["mma"] > 0 and r["tma"] > 0, name
             q = r["schedule"]
             assert q["n_chunks"] // q["segs"] >= 3, (name, q["n_chunks"], q["segs"])      # ring wrap-around, buffer alternation
+
+
+def test_pair_gradient_kernel_option(results):
+    """gmco_options.dose_kernel = 2 (k_grad_tc_pair): same numbers as k_grad_tc to the last bit where both
+    sum in the same order (no compaction), reached on the shapes it is meant for, falls back where the shape forbids it."""
+    for name in ("gpair_ring", "gpair_static", "gpair_static_4_tiles_ragged", "c3_full_size_gpair"):
+        r = _ok(results, name)
+        assert r["kernels"]["k_grad_tc_pair<16>"] == 1 and r["kernels"]["k_grad_tc<16>"] == 0 and r["schedule"]["grad_pair"] == 1, name
+    r = _ok(results, "gpair_odd_groups_falls_back")               # 7 dwell groups: the split of D by group needs an even count
+    assert r["kernels"]["k_grad_tc<16>"] == 1 and r["kernels"]["k_grad_tc_pair<16>"] == 0 and r["schedule"]["grad_pair"] == 0
+    assert _ok(results, "gpair_static")["digest"] == _ok(results, "pair_static")["digest"]
+    assert _ok(results, "gpair_ring")["digest"] == _ok(results, "pair_ring")["digest"]
+    assert _ok(results, "c3_full_size_gpair")["digest"] == _ok(results, "c3_full_size")["digest"]
+    for v in [n for n in SCENARIOS if n.startswith("gpair_static@")]:
+        assert _ok(results, v)["digest"] == _ok(results, "gpair_static")["digest"], v
+    q = _ok(results, "c3_full_size_gpair")["schedule"]
+    assert (q["grad_stages"], q["grad_stage_bytes"]) == (6, 32768) or q["grad_stages"] == 7     # 24 KB loaded + 8 KB R_lo per stage
+    r = _ok(results, "opt_eps_gpair_compaction")
+    assert r["grad_pair_launches"] >= 30 and r["status_gpu"] == r["status_ref"] and r["rel_F_same_iters_max"] < TOL_F_FINAL
+    assert r["launches"] == r["executed"]
+    r = _ok(results, "opt_gpair_no_compaction")
+    assert r["iters_gpu"] == r["iters_ref"] and r["rel_F_max"] < TOL_F_FINAL and r["dvh_pp_max"] < TOL_DVH_PP and r["grad_pair_launches"] >= 11
 
 
 def test_c3_runs_in_the_configuration_the_bench_times(results):
@@ -227,6 +263,8 @@ def test_no_lost_completion_anywhere_can_hang_or_corrupt(results, name):
     r = _ok(results, name)                                     # 40 faults in a row on one handle: no hazard, no hang, nothing leaks
     assert r["wrong"] == 0, r                                  # never a silently wrong result
     assert r["contained"] + r["harmless"] == 40 and r["contained"] >= 20, r
+    if "both_pair" in name:
+        assert any("k_grad_tc_pair" in k for k in r["sites"]) and any("k_dose_tc_pair" in k for k in r["sites"]), r["sites"]
     assert all(k.startswith("k_") and "wait:" in k for k in r["sites"]), r["sites"]
     e = r["errors_after"]
     assert e["dose"] < TOL_EVAL and e["F"] < TOL_EVAL and e["grad"] < TOL_EVAL

@@ -95,6 +95,7 @@ scenario("c1_simt_profile", c1, b.make_options(m=c1.m, precision=1), profile=Tru
 pair = gc.make_case("C1", n_plans=256)
 scenario("pair_ring", pair, b.make_options(m=pair.m))
 scenario("pair_forced_single", pair, b.make_options(m=pair.m, dose_kernel=1))
+scenario("pair_both_contractions", pair, b.make_options(m=pair.m, dose_kernel=2))
 wide = gc.make_case("C1", n_cath=24, n_pos=16, counts=(700, 130, 250, 190), n_plans=130, seed_points=9)
 scenario("wide_streamed", wide, b.make_options(m=wide.m, eps=1e-3, compaction=0))
 scenario("wide_split_main", wide, b.make_options(m=wide.m, wide_accum=1))
@@ -228,7 +229,7 @@ def test_every_launch_is_the_one_the_schedule_announces(report):
     cases = {"c1_tf32": (gc.make_case("C1"), 0, 0), "pair_ring": (gc.make_case("C1", n_plans=256), 0, 0),
              "pair_forced_single": (gc.make_case("C1", n_plans=256), 1, 0),
              "wide_streamed": (wide, 0, 0), "wide_split_main": (wide, 0, 1),
-             "c3_pair_static": (gc.make_case("C3"), 0, 0)}
+             "c3_pair_static": (gc.make_case("C3"), 0, 0), "pair_both_contractions": (gc.make_case("C1", n_plans=256), 2, 0)}
     names = {0: "k_dose_tcILb1ELb0", 1: "k_dose_tcILb0ELb0", 2: "k_dose_tc_pairILi4ELi6", 3: "k_dose_tc_pairILi0ELi0"}
     for tag, (c, dk, wa) in cases.items():
         q = g.gmco_tc_schedule(c.n_dwell, [s.n_points for s in c.structures], c.n_plans, 148, dk, wa)
@@ -237,8 +238,15 @@ def test_every_launch_is_the_one_the_schedule_announces(report):
         dose = _one(rep, names[q["dose_kernel"]])
         grid = [q["n_tiles"], q["segs"], 1] if q["dose_kernel"] >= 2 else [q["segs"], q["n_tiles"], 1]
         assert dose["grid"] == grid and dose["block"] == [320, 1, 1] and dose["smem"] == q["dose_smem_bytes"], tag
-        grad = _one(rep, "k_grad_tc")
-        assert grad["grid"] == [q["segs"], q["n_tiles"], 1] and grad["block"] == [192, 1, 1] and grad["smem"] == q["grad_smem_bytes"], tag
+        if q["grad_pair"]:                 # gmco_options.dose_kernel = 2: CTA pairs for the gradient contraction as well
+            grad = _one(rep, "k_grad_tc_pair")
+            assert grad["grid"] == [q["n_tiles"], q["segs"], 1], tag     # (the scenario's later 128-plan call has one tile: k_grad_tc)
+            first_grad = [x for x in rep["launches"] if "k_grad_tc" in x["name"]][0]
+            assert "k_grad_tc_pair" in first_grad["name"], tag
+        else:
+            grad = _one(rep, "k_grad_tcILi16")
+            assert grad["grid"] == [q["segs"], q["n_tiles"], 1], tag
+        assert grad["block"] == [192, 1, 1] and grad["smem"] == q["grad_smem_bytes"], tag
         # the same kernels inside the captured loop body
         assert _one(rep, names[q["dose_kernel"]], captured=1)["smem"] == q["dose_smem_bytes"]
         assert _one(rep, "k_step", captured=1) and _one(rep, "k_loop_cond", captured=1)

@@ -28,7 +28,7 @@ def _shapes():
             yield a, tiles
 
 
-@pytest.mark.parametrize("dose_kernel,wide_accum", [(0, 0), (1, 0), (0, 1)])
+@pytest.mark.parametrize("dose_kernel,wide_accum", [(0, 0), (1, 0), (0, 1), (2, 0)])
 def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel, wide_accum):
     n = 0
     for a, tiles in _shapes():
@@ -48,7 +48,7 @@ def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel, wi
             # ring entries hold their TMA boxes; every operand area starts 1024-aligned (SWIZZLE_128B atoms)
             assert q["dose_stages"] >= 2 and q["grad_stages"] >= 2
             if q["dose_kernel"] in (2, 3):
-                assert tiles % 2 == 0 and G <= 8 and dose_kernel == 0             # any dwell-group count, odd ones included
+                assert tiles % 2 == 0 and G <= 8 and dose_kernel in (0, 2)        # any dwell-group count, odd ones included
                 assert q["dose_stage_bytes"] == K_PAIR_ENTRY == 32 * 4 * 64 * 2       # box {32 dwell, 64 points, 2 groups}
                 assert q["dose_tmem_cols"] == 32 * G + 256
                 if q["dose_kernel"] == 2:
@@ -64,7 +64,13 @@ def test_every_shape_fits_shared_memory_tmem_and_the_allocations(dose_kernel, wi
             if q["dose_kernel"] != 1:
                 assert (q["dose_tmem_groups"], q["dose_n_main"]) == (8, 1)            # wide_accum touches the streamed layout only
             assert q["dose_stage_bytes"] % 1024 == 0 and q["grad_stage_bytes"] % 1024 == 0
-            assert q["grad_stage_bytes"] == 2 * 4 * q["grad_ps"] * 128 + 2 * G * q["grad_ps"] * 128
+            if q["grad_pair"]:     # k_grad_tc_pair: each CTA holds its R tile and HALF of the dwell groups of a D slab
+                assert dose_kernel == 2 and q["dose_kernel"] in (2, 3) and G % 2 == 0 and q["a_pad"] <= 256 and tiles % 2 == 0
+                assert q["grad_stage_bytes"] == 2 * 4 * q["grad_ps"] * 128 + 2 * (G // 2) * q["grad_ps"] * 128
+                assert q["grad_tmem_cols"] == 256 + q["a_pad"] <= 512
+            else:
+                assert dose_kernel != 2 or not (q["dose_kernel"] in (2, 3) and G % 2 == 0)
+                assert q["grad_stage_bytes"] == 2 * 4 * q["grad_ps"] * 128 + 2 * G * q["grad_ps"] * 128
             # TMA boxes stay inside the global allocations (rows of D / R: n_alloc; rows of T: k_pad)
             assert q["n_chunks"] * 128 <= q["n_alloc"] and q["n_chunks"] == (q["n_pad"] + 127) // 128
             assert q["n_slabs"] * q["grad_ps"] == q["n_pad"] <= q["n_alloc"]
