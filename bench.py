@@ -217,6 +217,7 @@ def workload_config(case, args, stats):
     cfg["compaction"] = getattr(args, "compaction", 1)
     cfg["line_search"] = getattr(args, "line_search", 0)
     cfg["wide_accum"] = getattr(args, "wide_accum", 0)
+    cfg["dose_kernel_option"] = getattr(args, "dose_kernel", 0)
     if stats:
         cfg["rounds"] = stats["rounds"]
         cfg["device_bytes"] = stats["device_bytes"]
@@ -235,7 +236,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=256, help="plans per oracle step (bounded sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-peak", action="store_true", help="skip the live tf32 matmul peak measurement (roofline falls back to the nominal ratio)")
-    ap.add_argument("--dose-kernel", type=int, default=0, choices=[0, 1], help="gmco_options.dose_kernel (1 = keep the single-CTA dose kernel)")
+    ap.add_argument("--dose-kernel", type=int, default=0, choices=[0, 1, 2], help="gmco_options.dose_kernel (1 = keep the single-CTA dose kernel; 2 = CTA pairs for the gradient contraction as well, an option that is off by default)")
     ap.add_argument("--line-search", type=int, default=0, choices=[0, 1], help="gmco_options.line_search (1 = polynomial line search, an option that is off by default)")
     ap.add_argument("--wide-accum", type=int, default=0, choices=[0, 1], help="gmco_options.wide_accum (1 = split main accumulator above 256 dwell positions)")
     ap.add_argument("--no-gsa", action="store_true", help="skip the gSA-vs-gL-BFGS comparison leg (C5)")
