@@ -297,18 +297,17 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
   constexpr uint32_t corr_off = (uint32_t)n_main * kPC;        // column offset of the correction accumulator
 
   if (warp == 0) {
-    // whole warp walks the ring (uniform control flow); one elected lane issues
+    // run by ONE elected lane, like the issue loop: per ring entry one poll, expect_tx and the TMA loads
     auto producer = [&]() {
       if (c1 <= c0) return;
       const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
       if (kResident) {                         // fp32 T of the tile lands where its lo part will live
-        if (elect_one()) {
+        {
           for (int g = 0; g < G; ++g) {
             mbar_expect_tx(tin_full + g, (uint32_t)kTloBox);
             tma_load_3d(&tmT, tlo + (size_t)g * kTloBox, tin_full + g, 0, tile * 128, g, polT);
           }
         }
-        __syncwarp();
       }
       int st = 0; uint32_t ph = 0;
       bool scratch_busy = !kResident;          // resident mode transposes through the T_lo area itself
@@ -316,23 +315,23 @@ k_dose_tc(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant__ CU
         for (int g2 = 0; g2 < 2 * G; ++g2) {          // entry 2 g: D_hi (+ streamed T_lo), entry 2 g + 1: D_lo
           const int g = g2 >> 1, lo = g2 & 1;
           if (scratch_busy && st >= scr_slot) {       // the prologue's transposition scratch overlaps these slots
-            for (int i = 0; i < G; ++i) GMCO_WAIT(mbar_wait(w, tg_ready + i, 0, DEVERR_W_TG_READY));
+            for (int i = 0; i < G; ++i) GMCO_WAIT(mbar_wait1_addr(w, smem_u32(tg_ready + i), 0, DEVERR_W_TG_READY));
             scratch_busy = false;
           }
-          GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
-          if (elect_one()) {
+          GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));
+          {
             uint8_t* dst = ring + (size_t)st * stageBytes;
             const bool with_t = !lo && !kResident;
             mbar_expect_tx(full + st, (uint32_t)(with_t ? kSlabBytes + kTloBox : kSlabBytes));
             tma_load_3d(lo ? &tmD_lo : &tmD_hi, dst, full + st, 0, c * kPC, g, polD);
             if (with_t) tma_load_3d(&tmT_lo, dst + kSlabBytes, full + st, 0, tile * 128, g, polT);
           }
-          __syncwarp();
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
         }
       }
     };
-    producer();
+    if (elect_one()) producer();                      // one lane issues every TMA load of the CTA
+    __syncwarp();
   } else if (warp == 1) {
     auto issuer = [&]() {
       if (c1 <= c0) return;
@@ -647,30 +646,33 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
     auto producer = [&]() {
       if (c1 <= c0) return;
       const uint64_t polD = l2_evict_last(), polT = l2_evict_normal();
-      if (elect_one()) {
+      {
         for (int g = 0; g < G; ++g) {
           mbar_expect_tx(tin_full + g, (uint32_t)kTloBox);
           tma_load_3d(&tmT, tlo + (size_t)g * kTloBox, tin_full + g, 0, tile * 128, g, polT);
         }
       }
-      __syncwarp();
-      const uint32_t lfull0 = leader_addr(full);
+      const uint32_t lfull0 = leader_addr(full), empty0 = smem_u32(empty);
+      const int n_stage = a.n_stage;
       int st = 0; uint32_t ph = 0;
+      // one ring entry: this CTA's half (64 points) of two dwell groups of a D slab; the bytes count on the LEADER's barrier
+      auto load = [&](const CUtensorMap* map, const int c, const int gp) -> bool {
+        if (!mbar_wait1_addr(w, empty0 + 8u * (uint32_t)st, ph ^ 1, DEVERR_W_EMPTY)) return false;
+        if (leader) mbar_expect_tx(full + st, 2u * (uint32_t)kPairEntry);
+        tma_load_3d_pair(map, ring + (size_t)st * kPairEntry, lfull0 + 8u * (uint32_t)st, 0, c * kPC + rank * kHalfPC, 2 * gp, polD);
+        if (++st == n_stage) { st = 0; ph ^= 1; }
+        return true;
+      };
       for (int c = c0; c < c1; ++c) {
-        for (int g2 = 0; g2 < 3 * Gp; ++g2) {         // entries 2 p, 2 p + 1: D_lo, D_hi (corrections); 2 Gp + p: D_hi (main)
-          const int gp = g2 < 2 * Gp ? g2 >> 1 : g2 - 2 * Gp, lo = g2 < 2 * Gp ? (g2 & 1) ^ 1 : 0;
-          GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
-          if (elect_one()) {
-            if (leader) mbar_expect_tx(full + st, 2u * (uint32_t)kPairEntry);
-            tma_load_3d_pair(lo ? &tmD_lo : &tmD_hi, ring + (size_t)st * kPairEntry, lfull0 + 8u * (uint32_t)st, 0,
-                             c * kPC + rank * kHalfPC, 2 * gp, polD);
-          }
-          __syncwarp();
-          if (++st == a.n_stage) { st = 0; ph ^= 1; }
+        for (int gp = 0; gp < Gp; ++gp) {             // entries 2 p, 2 p + 1: D_lo, D_hi (corrections)
+          GMCO_WAIT(load(&tmD_lo, c, gp));
+          GMCO_WAIT(load(&tmD_hi, c, gp));
         }
+        for (int gp = 0; gp < Gp; ++gp) GMCO_WAIT(load(&tmD_hi, c, gp));   // entries 2 Gp + p: D_hi again (main product)
       }
     };
-    producer();
+    if (elect_one()) producer();                      // one lane issues every TMA load of the CTA
+    __syncwarp();
   } else if (warp == 1) {
     auto issuer = [&]() {
       if (!leader || c1 <= c0) return;
@@ -913,19 +915,19 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
       const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
-        if (elect_one()) {
+        GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));
+        {
           uint8_t* dst = smem + (size_t)st * stageBytes;
           mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
           tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
           tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);
           tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
         }
-        __syncwarp();
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
     };
-    producer();
+    if (elect_one()) producer();                      // one lane issues every TMA load of the CTA
+    __syncwarp();
   } else if (warp == 1) {
     auto issuer = [&]() {
       if (s1 <= s0) return;
@@ -1100,19 +1102,19 @@ k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ 
       const uint64_t polD = l2_evict_last(), polR = l2_evict_first();
       int st = 0; uint32_t ph = 0;
       for (int s = s0; s < s1; ++s) {
-        GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));
-        if (elect_one()) {
+        GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));
+        {
           uint8_t* dst = smem + (size_t)st * stageBytes;
           mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
           tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
           tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, rank * Gh, polD);
           tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, rank * Gh, polD);
         }
-        __syncwarp();
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
     };
-    producer();
+    if (elect_one()) producer();                      // one lane issues every TMA load of the CTA
+    __syncwarp();
   } else if (warp == 1) {
     auto issuer = [&]() {                             // run by ONE elected lane of the leader
       if (!leader || s1 <= s0) return;

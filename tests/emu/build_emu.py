@@ -106,7 +106,7 @@ def _build(force: bool, sanitize: bool) -> Path:
 # name -> (file, text to find, replacement, occurrences expected)
 MUTANTS = {
     # producer refills a ring slot without waiting for the commit of the MMAs that read it
-    "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait(w, empty + st, ph ^ 1, DEVERR_W_EMPTY));", "", 4),
+    "producer_skips_empty_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));", "", 3),
     # MMAs issued before the TMA bytes of their operands have landed
     "issuer_skips_full_wait": ("kernels_tc.cu", "GMCO_WAIT(mbar_wait1_addr(w, full0 + 8 * st, ph, DEVERR_W_FULL));", "", 2),
     # gradient MMAs issued before the converter warps have split the R tile (and before it has landed)
@@ -123,7 +123,7 @@ MUTANTS = {
     # ... and the same with the self-check gone: the emulated hardware's window check is what is left
     "host_smem_too_small_unchecked": ("*", None, None, 0),
     # producer's ring phase never flips: the second trip round the ring waits for ever -> bounded wait -> error word
-    "producer_phase_never_flips": ("kernels_tc.cu", "if (++st == a.n_stage) { st = 0; ph ^= 1; }", "if (++st == a.n_stage) { st = 0; }", 6),
+    "producer_phase_never_flips": ("kernels_tc.cu", "if (++st == a.n_stage) { st = 0; ph ^= 1; }", "if (++st == a.n_stage) { st = 0; }", 5),
     # TMEM is never given back
     "tmem_never_freed": ("kernels_tc.cu", "tc_fence_after(); tmem_dealloc(tmem, 512); }", "tc_fence_after(); }", 2),
     # the D slab of the wrong chunk is loaded (index error: wrong numbers, nothing else)
