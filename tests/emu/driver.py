@@ -210,6 +210,25 @@ def sc_sa(g, E, a):
     return report(E, accepted_gpu=out["n_accepted"].tolist(), accepted_ref=acc_ref, T_abs_err=t_err, F_rel_err=f_err)
 
 
+def sc_exact(g, E, a):
+    """Index check with exact arithmetic: D holds small integers (exact in tf32), plan k dwells for exactly 1 s at ONE
+    position a_k, so dose[i, k] must equal D[i, a_k] to the last bit on every route -- any slip in a TMA coordinate, a
+    swizzle, a descriptor or an accumulator column gives a different integer."""
+    c = custom_case(a)
+    rng = np.random.Generator(np.random.PCG64(99))
+    D = rng.integers(1, 1000, size=c.D.shape).astype(np.float32)
+    K, A = c.n_plans, c.n_dwell
+    pos = (np.arange(K) * 7 + 3) % A
+    T = np.zeros((K, A), np.float32)
+    T[np.arange(K), pos] = 1.0
+    h = g.gmco_create(D, c.structures, c.rx, options(a, c))
+    try:
+        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=False, host=True)
+    finally:
+        g.gmco_destroy(h)
+    return report(E, exact=bool(np.array_equal(out["dose"], D[:, pos])), mismatches=int((out["dose"] != D[:, pos]).sum()))
+
+
 def sc_smoke(g, E, a):
     """The call sequence of __graft_entry__.smoke() (same cases, same arguments, same bars), on the emulation."""
     c = gc.make_case("C1")
@@ -273,7 +292,7 @@ def sc_pool(g, E, a):
                   dose_rate=dict(max_ulp=int(ulp.max()), exact_fraction=float((ulp == 0).mean())))
 
 
-SCENARIOS = {"smoke": sc_smoke, "fault_sweep": sc_fault_sweep, "evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
+SCENARIOS = {"exact": sc_exact, "smoke": sc_smoke, "fault_sweep": sc_fault_sweep, "evaluate": sc_evaluate, "optimize": sc_optimize, "fault": sc_fault, "sa": sc_sa, "pool": sc_pool}
 
 
 def main():

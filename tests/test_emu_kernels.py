@@ -24,7 +24,11 @@ import sys
 from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
+import platform
+
 import pytest
+
+pytestmark = pytest.mark.skipif(platform.machine() != "x86_64", reason="tests/emu switches fibers with x86-64 assembly")
 
 ROOT = Path(__file__).resolve().parents[1]
 TOL_EVAL, TOL_F_FINAL, TOL_DVH_PP = 1e-4, 1e-3, 0.5
@@ -108,6 +112,13 @@ SCENARIOS = {
     # a lost history copy of k_step inside the device-side loop
     "fault_step_history": dict(scenario="fault", sm_count=2, drop="drop_tma", nth=377, via="optimize", iters=6),
     # ---- the other entry points ----
+    # exact-integer index checks: dose[i, k] == D[i, a_k] bit for bit
+    "exact_simt": dict(scenario="exact", precision=1, sm_count=4, n_plans=130, n_cath=5, n_pos=9, counts=[333, 65, 127, 70]),
+    "exact_resident": dict(scenario="exact", sm_count=4, n_plans=130, n_cath=5, n_pos=9, counts=[333, 65, 127, 70]),
+    "exact_pair_static": dict(scenario="exact", sm_count=4, n_plans=256, n_cath=17, n_pos=14, counts=[333, 65, 127, 70]),
+    "exact_pair_ring_odd": dict(scenario="exact", sm_count=4, n_plans=256, n_cath=16, n_pos=10, counts=[333, 65, 127, 70]),
+    "exact_streamed": dict(scenario="exact", sm_count=2, n_plans=130, n_cath=24, n_pos=16, counts=[333, 65, 127, 70]),
+    "exact_streamed_wide": dict(scenario="exact", sm_count=2, n_plans=130, n_cath=22, n_pos=16, wide_accum=1, counts=[333, 65, 127, 70]),
     "smoke": dict(scenario="smoke"),                           # the call sequence of __graft_entry__.smoke()
     "sa_fp64": dict(scenario="sa", n_plans=3, steps=300),
     "pool": dict(scenario="pool"),
@@ -273,6 +284,12 @@ def test_no_lost_completion_anywhere_can_hang_or_corrupt(results, name):
 def test_lost_history_copy_of_k_step_is_contained(results):
     r = _ok(results, "fault_step_history")
     assert r["code"] == -3 and "barrier wait did not complete" in r["error"], r["error"]
+
+
+@pytest.mark.parametrize("name", [n for n in SCENARIOS if n.startswith("exact_")])
+def test_one_hot_plans_read_the_dose_rate_matrix_back_exactly(results, name):
+    r = _ok(results, name)
+    assert r["exact"] and r["mismatches"] == 0, (name, r["mismatches"])
 
 
 def test_the_call_sequence_of_smoke_meets_its_bars(results):

@@ -15,7 +15,11 @@ import sys
 from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
+import platform
+
 import pytest
+
+pytestmark = pytest.mark.skipif(platform.machine() != "x86_64", reason="tests/emu switches fibers with x86-64 assembly")
 
 ROOT = Path(__file__).resolve().parents[1]
 STREAMED = dict(n_plans=128, n_cath=24, n_pos=16, sm_count=2, counts=[500, 100, 120, 120])   # 5-entry ring, 24 entries per chunk

@@ -105,3 +105,24 @@ def test_device_error_word_is_clear_after_a_normal_run_and_stats_name_the_kernel
         g.gmco_destroy(h)
     assert np.isfinite(out["objective"]).all()
     assert st["dose_kernel"] == 3 and st["rounds"] >= 11            # run-time-ring pair kernel; rounds that had work
+
+
+@pytest.mark.parametrize("n_cath,n_pos,n_plans,dose_kernel,prec", [(5, 9, 130, 0, 1), (5, 9, 130, 0, 0), (17, 14, 256, 0, 0), (17, 14, 256, 1, 0),
+                                                                  (16, 10, 256, 0, 0), (24, 16, 130, 0, 0)],
+                         ids=["simt", "resident", "pair_static", "forced_single", "pair_5_groups", "streamed_384"])
+def test_one_hot_plans_read_the_dose_rate_matrix_back_exactly(g, n_cath, n_pos, n_plans, dose_kernel, prec):
+    """Index check with exact arithmetic: D holds small integers (exact in tf32, every partial sum far below 2^24), plan k
+    dwells for exactly 1 s at ONE position a_k, so dose[i, k] must equal D[i, a_k] to the last bit on every route: a slip
+    in a TMA coordinate, a swizzle, a descriptor or an accumulator column gives a different integer, whatever the rounding."""
+    c = gc.make_case("C1", n_cath=n_cath, n_pos=n_pos, counts=(333, 65, 127, 70), n_plans=n_plans)
+    rng = np.random.Generator(np.random.PCG64(99))
+    D = rng.integers(1, 1000, size=c.D.shape).astype(np.float32)
+    pos = (np.arange(n_plans) * 7 + 3) % c.n_dwell
+    T = np.zeros((n_plans, c.n_dwell), np.float32)
+    T[np.arange(n_plans), pos] = 1.0
+    h = g.gmco_create(D, c.structures, c.rx, g.binding.make_options(m=c.m, dose_kernel=dose_kernel, precision=prec))
+    try:
+        out = g.gmco_evaluate(h, T, c.weights, want_dose=True, want_grad=False, host=True)
+    finally:
+        g.gmco_destroy(h)
+    assert np.array_equal(out["dose"], D[:, pos]), int((out["dose"] != D[:, pos]).sum())
