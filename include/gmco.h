@@ -40,7 +40,7 @@ extern "C" {
 #define GMCO_API
 #endif
 
-#define GMCO_VERSION 130          /* 0.1.3 */
+#define GMCO_VERSION 140          /* 0.1.4: gmco_tc_info.grad_pair, gmco_options.dose_kernel = 2 */
 #define GMCO_MAX_STRUCTS 8
 #define GMCO_MAX_HISTORY 16
 #define GMCO_MAX_CRITERIA 8

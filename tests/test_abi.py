@@ -36,7 +36,7 @@ def test_library_exports_every_declared_symbol(built_lib):
 
 def test_version_and_default_options(built_lib):
     import paper_1904_01567_b200 as g
-    assert g.gmco_version() == 130
+    assert g.gmco_version() == 140
     o = g.binding.make_options()
     assert (o.m, o.max_trials, o.precision) == (10, 20, g.GMCO_PREC_TF32X3)
     assert o.c1 == pytest.approx(1e-4) and o.eps == 0.0
