@@ -104,7 +104,7 @@ typedef struct gmco_options {
                          step halvings); 0: every plan keeps its tile            default 1        */
   int32_t dose_kernel;/* 0: automatic -- CTA pairs (tcgen05 cta_group::2) where the shape allows, else one CTA per
                          plan tile, and a gradient kernel that loads the fp32 D and derives its tf32 lo part itself;
-                         1: the round-1 kernels -- always one CTA per plan tile, D_hi / D_lo pre-split in memory.  The
+                         1: round 1's kernel choice -- always one CTA per plan tile, D_hi / D_lo pre-split in memory.  The
                          choices compute the same products; they differ in partial-sum order and in how D is split
                          (low-order bits).  gmco_stats.dose_kernel says which one ran.
                          2: as 0, and the GRADIENT contraction runs on CTA pairs as well (k_grad_tc_pair: each CTA

@@ -873,7 +873,7 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
 // kSplitD (default route): TMA brings R and the fp32 D itself (24 KB instead of 40 KB per 16-point stage on C3 -- the
 // kernel is bound by operand delivery from L2); the same warps derive D_lo = d - trunc(d) into the
 // D_lo area.  D stays where it landed: the tensor core ignores the low 13 bits of an fp32 word read as tf32, so the
-// fp32 tile IS the truncated hi part.  With kSplitD = false (gmco_options.dose_kernel = 1, the round-1 kernels) both
+// fp32 tile IS the truncated hi part.  With kSplitD = false (gmco_options.dose_kernel = 1, round 1's kernel choice) both
 // parts come pre-split (round to nearest) from memory.
 template <int PS, bool kSplitD>
 __global__ void __launch_bounds__(kThreads, 1)
