@@ -121,7 +121,7 @@ def sc_optimize(g, E, a):
         st = g.gmco_get_stats(h)
     finally:
         g.gmco_destroy(h)
-    rel_f = np.abs(out["objective"] - ref["F"]) / ref["F"]
+    rel_f = np.abs(out["objective"] - ref["F"]) / np.maximum(ref["F"], np.finfo(np.float64).tiny)     # F = 0 exactly on both sides: 0
     dvh_pp = np.abs(out["dvh"] - ref["dvh"])
     same_it = out["iters_done"] == ref["iters_done"]
     return report(E, rel_F_max=float(rel_f.max()), rel_F_same_iters_max=float(rel_f[same_it].max()) if same_it.any() else None,
