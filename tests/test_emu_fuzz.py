@@ -3,8 +3,8 @@
 delays and shared-memory alignments.  For every configuration: no violation recorded by the emulated hardware, no device
 error, nothing leaked; dose within 1e-4 of the oracle element by element; for the optimisations the iteration counts of
 the oracle and as many kernels executed as gmco_stats claims.  (Objective and gradient are held to 1e-4 only where the
-plan has a penalty worth the name: a plan that sits on its thresholds has F ~ 0 and any relative error.)  A longer run of
-the same generator (240 configurations) found no defect; its two kinds of findings were properties of the method, not
+plan has a penalty worth the name: a plan that sits on its thresholds has F ~ 0 and any relative error.)  Longer runs of
+the same generator (480 configurations) found no defect; their two kinds of findings were properties of the method, not
 of the kernels: Armijo decisions on the edge (a parabola's phi(2 alpha*) = phi(0)) flip between fp64 and 3xTF32, and
 plans with max_trials = 2 stall at different iterations."""
 import json
