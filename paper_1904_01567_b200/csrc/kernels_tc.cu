@@ -865,6 +865,30 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
   if (warp == 1) { tc_fence_after(); tmem_dealloc_pair(tmem, 512); }
 }
 
+// Converter warps of the gradient kernels: lo = d - trunc(d) of a D tile of n x 2048 bytes (this thread's 16 bytes of
+// every 2048), written to the D_lo area dBytes further on.  Four loads are in flight before the first store: the trip
+// count is a run-time value, and a load -> subtract -> store chain per iteration would cost a shared-memory latency each.
+__device__ __forceinline__ float4 lo_of_trunc(const float4 v) {
+  float4 lo;
+  lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
+  lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
+  lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
+  lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
+  return lo;
+}
+__device__ __forceinline__ void split_d_tile(uint8_t* dbase, const int dBytes) {
+  const int n = dBytes / 2048;
+  for (int i0 = 0; i0 < n; i0 += 4) {
+    float4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i0 + u < n) v[u] = *reinterpret_cast<const float4*>(dbase + (i0 + u) * 2048);
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i0 + u < n) *reinterpret_cast<float4*>(dbase + dBytes + (i0 + u) * 2048) = lo_of_trunc(v[u]);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a5 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point slabs [seg n_slabs / segs, (seg + 1) n_slabs / segs) of PS points each.
@@ -998,18 +1022,7 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
             *reinterpret_cast<float4*>(base + i * 2048) = hi;
             *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
           }
-          if (kSplitD) {                                // D_lo = d - trunc(d); element-wise, so the swizzle does not matter
-            uint8_t* dbase = base + 2 * kRBytes;
-            for (int i = 0; i < dBytes / 2048; ++i) {
-              const float4 v = *reinterpret_cast<const float4*>(dbase + i * 2048);
-              float4 lo;
-              lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-              lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-              lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-              lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
-              *reinterpret_cast<float4*>(dbase + dBytes + i * 2048) = lo;
-            }
-          }
+          if (kSplitD) split_d_tile(base + 2 * kRBytes, dBytes);   // D_lo = d - trunc(d); element-wise: the swizzle does not matter
           fence_proxy_async();
           mbar_arrive(conv + st);
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
@@ -1184,18 +1197,7 @@ k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ 
             *reinterpret_cast<float4*>(base + i * 2048) = hi;
             *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
           }
-          {                                             // D_lo = d - trunc(d) of this CTA's half slab (see k_grad_tc<PS, true>)
-            uint8_t* dbase = base + 2 * kRBytes;
-            for (int i = 0; i < dBytes / 2048; ++i) {
-              const float4 v = *reinterpret_cast<const float4*>(dbase + i * 2048);
-              float4 lo;
-              lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-              lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-              lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-              lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
-              *reinterpret_cast<float4*>(dbase + dBytes + i * 2048) = lo;
-            }
-          }
+          split_d_tile(base + 2 * kRBytes, dBytes);     // D_lo = d - trunc(d) of this CTA's half slab (see k_grad_tc<PS, true>)
           fence_proxy_async();
           mbar_arrive_cluster(l_conv + 8u * (uint32_t)st);         // releasing arrive at cluster scope
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
