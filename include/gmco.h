@@ -102,11 +102,11 @@ typedef struct gmco_options {
                          128-plan tiles every round, so a round costs what the RUNNING plans cost
                          (plans stop at different rounds: eps > 0, or unequal numbers of
                          step halvings); 0: every plan keeps its tile            default 1        */
-  int32_t dose_kernel;/* 0: automatic -- CTA pairs (tcgen05 cta_group::2) where the shape allows, else one CTA per
-                         plan tile, and a gradient kernel that loads the fp32 D and derives its tf32 lo part itself;
-                         1: round 1's kernel choice -- always one CTA per plan tile, D_hi / D_lo pre-split in memory.  The
-                         choices compute the same products; they differ in partial-sum order and in how D is split
-                         (low-order bits).  gmco_stats.dose_kernel says which one ran.
+  int32_t dose_kernel;/* 0: automatic -- the DOSE contraction runs on CTA pairs (tcgen05 cta_group::2) where the shape
+                         allows, else on one CTA per plan tile;
+                         1: round 1's kernel choice -- always one CTA per plan tile.  The choices compute the same
+                         products; they differ in partial-sum order (low-order bits).  gmco_stats.dose_kernel
+                         says which one ran.
                          2: as 0, and the GRADIENT contraction runs on CTA pairs as well (k_grad_tc_pair: each CTA
                          loads half of every D slab) where the shape allows -- at most 256 dwell positions, even
                          numbers of plan tiles and of 32-dwell groups; else as 0.  Not the default: it has run

@@ -865,41 +865,15 @@ k_dose_tc_pair(const __grid_constant__ CUtensorMap tmD_hi, const __grid_constant
   if (warp == 1) { tc_fence_after(); tmem_dealloc_pair(tmem, 512); }
 }
 
-// Converter warps of the gradient kernels: lo = d - trunc(d) of a D tile of n x 2048 bytes (this thread's 16 bytes of
-// every 2048), written to the D_lo area dBytes further on.  Four loads are in flight before the first store: the trip
-// count is a run-time value, and a load -> subtract -> store chain per iteration would cost a shared-memory latency each.
-__device__ __forceinline__ float4 lo_of_trunc(const float4 v) {
-  float4 lo;
-  lo.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-  lo.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-  lo.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-  lo.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
-  return lo;
-}
-__device__ __forceinline__ void split_d_tile(uint8_t* dbase, const int dBytes) {
-  const int n = dBytes / 2048;
-  for (int i0 = 0; i0 < n; i0 += 4) {
-    float4 v[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (i0 + u < n) v[u] = *reinterpret_cast<const float4*>(dbase + (i0 + u) * 2048);
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (i0 + u < n) *reinterpret_cast<float4*>(dbase + dBytes + (i0 + u) * 2048) = lo_of_trunc(v[u]);
-  }
-}
-
 // ---------------------------------------------------------------------------------------------
 // a5 on tensor cores.  grid = (segs, n_tiles); CTA (seg, tile) owns plans [128 tile, +128) and the
 // point slabs [seg n_slabs / segs, (seg + 1) n_slabs / segs) of PS points each.
 // Stage = [R | R_lo | D_hi | D_lo]: TMA brings R (fp32), D_hi, D_lo; warps 2-5 split R in place into its
 // tf32 parts (hi = truncation, lo = r - hi) before the MMA warp may read the stage.
-// kSplitD (default route): TMA brings R and the fp32 D itself (24 KB instead of 40 KB per 16-point stage on C3 -- the
-// kernel is bound by operand delivery from L2); the same warps derive D_lo = d - trunc(d) into the
-// D_lo area.  D stays where it landed: the tensor core ignores the low 13 bits of an fp32 word read as tf32, so the
-// fp32 tile IS the truncated hi part.  With kSplitD = false (gmco_options.dose_kernel = 1, round 1's kernel choice) both
-// parts come pre-split (round to nearest) from memory.
-template <int PS, bool kSplitD>
+// D_hi / D_lo come pre-split from memory (csrc/gmco_api.cu splits D once per case): deriving D_lo in these warps would
+// save 16 KB of TMA per stage but add 32 KB of shared-memory reads + writes to a stage that already moves 136 KB
+// through shared memory in 768 tensor-pipe cycles.
+template <int PS>
 __global__ void __launch_bounds__(kThreads, 1)
 k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmD_hi,
           const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {
@@ -947,10 +921,10 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
         GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));
         {
           uint8_t* dst = smem + (size_t)st * stageBytes;
-          mbar_expect_tx(full + st, (uint32_t)(kRBytes + (kSplitD ? 1 : 2) * dBytes));
+          mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
           tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
-          tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);      // kSplitD: the map is over the fp32 D
-          if (!kSplitD) tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
+          tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, 0, polD);
+          tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, 0, polD);
         }
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
@@ -1022,7 +996,6 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
             *reinterpret_cast<float4*>(base + i * 2048) = hi;
             *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
           }
-          if (kSplitD) split_d_tile(base + 2 * kRBytes, dBytes);   // D_lo = d - trunc(d); element-wise: the swizzle does not matter
           fence_proxy_async();
           mbar_arrive(conv + st);
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
@@ -1072,13 +1045,15 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
 
 // ---------------------------------------------------------------------------------------------
 // a5 on tensor cores, CTA-PAIR variant (tcgen05 cta_group::2; gmco_options.dose_kernel = 2, off by default: it has not
-// run on a GPU).  k_grad_tc needs 40 KB of operands per 16-point stage for 768 tensor-pipe cycles = 52 B/clk of a
-// measured 57 B/clk from L2 (profiles/r1_tma_bw.md): it is bound by operand delivery, not by the tensor pipe.  Here
-// the two CTAs of a cluster (2, 1, 1) own two adjacent plan tiles and the same point slabs.  One MMA spans both:
-// M = 256 plans (each CTA's own R tile is its half of the MN-major A operand), N = A_pad dwell positions whose D slab
-// is split between the CTAs by dwell group (each loads G / 2 groups: its half of the MN-major B operand) and, as in
-// k_grad_tc<PS, true>, arrives as the fp32 D whose lo part the converter warps derive: a CTA loads 8 + 8 = 16 KB per
-// stage on C3 (k_grad_tc: 24 KB; round 1: 40 KB) and the ring holds 6 stages instead of 4.
+// run on a GPU).  A stage of k_grad_tc moves 136 KB through shared memory (40 KB landing, 24 KB converter traffic,
+// 72 KB read by its six MMAs) in 768 tensor-pipe cycles: more than the 128 B/clk an SM's shared memory moves, and its
+// 40 KB of operands per stage are 52 B/clk of a measured 57 B/clk from L2 (profiles/r1_tma_bw.md) -- it is bound by
+// operand movement, not by the tensor pipe.  Here the two CTAs of a cluster (2, 1, 1) own two adjacent
+// plan tiles and the same point slabs.  One MMA spans both: M = 256 plans (each CTA's own R tile is its half of the
+// MN-major A operand), N = A_pad dwell positions whose D slab is split between the CTAs by dwell group (each loads
+// G / 2 groups of D_hi and of D_lo: its half of the MN-major B operand).  Per stage on C3 a CTA lands 24 KB instead of
+// 40 and its shared memory moves 96 KB instead of 136 (an MMA reads 4 + 4 KB of it instead of 4 + 8); the ring holds 6
+// stages instead of 4.
 // Each CTA's TMEM holds the accumulators of its own 128 plans (main at column 0, corrections at column 256).
 // Barriers: `full` (own CTA: bytes of its R tile and D halves), `conv` (in the leader: 256 arrivals, the converter
 // threads of both CTAs, which have waited for their own `full`), `empty` / `acc_full` (multicast commits).
@@ -1089,7 +1064,7 @@ __host__ __device__ constexpr uint32_t instr_desc_pair_mn(int n) {   // M = 256,
 template <int PS>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmD_hi,
-               const GradArgs a) {                    // tmD_hi: the map over the fp32 D (boxes of G / 2 dwell groups)
+               const __grid_constant__ CUtensorMap tmD_lo, const GradArgs a) {   // D maps: boxes of G / 2 dwell groups
   if (a.gate && *a.gate == 0) return;                 // both CTAs of a pair take every early exit together
   const int rank = (int)cluster_ctarank();
   const bool leader = rank == 0;
@@ -1121,7 +1096,7 @@ k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ 
     tmem_slot[1] = 0u;                                // abort flag
     fence_barrier_init();
   }
-  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmR); tma_prefetch_desc(&tmD_hi); }
+  if (warp == 0 && lane == 0) { tma_prefetch_desc(&tmR); tma_prefetch_desc(&tmD_hi); tma_prefetch_desc(&tmD_lo); }
   if (warp == 1) tmem_alloc_pair(tmem_slot, 512);
   tc_fence_before();
   cluster_sync_all();                                 // barriers of both CTAs exist before anything arrives on them
@@ -1136,9 +1111,10 @@ k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ 
         GMCO_WAIT(mbar_wait1_addr(w, smem_u32(empty + st), ph ^ 1, DEVERR_W_EMPTY));
         {
           uint8_t* dst = smem + (size_t)st * stageBytes;
-          mbar_expect_tx(full + st, (uint32_t)(kRBytes + dBytes));
+          mbar_expect_tx(full + st, (uint32_t)(kRBytes + 2 * dBytes));
           tma_load_3d(&tmR, dst, full + st, 0, s * PS, tile * 4, polR);
           tma_load_3d(&tmD_hi, dst + 2 * kRBytes, full + st, 0, s * PS, rank * Gh, polD);
+          tma_load_3d(&tmD_lo, dst + 2 * kRBytes + dBytes, full + st, 0, s * PS, rank * Gh, polD);
         }
         if (++st == a.n_stage) { st = 0; ph ^= 1; }
       }
@@ -1197,7 +1173,6 @@ k_grad_tc_pair(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ 
             *reinterpret_cast<float4*>(base + i * 2048) = hi;
             *reinterpret_cast<float4*>(base + kRBytes + i * 2048) = lo;
           }
-          split_d_tile(base + 2 * kRBytes, dBytes);     // D_lo = d - trunc(d) of this CTA's half slab (see k_grad_tc<PS, true>)
           fence_proxy_async();
           mbar_arrive_cluster(l_conv + 8u * (uint32_t)st);         // releasing arrive at cluster scope
           if (++st == a.n_stage) { st = 0; ph ^= 1; }
@@ -1272,10 +1247,8 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long cols,
 struct TcPlan {
   CUtensorMap dose_D_hi, dose_D_lo, dose_T_lo, dose_T;
   CUtensorMap grad_R, grad_D_hi, grad_D_lo;
-  CUtensorMap grad_D;                              // the fp32 D itself: the default gradient kernel splits it after the load
-  int grad_split_d = 1;                            // 0: gmco_options.dose_kernel = 1 (pre-split D_hi / D_lo from memory)
   CUtensorMap pair_D_hi, pair_D_lo;                // 64-point boxes of the CTA-pair dose kernel
-  CUtensorMap gpair_D;                             // the fp32 D in boxes of G / 2 dwell groups: the CTA-pair gradient kernel
+  CUtensorMap gpair_D_hi, gpair_D_lo;              // boxes of G / 2 dwell groups: the CTA-pair gradient kernel
   tcl::Schedule sch{};                             // every size the host chose (tc_layout.h)
   int* tile_seg_dev = nullptr;
   Thresholds thr{};
@@ -1293,8 +1266,7 @@ static cudaError_t tc_set_smem_caps() {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<4, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dose_tc_pair<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad_tc_pair<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, tcl::kSmemMax);
   done = e;
   return e;
@@ -1316,14 +1288,13 @@ TcPlan* tc_plan_create(const CaseDev& c, const PlanDev& p, const StructHost* sh,
             (q.tlo_resident || (p.T_lo && make_map(&t->dose_T_lo, p.T_lo, p.K_pad, c.A_pad, 128, 1, sK))) &&
             make_map(&t->grad_R, p.R, c.N_alloc, p.K_pad, q.grad_ps, 4, sMN) &&
             make_map(&t->grad_D_hi, c.D_hi, c.N_alloc, c.A_pad, q.grad_ps, G, sMN) &&
-            make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, q.grad_ps, G, sMN) &&
-            make_map(&t->grad_D, c.D, c.N_alloc, c.A_pad, q.grad_ps, G, sMN);
-  t->grad_split_d = force_single ? 0 : 1;
+            make_map(&t->grad_D_lo, c.D_lo, c.N_alloc, c.A_pad, q.grad_ps, G, sMN);
   if (q.dose_pair)
     ok = ok && make_map(&t->pair_D_hi, c.D_hi, c.N_alloc, c.A_pad, kHalfPC, 2, sK) &&
          make_map(&t->pair_D_lo, c.D_lo, c.N_alloc, c.A_pad, kHalfPC, 2, sK);
   if (q.grad_pair)
-    ok = ok && make_map(&t->gpair_D, c.D, c.N_alloc, c.A_pad, q.grad_ps, G / 2, sMN);
+    ok = ok && make_map(&t->gpair_D_hi, c.D_hi, c.N_alloc, c.A_pad, q.grad_ps, G / 2, sMN) &&
+         make_map(&t->gpair_D_lo, c.D_lo, c.N_alloc, c.A_pad, q.grad_ps, G / 2, sMN);
   if (!ok) { snprintf(err, errlen, "cuTensorMapEncodeTiled failed"); delete t; return nullptr; }
   if (q.tlo_resident) t->dose_T_lo = t->dose_T;   // the resident layout splits T in the kernel; the map is never used for a load
   cudaError_t e = tc_set_smem_caps();
@@ -1383,10 +1354,9 @@ int launch_tc_eval(const TcPlan* t, const CaseDev& c, const PlanDev& p, float* d
     ga.n_stage = q.grad_stages; ga.compact_cap = cap; ga.err = p.dev_err;
     if (q.grad_pair) {
       ga.n_stage = q.gpair_stages;
-      k_grad_tc_pair<16><<<dim3(q.n_tiles, q.segs), kThreads, q.gpair_smem, st>>>(t->grad_R, t->gpair_D, ga);
+      k_grad_tc_pair<16><<<dim3(q.n_tiles, q.segs), kThreads, q.gpair_smem, st>>>(t->grad_R, t->gpair_D_hi, t->gpair_D_lo, ga);
     } else {
-      if (t->grad_split_d) k_grad_tc<16, true><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D, t->grad_D_lo, ga);
-      else k_grad_tc<16, false><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
+      k_grad_tc<16><<<grid, kThreads, q.grad_smem, st>>>(t->grad_R, t->grad_D_hi, t->grad_D_lo, ga);
     }
     if (cudaGetLastError() != cudaSuccess) return -1;
     ++n;

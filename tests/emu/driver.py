@@ -101,7 +101,7 @@ def sc_evaluate(g, E, a):
     return report(E, errors=eval_errors(out, ref), schedule={k: int(v) for k, v in sched.items()},
                   digest=digest(out["dose"], out["F"], out["grad_x"]),
                   kernels={k: int(E.emu_counter(k.encode())) for k in ("k_dose_tc<true>", "k_dose_tc<false>", "k_dose_tc<false, true>",
-                                                                       "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16, true>", "k_grad_tc<16, false>", "k_grad_tc_pair<16>", "k_simt_dose", "k_simt_grad")})
+                                                                       "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16>", "k_grad_tc_pair<16>", "k_simt_dose", "k_simt_grad")})
 
 
 def sc_optimize(g, E, a):

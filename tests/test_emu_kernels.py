@@ -175,8 +175,7 @@ def test_every_dose_kernel_and_the_multi_chunk_paths_were_reached(results):
         r = _ok(results, name)
         assert r["kernels"][kernel] == 1 and sum(r["kernels"][k] for k in r["kernels"] if "dose" in k) == 1, (name, r["kernels"])
         if name != "simt":
-            grad = "k_grad_tc<16, false>" if name == "resident_forced_single" else "k_grad_tc<16, true>"     # dose_kernel = 1: round-1 kernels
-            assert r["kernels"][grad] == 1 and r["mma"] > 0 and r["tma"] > 0, name
+            assert r["kernels"]["k_grad_tc<16>"] == 1 and r["mma"] > 0 and r["tma"] > 0, name
             q = r["schedule"]
             assert q["n_chunks"] // q["segs"] >= 3, (name, q["n_chunks"], q["segs"])      # ring wrap-around, buffer alternation
 
@@ -186,10 +185,10 @@ def test_pair_gradient_kernel_option(results):
     sum in the same order (no compaction), reached on the shapes it is meant for, falls back where the shape forbids it."""
     for name in ("gpair_ring", "gpair_static", "gpair_static_4_tiles_ragged", "c3_full_size_gpair"):
         r = _ok(results, name)
-        assert r["kernels"]["k_grad_tc_pair<16>"] == 1 and r["kernels"]["k_grad_tc<16, true>"] == 0 and r["schedule"]["grad_pair"] == 1, name
+        assert r["kernels"]["k_grad_tc_pair<16>"] == 1 and r["kernels"]["k_grad_tc<16>"] == 0 and r["schedule"]["grad_pair"] == 1, name
     r = _ok(results, "gpair_odd_groups_falls_back")               # 7 dwell groups: the split of D by group needs an even count
-    assert r["kernels"]["k_grad_tc<16, true>"] == 1 and r["kernels"]["k_grad_tc_pair<16>"] == 0 and r["schedule"]["grad_pair"] == 0
-    # same products in the same order as k_grad_tc<16, true>: same bits
+    assert r["kernels"]["k_grad_tc<16>"] == 1 and r["kernels"]["k_grad_tc_pair<16>"] == 0 and r["schedule"]["grad_pair"] == 0
+    # same products in the same order as k_grad_tc<16>: same bits
     assert _ok(results, "gpair_static")["digest"] == _ok(results, "pair_static")["digest"]
     assert _ok(results, "gpair_ring")["digest"] == _ok(results, "pair_ring")["digest"]
     assert _ok(results, "c3_full_size_gpair")["digest"] == _ok(results, "c3_full_size")["digest"]
