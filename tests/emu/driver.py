@@ -124,7 +124,8 @@ def sc_optimize(g, E, a):
     rel_f = np.abs(out["objective"] - ref["F"]) / np.maximum(ref["F"], np.finfo(np.float64).tiny)     # F = 0 exactly on both sides: 0
     dvh_pp = np.abs(out["dvh"] - ref["dvh"])
     same_it = out["iters_done"] == ref["iters_done"]
-    return report(E, rel_F_max=float(rel_f.max()), rel_F_same_iters_max=float(rel_f[same_it].max()) if same_it.any() else None,
+    return report(E, rel_F_max=float(rel_f.max()), rel_F_median=float(np.median(rel_f)), rel_F_p99=float(np.quantile(rel_f, 0.99)),
+                  rel_F_over_1e3=int((rel_f > 1e-3).sum()), rel_F_same_iters_max=float(rel_f[same_it].max()) if same_it.any() else None,
                   dvh_pp_max=float(dvh_pp.max()), iters_gpu=out["iters_done"].tolist(), iters_ref=np.asarray(ref["iters_done"]).tolist(),
                   status_gpu=out["plan_status"].tolist(), status_ref=np.asarray(ref["status"]).tolist(),
                   rounds=int(st["rounds"]), launches=int(st["kernel_launches"]), executed=executed, dose_kernel=int(st["dose_kernel"]),
