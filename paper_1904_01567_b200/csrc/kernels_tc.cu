@@ -1046,14 +1046,14 @@ k_grad_tc(const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUten
 // ---------------------------------------------------------------------------------------------
 // a5 on tensor cores, CTA-PAIR variant (tcgen05 cta_group::2; gmco_options.dose_kernel = 2, off by default: it has not
 // run on a GPU).  A stage of k_grad_tc moves 136 KB through shared memory (40 KB landing, 24 KB converter traffic,
-// 72 KB read by its six MMAs) in 768 tensor-pipe cycles: more than the 128 B/clk an SM's shared memory moves, and its
+// 72 KB read by its six MMAs) in 768 tensor-pipe cycles = 181 B/clk, more than the 128 B/clk an SM's shared memory moves, and its
 // 40 KB of operands per stage are 52 B/clk of a measured 57 B/clk from L2 (profiles/r1_tma_bw.md) -- it is bound by
 // operand movement, not by the tensor pipe.  Here the two CTAs of a cluster (2, 1, 1) own two adjacent
 // plan tiles and the same point slabs.  One MMA spans both: M = 256 plans (each CTA's own R tile is its half of the
 // MN-major A operand), N = A_pad dwell positions whose D slab is split between the CTAs by dwell group (each loads
 // G / 2 groups of D_hi and of D_lo: its half of the MN-major B operand).  Per stage on C3 a CTA lands 24 KB instead of
-// 40 and its shared memory moves 96 KB instead of 136 (an MMA reads 4 + 4 KB of it instead of 4 + 8); the ring holds 6
-// stages instead of 4.
+// 40 and its shared memory moves 96 KB = 128 B/clk instead of 136 KB (an MMA reads 4 + 4 KB of it instead of 4 + 8);
+// the ring holds 6 stages instead of 4.
 // Each CTA's TMEM holds the accumulators of its own 128 plans (main at column 0, corrections at column 256).
 // Barriers: `full` (own CTA: bytes of its R tile and D halves), `conv` (in the leader: 256 arrivals, the converter
 // threads of both CTAs, which have waited for their own `full`), `empty` / `acc_full` (multicast commits).
