@@ -36,6 +36,8 @@ def load(lib: Path):
     E.emu_set.argtypes = [C.c_char_p, C.c_long]
     E.emu_counter.argtypes = [C.c_char_p]
     E.emu_counter.restype = C.c_long
+    E.emu_traffic.argtypes = [C.c_char_p, C.c_int]
+    E.emu_traffic.restype = C.c_long
     return g, E
 
 
@@ -100,6 +102,9 @@ def sc_evaluate(g, E, a):
         g.gmco_destroy(h)
     return report(E, errors=eval_errors(out, ref), schedule={k: int(v) for k, v in sched.items()},
                   digest=digest(out["dose"], out["F"], out["grad_x"]),
+                  # per tensor kernel that ran: [bytes landed in shared memory by TMA, bytes of it read by MMA operands, tensor-pipe cycles x SMs]
+                  traffic={k: [int(E.emu_traffic(k.encode(), w)) for w in range(3)]
+                           for k in ("k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_dose_tc<true>", "k_grad_tc<16>", "k_grad_tc_pair<16>") if E.emu_traffic(k.encode(), 2)},
                   kernels={k: int(E.emu_counter(k.encode())) for k in ("k_dose_tc<true>", "k_dose_tc<false>", "k_dose_tc<false, true>",
                                                                        "k_dose_tc_pair<4, 6>", "k_dose_tc_pair<0, 0>", "k_grad_tc<16>", "k_grad_tc_pair<16>", "k_simt_dose", "k_simt_grad")})
 

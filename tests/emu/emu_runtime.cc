@@ -13,6 +13,7 @@
 #include <time.h>
 
 #include <deque>
+#include <array>
 #include <map>
 #include <memory>
 #include <string>
@@ -49,6 +50,9 @@ static Config g_cfg;
 static int g_violations;
 static char g_violation_msg[1024];
 static long g_tma_count, g_commit_count, g_mma_count, g_hangs;
+// per kernel: bytes landed in shared memory by TMA / bulk copies, bytes of shared memory read by MMA operands, tensor-pipe
+// cycles x SMs (a kind::tf32 MMA of N columns keeps each SM it runs on busy for N / 2 cycles: profiles/r1_mma_rate.md)
+static std::map<std::string, std::array<long, 3>> g_traffic;
 struct LaunchRec { std::string name; dim3 grid, block; size_t smem; int captured; };
 static std::vector<LaunchRec> g_launches;
 static std::map<std::string, long> g_kernel_runs;
@@ -603,6 +607,7 @@ void tma_load(const CUtensorMap* map, uint32_t dst, uint32_t bar, int c0, int c1
   Cta* bar_cta = owner_of(bar, c);
   if (!bar_cta) return;
   const long id = g_tma_count++;
+  g_traffic[g->kernel][0] += (long)bytes;
   const int coord[3] = {c0, c1, c2};
   check_smem_write_issue(g, c, dst, dst + (uint32_t)bytes, "TMA load");
   asan_guard(c, dst, bytes, true);
@@ -640,6 +645,7 @@ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   if ((dst & 15u) || ((uintptr_t)src & 15u) || (bytes & 15u) || bytes == 0) { violation("%s: cp.async.bulk needs 16-byte aligned addresses and size (dst 0x%x, src %p, %u bytes)", g->kernel, dst, src, bytes); return; }
   if (!in_device(src, bytes)) { violation("%s: cp.async.bulk reads [%p, +%u) outside every device allocation", g->kernel, src, bytes); return; }
   const long id = g_tma_count++;
+  g_traffic[g->kernel][0] += (long)bytes;
   check_smem_write_issue(g, c, dst, dst + bytes, "cp.async.bulk");
   asan_guard(c, dst, bytes, true);
   Touch touch; touch.smem_w.push_back(Range{c, dst, dst + bytes});
@@ -806,6 +812,11 @@ void tc_mma(uint32_t d_tmem, bool a_in_tmem, uint32_t a_tmem, uint64_t a_desc, u
   {
     const int N = (int)((idesc >> 17) & 0x3f) << 3, a_mn = (int)(idesc >> 15) & 1, b_mn = (int)(idesc >> 16) & 1;
     const int ncta = pair ? 2 : 1;
+    {
+      std::array<long, 3>& t = g_traffic[g->kernel];
+      t[1] += (long)ncta * ((N / ncta) * 32 + (a_in_tmem ? 0 : 128 * 32));      // rows x 8 tf32 words per operand and CTA
+      t[2] += (long)ncta * (N / 2);
+    }
     auto operand = [&](const Cta* cc, uint64_t desc, bool mn, int rows) {
       const uint32_t start = (uint32_t)(desc & 0x3fff) << 4, lbo = (uint32_t)((desc >> 16) & 0x3fff) << 4, sbo = (uint32_t)((desc >> 32) & 0x3fff) << 4;
       if (!mn) touch.smem_r.push_back(Range{cc, start & ~127u, (start & ~127u) + (uint32_t)((rows + 7) / 8 - 1) * sbo + 1024u});
@@ -1138,8 +1149,12 @@ cudaError_t cudaGetDriverEntryPoint(const char* name, void** fn, unsigned long l
 #pragma GCC visibility push(default)
 int emu_violations(void) { return g_violations; }
 const char* emu_violation_message(void) { return g_violation_msg; }
-void emu_clear(void) { g_violations = 0; g_violation_msg[0] = 0; g_launches.clear(); g_kernel_runs.clear(); g_kernel_secs.clear(); g_sticky = cudaSuccess; g_last_error = cudaSuccess; g_hangs = 0; }
+void emu_clear(void) { g_traffic.clear(); g_violations = 0; g_violation_msg[0] = 0; g_launches.clear(); g_kernel_runs.clear(); g_kernel_secs.clear(); g_sticky = cudaSuccess; g_last_error = cudaSuccess; g_hangs = 0; }
 int emu_live_allocations(void) { int n = 0; for (const Alloc& a : g_allocs) n += a.p != nullptr; return n; }
+long emu_traffic(const char* kernel, int what) {     // what: 0 bytes landed, 1 bytes read by MMA operands, 2 tensor-pipe cycles x SMs
+  auto it = g_traffic.find(kernel);
+  return it == g_traffic.end() || what < 0 || what > 2 ? 0 : it->second[(size_t)what];
+}
 long emu_counter(const char* what) {
   const std::string w(what);
   if (w == "tma") return g_tma_count;

@@ -203,6 +203,20 @@ def test_pair_gradient_kernel_option(results):
     assert r["iters_gpu"] == r["iters_ref"] and r["rel_F_max"] < TOL_F_FINAL and r["dvh_pp_max"] < TOL_DVH_PP and r["grad_pair_launches"] >= 11
 
 
+def test_shared_memory_traffic_per_tensor_pipe_cycle_on_c3(results):
+    """DESIGN.md 5.2 / 5.2b argue from bytes moved through an SM's shared memory per tensor-pipe cycle.  The emulated TMA
+    and MMA units count what the kernels' own descriptors make them move on C3 (the converter warps' generic loads and
+    stores -- 24 KB per 768-cycle stage in both gradient kernels, 32 B/clk -- are not seen by them and are added by hand
+    in DESIGN.md): k_grad_tc lands 40 KB and its MMAs read 72 KB per stage, k_grad_tc_pair 24 KB and 48 KB per CTA."""
+    landed, read, cycles = _ok(results, "c3_full_size")["traffic"]["k_grad_tc<16>"]
+    assert landed / cycles == pytest.approx(40 * 1024 / 768) and read / cycles == pytest.approx(72 * 1024 / 768)
+    landed, read, cycles = _ok(results, "c3_full_size_gpair")["traffic"]["k_grad_tc_pair<16>"]
+    assert landed / cycles == pytest.approx(24 * 1024 / 768) and read / cycles == pytest.approx(48 * 1024 / 768)
+    landed, read, cycles = _ok(results, "c3_full_size")["traffic"]["k_dose_tc_pair<4, 6>"]
+    assert read / cycles == pytest.approx(320 * 1024 / 6144)                   # per 128-point chunk: 96 MMAs, 64 of them with A in TMEM
+    assert 192 * 1024 / 6144 <= landed / cycles < 1.2 * 192 * 1024 / 6144      # 12 ring entries of 16 KB per chunk + T once per CTA
+
+
 def test_c3_runs_in_the_configuration_the_bench_times(results):
     q = _ok(results, "c3_full_size")["schedule"]
     assert (q["n_tiles"], q["segs"], q["dose_kernel"], q["dose_stages"]) == (8, 18, 2, 6) and q["n_chunks"] // q["segs"] >= 5
